@@ -1,0 +1,1091 @@
+// fg_oracle.cpp — plain CPU oracle for the hot path of arXiv:1909.08015 (Volkov).
+//
+// TEST INFRASTRUCTURE ONLY.  Nothing in the product path (paper_1909_08015_b200/) may
+// include, link or call this file.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs use it.  It shares no code, header, table or constant
+// generator with the CUDA path.
+//
+// What it computes, in the paper's order and notation (PAPER.md = /root/reference/PAPER.md):
+//   O1  graphs without lepton loops, validity, enumeration
+//   O2  UV-divergent subgraphs (self-energy / vertexlike)               PAPER.md:139, fn.7 at 155
+//   O3  forests F[G], chain I[G], operator table M of R^new
+//   O4  operators A, U, L as rest-frame trace functionals
+//   O5  per-element Kirchhoff polynomials by EXPLICIT ENUMERATION of spanning trees and of
+//       spanning unicyclic subgraphs (no determinants, no matrix inverse) PAPER.md:205 (method by ref.)
+//   O6  assembly  I(z) = sum_{(F,G')} ...
+//   O7  3n -> 3n-1 variables                                              PAPER.md:222, fn.12-13
+//   O8  Hepp-sector density (13)-(14), sampling, pdf as x*2^j
+//   O9  Philox4x32-10
+//   O10 estimator (16)-(17)
+//   O11 precision: every sample in double AND in __float128
+// Readings of the points on which the paper is silent are listed in DESIGN.md ("Readings").
+//
+// Parity pins (tests/test_oracle_*.py): 1-loop 1/2 and closed form, 2-loop sum, eq.(11),
+// graph counts, matrix-tree vs determinants, int g = 1, Philox known answers, scaling limits.
+// Unpinned: 3-,4-,5-loop *values* (the paper prints none per graph) — "parity unpinned" for those
+// values; only invariants (mirror symmetry, affine-in-split, finiteness, P_n = 0) apply.
+
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <set>
+#include <string>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef __float128 quad;
+
+// ------------------------------------------------------------------------------------------
+// O9  Philox4x32-10 (Salmon et al. 2011; named in PAPER.md:370)
+// ------------------------------------------------------------------------------------------
+static void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// uniform in (0,1) from two 32-bit words: ((w0*2^32 + w1) >> 11 + 1/2) * 2^-53
+static double u01(uint32_t w0, uint32_t w1) {
+  uint64_t v = (((uint64_t)w0 << 32) | w1) >> 11;
+  return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+// the k-th uniform of sample `sid` under `seed`: call index k/2, word pair k%2
+struct UniformStream {
+  uint64_t sid, seed; uint32_t call; uint32_t w[4]; int have;
+  UniformStream(uint64_t sid_, uint64_t seed_) : sid(sid_), seed(seed_), call(0), have(0) {}
+  double next() {
+    if (have == 0) {
+      uint32_t ctr[4] = {(uint32_t)sid, (uint32_t)(sid >> 32), call, 0u};
+      uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+      philox4x32_10(ctr, key, w);
+      ++call; have = 2;
+    }
+    double u = (have == 2) ? u01(w[0], w[1]) : u01(w[2], w[3]);
+    --have;
+    return u;
+  }
+};
+
+// ------------------------------------------------------------------------------------------
+// O4 (tools)  Clifford algebra Cl(1,3): basis element gamma^S = product of gamma^mu, mu in S
+// ascending.  {gamma^mu,gamma^nu} = 2 g^{mu nu}, g = diag(+,-,-,-)
+// ------------------------------------------------------------------------------------------
+static const int G_DIAG[4] = {1, -1, -1, -1};
+struct Cl { int sign; int mask; };   // sign * gamma^mask
+static inline Cl cl_mul_right(Cl a, int mu) {   // a * gamma^mu
+  int cnt = __builtin_popcount(a.mask >> (mu + 1));   // gammas with larger index to hop over
+  if (cnt & 1) a.sign = -a.sign;
+  if ((a.mask >> mu) & 1) a.sign *= G_DIAG[mu];
+  a.mask ^= (1 << mu);
+  return a;
+}
+static inline int cl_trace(Cl a) { return a.mask == 0 ? 4 * a.sign : 0; }
+
+// explicit 4x4 Dirac matrices, used only to pin the (sign,mask) arithmetic above
+typedef std::complex<double> cplx;
+struct Mat4 { cplx m[4][4]; };
+static Mat4 mat_identity() { Mat4 r; for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) r.m[i][j] = (i == j) ? 1.0 : 0.0; return r; }
+static Mat4 mat_mul(const Mat4& a, const Mat4& b) {
+  Mat4 r;
+  for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) { cplx s = 0; for (int k = 0; k < 4; ++k) s += a.m[i][k] * b.m[k][j]; r.m[i][j] = s; }
+  return r;
+}
+static Mat4 mat_gamma(int mu) {   // Dirac representation
+  Mat4 r; for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) r.m[i][j] = 0;
+  if (mu == 0) { r.m[0][0] = 1; r.m[1][1] = 1; r.m[2][2] = -1; r.m[3][3] = -1; return r; }
+  cplx I(0, 1);
+  cplx s[2][2];
+  if (mu == 1) { s[0][0] = 0; s[0][1] = 1; s[1][0] = 1; s[1][1] = 0; }
+  if (mu == 2) { s[0][0] = 0; s[0][1] = -I; s[1][0] = I; s[1][1] = 0; }
+  if (mu == 3) { s[0][0] = 1; s[0][1] = 0; s[1][0] = 0; s[1][1] = -1; }
+  for (int i = 0; i < 2; ++i) for (int j = 0; j < 2; ++j) { r.m[i][2 + j] = s[i][j]; r.m[2 + i][j] = -s[i][j]; }
+  return r;
+}
+static cplx mat_trace(const Mat4& a) { return a.m[0][0] + a.m[1][1] + a.m[2][2] + a.m[3][3]; }
+
+// ------------------------------------------------------------------------------------------
+// O1  Graph
+// ------------------------------------------------------------------------------------------
+struct Graph {
+  int n = 0;        // loops
+  int nv = 0;       // 2n+1 vertices v_0..v_2n on the electron path
+  int x = 0;        // vertex of the external photon
+  std::vector<int> partner;            // partner[v] = other end of v's photon, -1 for v_x
+  std::vector<std::array<int, 2>> ph;  // photons (a<b), sorted by a
+  // line ids: electron line e_i=(v_{i-1},v_i), i=1..2n  -> id i-1 ; photon k -> id 2n+k
+  int nlines() const { return 3 * n; }
+};
+
+static bool graph_valid(const Graph& g) {
+  // every electron line e_i must be spanned by a photon (a <= i-1, b >= i): 1PI, no leg corrections
+  for (int i = 1; i <= 2 * g.n; ++i) {
+    bool ok = false;
+    for (auto& p : g.ph) if (p[0] <= i - 1 && p[1] >= i) ok = true;
+    if (!ok) return false;
+  }
+  return true;
+}
+
+static bool graph_make(int n, int x, const int* photons /* n pairs */, Graph& g) {
+  g.n = n; g.nv = 2 * n + 1; g.x = x;
+  g.partner.assign(g.nv, -1); g.ph.clear();
+  if (x < 0 || x >= g.nv) return false;
+  std::vector<int> seen(g.nv, 0);
+  for (int k = 0; k < n; ++k) {
+    int a = photons[2 * k], b = photons[2 * k + 1];
+    if (a > b) std::swap(a, b);
+    if (a < 0 || b >= g.nv || a == b || a == x || b == x || seen[a] || seen[b]) return false;
+    seen[a] = seen[b] = 1; g.partner[a] = b; g.partner[b] = a;
+    g.ph.push_back({a, b});
+  }
+  std::sort(g.ph.begin(), g.ph.end());
+  return graph_valid(g);
+}
+
+// all directed graphs with n loops, lexicographic in (x, sorted photons)
+static void enum_matchings(std::vector<int>& free_v, std::vector<std::array<int, 2>>& cur,
+                           std::vector<std::vector<std::array<int, 2>>>& out) {
+  if (free_v.empty()) { out.push_back(cur); return; }
+  int a = free_v[0];
+  for (size_t k = 1; k < free_v.size(); ++k) {
+    int b = free_v[k];
+    std::vector<int> rest;
+    for (size_t q = 1; q < free_v.size(); ++q) if (q != k) rest.push_back(free_v[q]);
+    cur.push_back({a, b});
+    enum_matchings(rest, cur, out);
+    cur.pop_back();
+  }
+}
+static std::vector<Graph> enumerate_graphs(int n) {
+  std::vector<Graph> res;
+  int nv = 2 * n + 1;
+  for (int x = 0; x < nv; ++x) {
+    std::vector<int> fv; for (int v = 0; v < nv; ++v) if (v != x) fv.push_back(v);
+    std::vector<std::array<int, 2>> cur; std::vector<std::vector<std::array<int, 2>>> ms;
+    enum_matchings(fv, cur, ms);
+    for (auto& m : ms) {
+      std::vector<int> flat; for (auto& p : m) { flat.push_back(p[0]); flat.push_back(p[1]); }
+      Graph g; if (graph_make(n, x, flat.data(), g)) res.push_back(g);
+    }
+  }
+  return res;
+}
+
+// ------------------------------------------------------------------------------------------
+// O2  UV-divergent subgraphs = vertex intervals [a,b]
+// ------------------------------------------------------------------------------------------
+struct Sub { int a, b; int type; /* 0 self-energy, 1 vertexlike */ bool in_chain; int nph; };
+
+static bool classify_interval(const Graph& g, int a, int b, Sub& s) {
+  int ext = 0, nin = 0;
+  for (int v = a; v <= b; ++v) {
+    int p = g.partner[v];
+    if (p < 0) ++ext;                       // v_x : external photon of G leaves
+    else if (p < a || p > b) ++ext;         // photon leaves the interval
+    else ++nin;
+  }
+  nin /= 2;
+  if (nin < 1) return false;
+  for (int i = a + 1; i <= b; ++i) {        // every electron line spanned by an internal photon
+    bool ok = false;
+    for (auto& p : g.ph) if (p[0] >= a && p[1] <= b && p[0] <= i - 1 && p[1] >= i) ok = true;
+    if (!ok) return false;
+  }
+  if (ext > 1) return false;
+  s.a = a; s.b = b; s.type = (ext == 0) ? 0 : 1; s.nph = nin;
+  s.in_chain = (s.type == 1 && g.x >= a && g.x <= b);
+  return true;
+}
+
+static bool intervals_overlap(const Sub& p, const Sub& q) {
+  bool share_line = std::max(p.a, q.a) < std::min(p.b, q.b);
+  bool nested = (p.a <= q.a && q.b <= p.b) || (q.a <= p.a && p.b <= q.b);
+  return share_line && !nested;
+}
+
+// ------------------------------------------------------------------------------------------
+// O3  forests and terms
+// ------------------------------------------------------------------------------------------
+enum Op { OP_A = 0, OP_U = 1, OP_L = 2, OP_LMU = 3 };
+struct Term { std::vector<int> members;   // indices into subs, members[0] = G
+              std::vector<int> ops;       // operator of each member
+              int gprime; int sign; };
+
+// ------------------------------------------------------------------------------------------
+// O5  element = forest member with its children shrunk
+// ------------------------------------------------------------------------------------------
+struct Tok { int kind; /* 0 chord (photon) , 1 external index, 2 slot */ int id; };
+struct Slot { int own_e;     // index into own_e of the line whose eta-row / A / A^q it shares
+              int child;     // -1 for an own electron line, else sub index of the self-energy child
+              int xiq; };    // -1 before the site of v_x, +1 after (used by the A element)
+struct Pattern { int match;                    // index into matchings
+                 uint32_t tmask;               // unmatched slots that carry gamma^0 (A_j p-hat)
+                 int qslot;                    // -1 or the unmatched slot that carries gamma^nu A^q_j
+                 double c[2]; };               // coefficient(s): [0] scalar / u ; [1] v (self-energy)
+struct Matching { std::vector<std::array<int, 2>> pairs; std::vector<int> unmatched; };
+
+struct ElemGeom {   // depends on (sub, children) only
+  int sub; std::vector<int> children;
+  std::vector<int> own_e, own_ph;              // global line ids
+  int nsites; int l;
+  std::vector<std::array<int, 2>> line_ends;   // site ends of own lines (own_e then own_ph), lower site first
+  std::vector<Tok> toks; std::vector<Slot> slots;
+  std::vector<int> vc_children;                // vertexlike children (multiply in as scalars)
+  // Kirchhoff enumeration (plan time): U = sum over complements of spanning trees
+  std::vector<std::vector<int>> Usets;         // each: l indices into own lines
+  struct BSet { std::vector<int> lines; std::vector<std::array<int, 3>> pairs; };  // pairs: (i,j,sign), i<=j own_e idx
+  std::vector<BSet> Bsets;
+  std::vector<Matching> matchings;
+};
+struct ElemNum {    // (geom, op): pattern table
+  int geom; int op; std::vector<Pattern> pats;
+};
+
+// --- Dirac strings ---------------------------------------------------------------------------
+// A "piece" of a functional:  weight * Tr[ F * X(ext = ext_mu ; q-slot = gamma^nu) ]
+struct Piece { double w; std::vector<int> F; int ext; int nu; };
+
+struct DiracCtx {
+  const std::vector<Tok>* toks; int nslots;
+  std::vector<int> role;        // per slot: -1 unit/gamma0 gap (unmatched), >=0 wick chord id, -2 fixed q gamma
+  std::vector<int> gapidx;      // per slot: index among gaps
+  int nchord_ph; int ext; int nu;
+  // DFS state
+  std::vector<int> val;         // value of chords (photon chords then wick chords), -1 unset
+  std::vector<double>* acc;     // acc[parity][cbits]
+  double trF[2][16];            // trF[p][mask] = w*Tr[F gamma0^p gamma^mask]
+  int ngaps;
+};
+
+static void dirac_dfs(DiracCtx& c, size_t pos, Cl cur, int nsp_parity, uint32_t cbits) {
+  const std::vector<Tok>& T = *c.toks;
+  if (pos == T.size()) {
+    for (int p = 0; p < 2; ++p) {
+      double t = c.trF[p][cur.mask] * cur.sign;
+      if (t != 0.0) c.acc[p][cbits] += t;
+    }
+    return;
+  }
+  const Tok& tk = T[pos];
+  if (tk.kind == 1) {                 // external index (fixed for this run)
+    int mu = c.ext;
+    dirac_dfs(c, pos + 1, cl_mul_right(cur, mu), nsp_parity ^ (mu != 0), cbits);
+    return;
+  }
+  int chord = -1;
+  if (tk.kind == 0) chord = tk.id;
+  else {
+    int r = c.role[tk.id];
+    if (r == -1) {                    // gap: remember sign picked up by a gamma^0 moved to the front
+      int gi = c.gapidx[tk.id];
+      dirac_dfs(c, pos + 1, cur, nsp_parity, cbits | ((uint32_t)nsp_parity << gi));
+      return;
+    }
+    if (r == -2) { int mu = c.nu; dirac_dfs(c, pos + 1, cl_mul_right(cur, mu), nsp_parity ^ (mu != 0), cbits); return; }
+    chord = c.nchord_ph + r;
+  }
+  if (c.val[chord] < 0) {             // first end: gamma^rho, sum over rho
+    for (int rho = 0; rho < 4; ++rho) {
+      c.val[chord] = rho;
+      dirac_dfs(c, pos + 1, cl_mul_right(cur, rho), nsp_parity ^ (rho != 0), cbits);
+    }
+    c.val[chord] = -1;
+  } else {                            // second end: gamma_rho = g_rr gamma^rho
+    int rho = c.val[chord];
+    Cl nx = cl_mul_right(cur, rho); nx.sign *= G_DIAG[rho];
+    c.val[chord] = -2 - rho;          // mark closed (so that a third use would be caught)
+    dirac_dfs(c, pos + 1, nx, nsp_parity ^ (rho != 0), cbits);
+    c.val[chord] = rho;
+  }
+}
+
+// coefficient table of one matching for a list of pieces: out[T] for all subsets T of gaps
+static void dirac_matching_table(const std::vector<Tok>& toks, int nslots, int nchord_ph,
+                                 const Matching& m, int qslot, const std::vector<Piece>& pieces,
+                                 std::vector<double>& out /* size 2^ngaps */) {
+  DiracCtx c; c.toks = &toks; c.nslots = nslots; c.nchord_ph = nchord_ph;
+  c.role.assign(nslots, -1); c.gapidx.assign(nslots, -1);
+  for (size_t k = 0; k < m.pairs.size(); ++k) { c.role[m.pairs[k][0]] = (int)k; c.role[m.pairs[k][1]] = (int)k; }
+  if (qslot >= 0) c.role[qslot] = -2;
+  int ng = 0;
+  for (int s : m.unmatched) if (s != qslot) c.gapidx[s] = ng++;
+  c.ngaps = ng;
+  size_t nT = (size_t)1 << ng;
+  out.assign(nT, 0.0);
+  std::vector<double> acc[2];
+  for (const Piece& pc : pieces) {
+    c.ext = pc.ext; c.nu = pc.nu;
+    Cl f{1, 0}; for (int mu : pc.F) f = cl_mul_right(f, mu);
+    for (int p = 0; p < 2; ++p) {
+      Cl fp = f; if (p) fp = cl_mul_right(fp, 0);
+      for (int mask = 0; mask < 16; ++mask) {
+        // Tr[F g0^p gamma^mask]: gamma^mask as ordered product
+        Cl t = fp; for (int mu = 0; mu < 4; ++mu) if ((mask >> mu) & 1) t = cl_mul_right(t, mu);
+        c.trF[p][mask] = pc.w * cl_trace(t);
+      }
+    }
+    acc[0].assign(nT, 0.0); acc[1].assign(nT, 0.0); c.acc = acc;
+    c.val.assign(nchord_ph + m.pairs.size(), -1);
+    dirac_dfs(c, 0, Cl{1, 0}, 0, 0u);
+    // Z_p(T) = sum_cbits acc[p][cbits] (-1)^{|T & cbits|};  c(T) = Z_{|T| mod 2}(T)
+    for (size_t Tm = 0; Tm < nT; ++Tm) {
+      int p = __builtin_popcount((unsigned)Tm) & 1;
+      double s = 0;
+      for (size_t cb = 0; cb < nT; ++cb) {
+        double a = acc[p][cb]; if (a == 0.0) continue;
+        s += (__builtin_popcount((unsigned)(Tm & cb)) & 1) ? -a : a;
+      }
+      out[Tm] += s;
+    }
+  }
+  // every weight is a multiple of 1/48 and every trace an integer: the exact value is k/48.
+  // Round the double sum to that rational (one rounding, independent of the order of the pieces).
+  for (size_t Tm = 0; Tm < nT; ++Tm) {
+    double k = std::nearbyint(out[Tm] * 48.0);
+    if (std::fabs(out[Tm] * 48.0 - k) > 1e-6) { std::fprintf(stderr, "fg_oracle: coefficient not a multiple of 1/48\n"); std::abort(); }
+    out[Tm] = k / 48.0;
+  }
+}
+
+// the same coefficient for ONE pattern by explicit 4x4 matrices and explicit index sums
+// (slow; pins dirac_matching_table in tests)
+static double dirac_explicit(const std::vector<Tok>& toks, int nslots, int nchord_ph, const Matching& m,
+                             int qslot, uint32_t tmask_slots, const std::vector<Piece>& pieces) {
+  std::vector<int> role(nslots, -1);
+  for (size_t k = 0; k < m.pairs.size(); ++k) { role[m.pairs[k][0]] = (int)k; role[m.pairs[k][1]] = (int)k; }
+  int nch = nchord_ph + (int)m.pairs.size();
+  Mat4 G[4]; for (int mu = 0; mu < 4; ++mu) G[mu] = mat_gamma(mu);
+  double total = 0;
+  for (const Piece& pc : pieces) {
+    long nassign = 1; for (int k = 0; k < nch; ++k) nassign *= 4;
+    cplx sum = 0;
+    for (long as = 0; as < nassign; ++as) {
+      std::vector<int> val(nch); long t = as; for (int k = 0; k < nch; ++k) { val[k] = t & 3; t >>= 2; }
+      std::vector<int> seen(nch, 0);
+      Mat4 P = mat_identity(); double metric = 1;
+      for (int mu : pc.F) P = mat_mul(P, G[mu]);
+      for (const Tok& tk : toks) {
+        if (tk.kind == 1) { P = mat_mul(P, G[pc.ext]); continue; }
+        int chord = -1;
+        if (tk.kind == 0) chord = tk.id;
+        else {
+          if (tk.id == qslot) { P = mat_mul(P, G[pc.nu]); continue; }
+          if (role[tk.id] < 0) { if ((tmask_slots >> tk.id) & 1) P = mat_mul(P, G[0]); continue; }
+          chord = nchord_ph + role[tk.id];
+        }
+        P = mat_mul(P, G[val[chord]]);
+        if (seen[chord]) metric *= G_DIAG[val[chord]];
+        seen[chord] = 1;
+      }
+      sum += metric * mat_trace(P);
+    }
+    total += pc.w * sum.real();
+  }
+  return total;
+}
+
+// O4 functionals as lists of pieces.  `printed` = the A projector exactly as stated in DESIGN.md
+// (sum over all mu != nu); otherwise its rotationally reduced form (pinned equal in tests).
+static std::vector<Piece> pieces_for(int op, int sub_type, int comp, bool qpart, bool printed) {
+  std::vector<Piece> P;
+  if (sub_type == 0) {            // self-energy, U:  u = 1/4 Tr[Sigma], v = 1/4 Tr[gamma^0 Sigma]
+    if (comp == 0) P.push_back({0.25, {}, 0, 0}); else P.push_back({0.25, {0}, 0, 0});
+    return P;
+  }
+  if (op == OP_U || op == OP_LMU) {   // a = 1/4 Tr[gamma^3 Gamma_3], Gamma_3 = -Gamma^3
+    double w = (op == OP_U) ? 0.25 : -0.25;
+    P.push_back({-w, {3}, 3, 0});
+  }
+  if (op == OP_L || op == OP_LMU) {   // a+b+c = 1/4 Tr[(1+gamma^0) Gamma_0]
+    P.push_back({0.25, {}, 0, 0}); P.push_back({0.25, {0}, 0, 0});
+  }
+  if (op == OP_A && !qpart) {       // (1/12){ Tr[gamma_mu V^mu] - Tr[(4 gamma^0 + 3) V^0] }
+    for (int mu = 0; mu < 4; ++mu) P.push_back({G_DIAG[mu] / 12.0, {mu}, mu, 0});
+    P.push_back({-4.0 / 12.0, {0}, 0, 0}); P.push_back({-3.0 / 12.0, {}, 0, 0});
+  }
+  if (op == OP_A && qpart) {        // (1/48) sum_{mu!=nu} Tr[(g0+1)[gamma_mu,gamma_nu](g0+1) T^{nu mu}]
+    if (printed) {
+      for (int mu = 0; mu < 4; ++mu) for (int nu = 0; nu < 4; ++nu) if (mu != nu) {
+        double w = 2.0 * G_DIAG[mu] * G_DIAG[nu] / 48.0;    // [g_mu,g_nu] = 2 g_mu g_nu (mu != nu), lowered
+        P.push_back({w, {0, mu, nu, 0}, mu, nu}); P.push_back({w, {0, mu, nu}, mu, nu});
+        P.push_back({w, {mu, nu, 0}, mu, nu});    P.push_back({w, {mu, nu}, mu, nu});
+      }
+    } else {                        // = 1/2 Tr[gamma^1 gamma^2 (1+gamma^0) T^{21}]
+      P.push_back({0.5, {1, 2}, 1, 2}); P.push_back({0.5, {1, 2, 0}, 1, 2});
+    }
+  }
+  return P;
+}
+
+// ------------------------------------------------------------------------------------------
+// The oracle object
+// ------------------------------------------------------------------------------------------
+struct Oracle {
+  Graph g; int merge = 0; int M = 0;
+  std::vector<std::vector<int>> var_lines;       // variable -> global line ids
+  std::vector<Sub> subs;                         // subs[0] = G
+  std::vector<std::vector<int>> forests;         // member lists (indices into subs), [0] = G
+  std::vector<Term> terms;
+  std::vector<ElemGeom> geoms; std::vector<ElemNum> nums;
+  std::map<std::vector<int>, int> geom_index, num_index;
+  // per term: for each member the (geom,num) ids
+  std::vector<std::vector<int>> term_geom, term_num;
+  // value nodes: an element together with the complete subtree below it (the operator of a
+  // vertexlike child depends on the term, so a value is identified by its whole subtree)
+  struct Node { int num; std::vector<int> kids; };   // kids aligned with geoms[].children
+  std::vector<Node> nodes; std::map<std::vector<int>, int> node_index; std::vector<int> term_top;
+  bool printed_projector = true; bool structure_only = false;
+  // density
+  double C[4] = {0.9, 0.03, 0.01, 0.06}; double D = 0.75;
+  std::vector<double> deg1, Z1, Z3; double lnZfull[4];
+
+  int build_geom(int sub, const std::vector<int>& children);
+  int build_num(int geom, int op);
+  void build_structure();
+  void build_density(const double* deg_override);
+  template <class T> T eval_point(const T* zvars, double* dbg) const;
+};
+
+static void all_matchings(int ns, std::vector<Matching>& out) {
+  // all partial matchings of {0..ns-1}
+  std::vector<int> used(ns, 0); Matching cur;
+  struct Rec { static void go(int i, int ns, std::vector<int>& used, Matching& cur, std::vector<Matching>& out) {
+    while (i < ns && used[i]) ++i;
+    if (i == ns) { out.push_back(cur); return; }
+    used[i] = 1;
+    cur.unmatched.push_back(i); go(i + 1, ns, used, cur, out); cur.unmatched.pop_back();
+    for (int j = i + 1; j < ns; ++j) if (!used[j]) {
+      used[j] = 1; cur.pairs.push_back({i, j}); go(i + 1, ns, used, cur, out); cur.pairs.pop_back(); used[j] = 0;
+    }
+    used[i] = 0;
+  } };
+  Rec::go(0, ns, used, cur, out);
+  for (auto& m : out) std::sort(m.unmatched.begin(), m.unmatched.end());
+}
+
+int Oracle::build_geom(int sub, const std::vector<int>& children) {
+  std::vector<int> key; key.push_back(sub); for (int c : children) key.push_back(c);
+  auto it = geom_index.find(key); if (it != geom_index.end()) return it->second;
+  ElemGeom E; E.sub = sub; E.children = children;
+  const Sub& S = subs[sub];
+  int n2 = 2 * g.n;
+  // sites in path order
+  struct Site { int kind; int v; int child; };   // kind 0 plain vertex, 1 vertexlike child, 2 self-energy child
+  std::vector<Site> sites; std::vector<int> site_of_vertex(g.nv, -1);
+  std::vector<int> seq;   // interleaved: site index (>=0) or ~own_e index (<0) in path order
+  int v = S.a;
+  while (v <= S.b) {
+    int ch = -1; for (int c : children) if (subs[c].a == v) ch = c;
+    int site = (int)sites.size();
+    if (ch >= 0) { sites.push_back({subs[ch].type == 1 ? 1 : 2, v, ch}); for (int w = subs[ch].a; w <= subs[ch].b; ++w) site_of_vertex[w] = site; v = subs[ch].b; }
+    else { sites.push_back({0, v, -1}); site_of_vertex[v] = site; }
+    seq.push_back(site);
+    if (v < S.b) { seq.push_back(~(int)E.own_e.size()); E.own_e.push_back(v); /* e_{v+1} has id v */ E.line_ends.push_back({site, site + 1}); }
+    ++v;
+  }
+  E.nsites = (int)sites.size();
+  // own photons: both ends in S, not both inside one child
+  std::vector<int> chord_of_photon(g.n, -1);
+  for (int k = 0; k < g.n; ++k) {
+    int a = g.ph[k][0], b = g.ph[k][1];
+    if (a < S.a || b > S.b) continue;
+    if (site_of_vertex[a] == site_of_vertex[b]) continue;    // inside one child
+    chord_of_photon[k] = (int)E.own_ph.size();
+    E.own_ph.push_back(n2 + k);
+    E.line_ends.push_back({site_of_vertex[a], site_of_vertex[b]});
+  }
+  E.l = (int)E.own_ph.size();
+  // site of the external index of S: the vertex whose photon leaves S (or v_x)
+  int ext_site = -1;
+  for (int w = S.a; w <= S.b; ++w) { int p = g.partner[w]; if (p < 0 || p < S.a || p > S.b) ext_site = site_of_vertex[w]; }
+  int xsite = (g.x >= S.a && g.x <= S.b) ? site_of_vertex[g.x] : -1;
+  // tokens in path order, then reversed (string reads from the outgoing end v_b to v_a)
+  std::vector<Tok> fw;
+  for (int s : seq) {
+    if (s >= 0) {
+      const Site& st = sites[s];
+      if (st.kind == 2) {     // self-energy child: pseudo-slot sharing the eta-row of its flanking line
+        int left_line = -1; for (size_t q = 0; q < E.own_e.size(); ++q) if (E.line_ends[q][1] == s) left_line = (int)q;
+        Slot sl; sl.own_e = left_line; sl.child = st.child; sl.xiq = (xsite >= 0) ? (s < xsite ? -1 : +1) : 0;
+        fw.push_back({2, (int)E.slots.size()}); E.slots.push_back(sl);
+      } else {
+        if (st.kind == 1) E.vc_children.push_back(st.child);
+        if (s == ext_site) fw.push_back({1, 0});
+        else {
+          // the photon attached at this site: plain vertex -> its photon; vertexlike child -> its leaving photon
+          int k = -1;
+          if (st.kind == 0) { for (int q = 0; q < g.n; ++q) if (g.ph[q][0] == st.v || g.ph[q][1] == st.v) k = q; }
+          else { for (int q = 0; q < g.n; ++q) { int a = g.ph[q][0], b = g.ph[q][1]; bool ina = (a >= subs[st.child].a && a <= subs[st.child].b), inb = (b >= subs[st.child].a && b <= subs[st.child].b); if (ina != inb) k = q; } }
+          fw.push_back({0, chord_of_photon[k]});
+        }
+      }
+    } else {
+      int q = ~s; Slot sl; sl.own_e = q; sl.child = -1;
+      sl.xiq = (xsite >= 0) ? (E.line_ends[q][1] <= xsite ? -1 : +1) : 0;
+      fw.push_back({2, (int)E.slots.size()}); E.slots.push_back(sl);
+    }
+  }
+  // reverse; slot ids are renumbered in string order
+  std::vector<Slot> rs(E.slots.rbegin(), E.slots.rend());
+  int ns = (int)E.slots.size();
+  for (auto it2 = fw.rbegin(); it2 != fw.rend(); ++it2) { Tok t = *it2; if (t.kind == 2) t.id = ns - 1 - t.id; E.toks.push_back(t); }
+  E.slots = rs;
+  // Kirchhoff enumeration over subsets of own lines (electron + photon)
+  int nl = (int)E.line_ends.size(), ne = (int)E.own_e.size(), l = E.l;
+  {
+    std::vector<int> comb(l);
+    // U: subsets S of size l whose complement is a spanning tree
+    std::vector<int> idx(l); for (int i = 0; i < l; ++i) idx[i] = i;
+    auto is_tree = [&](const std::vector<char>& removed) {
+      std::vector<int> par(E.nsites); for (int i = 0; i < E.nsites; ++i) par[i] = i;
+      auto find = [&](int a) { while (par[a] != a) a = par[a] = par[par[a]]; return a; };
+      int cnt = 0;
+      for (int q = 0; q < nl; ++q) if (!removed[q]) { int a = find(E.line_ends[q][0]), b = find(E.line_ends[q][1]); if (a == b) return false; par[a] = b; ++cnt; }
+      return cnt == E.nsites - 1;
+    };
+    if (l >= 1) {
+      while (true) {
+        std::vector<char> rem(nl, 0); for (int i = 0; i < l; ++i) rem[idx[i]] = 1;
+        if (is_tree(rem)) E.Usets.push_back(idx);
+        int i = l - 1; while (i >= 0 && idx[i] == nl - l + i) --i;
+        if (i < 0) break; ++idx[i]; for (int j = i + 1; j < l; ++j) idx[j] = idx[j - 1] + 1;
+      }
+    }
+    // U*beta_ij: subsets S' of size l-1 whose complement is spanning, connected, unicyclic;
+    // every pair of electron lines on the cycle contributes +-prod z_{S'}
+    int m1 = l - 1;
+    std::vector<int> id2(m1); for (int i = 0; i < m1; ++i) id2[i] = i;
+    while (true) {
+      std::vector<char> rem(nl, 0); for (int i = 0; i < m1; ++i) rem[id2[i]] = 1;
+      // strip leaves
+      std::vector<int> deg(E.nsites, 0); std::vector<char> alive(nl, 0);
+      for (int q = 0; q < nl; ++q) if (!rem[q]) { alive[q] = 1; ++deg[E.line_ends[q][0]]; ++deg[E.line_ends[q][1]]; }
+      // connectivity of the complement
+      std::vector<int> par(E.nsites); for (int i = 0; i < E.nsites; ++i) par[i] = i;
+      auto find = [&](int a) { while (par[a] != a) a = par[a] = par[par[a]]; return a; };
+      int ncomp = E.nsites;
+      for (int q = 0; q < nl; ++q) if (alive[q]) { int a = find(E.line_ends[q][0]), b = find(E.line_ends[q][1]); if (a != b) { par[a] = b; --ncomp; } }
+      if (ncomp == 1) {
+        bool changed = true;
+        while (changed) { changed = false; for (int q = 0; q < nl; ++q) if (alive[q]) { int a = E.line_ends[q][0], b = E.line_ends[q][1]; if (deg[a] == 1 || deg[b] == 1) { alive[q] = 0; --deg[a]; --deg[b]; changed = true; } } }
+        // remaining alive lines form the unique cycle; walk it
+        int start = -1; for (int q = 0; q < nl; ++q) if (alive[q]) { start = q; break; }
+        if (start >= 0) {
+          std::vector<int> dir(nl, 0);
+          int curv = E.line_ends[start][1]; dir[start] = +1; int prev = start; int from0 = E.line_ends[start][0];
+          while (curv != from0) {
+            int nxt = -1;
+            for (int q = 0; q < nl; ++q) if (alive[q] && q != prev && !dir[q] && (E.line_ends[q][0] == curv || E.line_ends[q][1] == curv)) { nxt = q; break; }
+            if (nxt < 0) break;
+            if (E.line_ends[nxt][0] == curv) { dir[nxt] = +1; curv = E.line_ends[nxt][1]; } else { dir[nxt] = -1; curv = E.line_ends[nxt][0]; }
+            prev = nxt;
+          }
+          ElemGeom::BSet bs; bs.lines = id2;
+          for (int i = 0; i < ne; ++i) if (dir[i]) for (int j = i; j < ne; ++j) if (dir[j]) bs.pairs.push_back({i, j, dir[i] * dir[j]});
+          if (!bs.pairs.empty()) E.Bsets.push_back(bs);
+        }
+      }
+      int i = m1 - 1; while (i >= 0 && id2[i] == nl - m1 + i) --i;
+      if (i < 0) break; ++id2[i]; for (int j = i + 1; j < m1; ++j) id2[j] = id2[j - 1] + 1;
+    }
+  }
+  all_matchings(ns, E.matchings);
+  int id = (int)geoms.size(); geoms.push_back(E); geom_index[key] = id; return id;
+}
+
+int Oracle::build_num(int geom, int op) {
+  std::vector<int> key = {geom, op};
+  auto it = num_index.find(key); if (it != num_index.end()) return it->second;
+  ElemNum N; N.geom = geom; N.op = op;
+  const ElemGeom& E = geoms[geom];
+  int st = subs[E.sub].type; int ns = (int)E.slots.size();
+  int nm = (int)E.matchings.size();
+  std::vector<std::vector<Pattern>> per(nm);
+  #pragma omp parallel for schedule(dynamic, 4)
+  for (int mi = 0; mi < nm; ++mi) {
+    const Matching& m = E.matchings[mi];
+    std::vector<double> tab0, tab1;
+    auto emit = [&](int qslot, const std::vector<double>& t0, const std::vector<double>* t1) {
+      std::vector<int> gaps; for (int s : m.unmatched) if (s != qslot) gaps.push_back(s);
+      for (size_t Tm = 0; Tm < t0.size(); ++Tm) {
+        double c0 = t0[Tm], c1 = t1 ? (*t1)[Tm] : 0.0;
+        if (c0 == 0.0 && c1 == 0.0) continue;
+        Pattern p; p.match = mi; p.qslot = qslot; p.tmask = 0; p.c[0] = c0; p.c[1] = c1;
+        for (size_t k = 0; k < gaps.size(); ++k) if ((Tm >> k) & 1) p.tmask |= (1u << gaps[k]);
+        per[mi].push_back(p);
+      }
+    };
+    if (st == 0) {
+      dirac_matching_table(E.toks, ns, E.l, m, -1, pieces_for(op, 0, 0, false, printed_projector), tab0);
+      dirac_matching_table(E.toks, ns, E.l, m, -1, pieces_for(op, 0, 1, false, printed_projector), tab1);
+      emit(-1, tab0, &tab1);
+    } else {
+      dirac_matching_table(E.toks, ns, E.l, m, -1, pieces_for(op, 1, 0, false, printed_projector), tab0);
+      emit(-1, tab0, nullptr);
+      if (op == OP_A) for (int q : m.unmatched) {
+        dirac_matching_table(E.toks, ns, E.l, m, q, pieces_for(op, 1, 0, true, printed_projector), tab0);
+        emit(q, tab0, nullptr);
+      }
+    }
+  }
+  for (int mi = 0; mi < nm; ++mi) for (auto& p : per[mi]) N.pats.push_back(p);
+  int id = (int)nums.size(); nums.push_back(N); num_index[key] = id; return id;
+}
+
+void Oracle::build_structure() {
+  int n = g.n;
+  // variables
+  var_lines.clear();
+  if (merge) {
+    for (int id = 0; id < 3 * n; ++id) {
+      if (id == g.x - 1) var_lines.push_back({g.x - 1, g.x});
+      else if (id == g.x) continue;
+      else var_lines.push_back({id});
+    }
+  } else for (int id = 0; id < 3 * n; ++id) var_lines.push_back({id});
+  M = (int)var_lines.size();
+  // subgraphs
+  subs.clear();
+  Sub G; classify_interval(g, 0, 2 * n, G); subs.push_back(G);
+  for (int a = 0; a <= 2 * n; ++a) for (int b = a + 1; b <= 2 * n; ++b) {
+    if (a == 0 && b == 2 * n) continue;
+    Sub s; if (classify_interval(g, a, b, s)) subs.push_back(s);
+  }
+  // forests: all sets of pairwise non-overlapping proper subgraphs, plus G
+  forests.clear();
+  int np = (int)subs.size() - 1;
+  for (uint32_t mask = 0; mask < (1u << np); ++mask) {
+    std::vector<int> mem = {0}; bool ok = true;
+    for (int i = 0; i < np && ok; ++i) if ((mask >> i) & 1) {
+      for (int j : mem) if (j != 0 && intervals_overlap(subs[i + 1], subs[j])) ok = false;
+      mem.push_back(i + 1);
+    }
+    if (ok) forests.push_back(mem);
+  }
+  // terms
+  terms.clear(); term_geom.clear(); term_num.clear();
+  for (auto& F : forests) {
+    std::vector<int> chain; for (int m : F) if (subs[m].in_chain) chain.push_back(m);
+    std::sort(chain.begin(), chain.end(), [&](int p, int q) { return (subs[p].b - subs[p].a) > (subs[q].b - subs[q].a); });
+    for (size_t r = 0; r < chain.size(); ++r) {
+      Term t; t.members = F; t.gprime = chain[r]; t.sign = ((F.size() - 1) % 2 == 0) ? +1 : -1;
+      for (int m : F) {
+        int op;
+        size_t pos = std::find(chain.begin(), chain.end(), m) - chain.begin();
+        if (m == chain[r]) op = OP_A;
+        else if (pos == chain.size()) op = OP_U;          // not in I[G]
+        else if (pos > r) op = OP_U;                      // G'' strictly inside G'
+        else op = (m == 0) ? OP_LMU : OP_L;               // G' strictly inside G''
+        t.ops.push_back(op);
+      }
+      terms.push_back(t);
+    }
+  }
+  // elements and value nodes
+  for (auto& t : terms) {
+    std::vector<int> tg, tn;
+    std::map<int, std::vector<int>> kids_of; std::map<int, int> num_of, op_of;
+    for (size_t k = 0; k < t.members.size(); ++k) {
+      int m = t.members[k];
+      std::vector<int> ch;
+      for (int c : t.members) if (c != m && subs[m].a <= subs[c].a && subs[c].b <= subs[m].b) {
+        bool maximal = true;
+        for (int d : t.members) if (d != m && d != c && subs[d].a <= subs[c].a && subs[c].b <= subs[d].b && subs[m].a <= subs[d].a && subs[d].b <= subs[m].b) maximal = false;
+        if (maximal) ch.push_back(c);
+      }
+      std::sort(ch.begin(), ch.end());
+      if (structure_only) continue;
+      int gi = build_geom(m, ch); tg.push_back(gi); int ni = build_num(gi, t.ops[k]); tn.push_back(ni);
+      kids_of[m] = ch; num_of[m] = ni;
+    }
+    term_geom.push_back(tg); term_num.push_back(tn);
+    if (structure_only) continue;
+    struct Rec { static int go(Oracle& o, int m, std::map<int, std::vector<int>>& kids_of, std::map<int, int>& num_of) {
+      std::vector<int> key = {num_of[m]}; std::vector<int> kids;
+      for (int c : kids_of[m]) { int id = go(o, c, kids_of, num_of); kids.push_back(id); key.push_back(id); }
+      auto it = o.node_index.find(key); if (it != o.node_index.end()) return it->second;
+      int id = (int)o.nodes.size(); o.nodes.push_back({num_of[m], kids}); o.node_index[key] = id; return id;
+    } };
+    term_top.push_back(Rec::go(*this, 0, kids_of, num_of));
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// O5/O6  evaluation at a point (T = double or __float128)
+// ------------------------------------------------------------------------------------------
+template <class T> struct Poly { T c[7]; Poly() { for (int i = 0; i < 7; ++i) c[i] = 0; } };
+template <class T> static Poly<T> pmul(const Poly<T>& a, const Poly<T>& b) { Poly<T> r; for (int i = 0; i < 7; ++i) for (int j = 0; i + j < 7; ++j) r.c[i + j] += a.c[i] * b.c[j]; return r; }
+
+template <class T> struct GeomVal { T U, W; std::vector<T> A, Aq, beta; int ne; bool done = false; };
+
+template <class T>
+T Oracle::eval_point(const T* zvars, double* dbg) const {
+  int n = g.n;
+  std::vector<T> z(3 * n);
+  for (int v = 0; v < M; ++v) for (int id : var_lines[v]) z[id] = zvars[v] / (T)(double)var_lines[v].size();
+  std::vector<GeomVal<T>> gv(geoms.size());
+  for (size_t gi = 0; gi < geoms.size(); ++gi) {
+    const ElemGeom& E = geoms[gi]; GeomVal<T>& V = gv[gi];
+    int ne = (int)E.own_e.size(); V.ne = ne;
+    auto zl = [&](int q) -> T { return q < ne ? z[E.own_e[q]] : z[E.own_ph[q - ne]]; };
+    T U = 0;
+    for (auto& S : E.Usets) { T p = 1; for (int q : S) p *= zl(q); U += p; }
+    std::vector<T> Ub(ne * ne, (T)0);
+    for (auto& bs : E.Bsets) { T p = 1; for (int q : bs.lines) p *= zl(q); for (auto& pr : bs.pairs) { if (pr[2] > 0) Ub[pr[0] * ne + pr[1]] += p; else Ub[pr[0] * ne + pr[1]] -= p; } }
+    V.U = U; V.beta.assign(ne * ne, (T)0);
+    for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) { T b = Ub[i * ne + j] / U; V.beta[i * ne + j] = b; V.beta[j * ne + i] = b; }
+    V.A.assign(ne, (T)0); V.Aq.assign(ne, (T)0);
+    // xi^q of own lines from the slots
+    std::vector<int> xiq(ne, 0); for (auto& s : E.slots) if (s.child < 0) xiq[s.own_e] = s.xiq;
+    T W = 0;
+    for (int j = 0; j < ne; ++j) {
+      T s = 0, sq = 0;
+      for (int e = 0; e < ne; ++e) { s += zl(e) * V.beta[j * ne + e]; sq += zl(e) * V.beta[j * ne + e] * (T)(0.5 * xiq[e]); }
+      V.A[j] = (T)1 - s; V.Aq[j] = (T)(0.5 * xiq[j]) - sq;
+      W += zl(j) * s;
+    }
+    V.W = W;
+  }
+  // node values (children have smaller node ids than their parents)
+  std::vector<std::array<Poly<T>, 2>> nv(nodes.size());
+  for (size_t nd = 0; nd < nodes.size(); ++nd) {
+    const ElemNum& N = nums[nodes[nd].num]; const ElemGeom& E = geoms[N.geom]; const GeomVal<T>& V = gv[N.geom];
+    int ne = V.ne; int ns = (int)E.slots.size();
+    auto node_of_child = [&](int child_sub) -> int { for (size_t q = 0; q < E.children.size(); ++q) if (E.children[q] == child_sub) return nodes[nd].kids[q]; return -1; };
+    Poly<T> acc0, acc1;
+    std::vector<T> As(ns), Aqs(ns);
+    for (int s = 0; s < ns; ++s) { As[s] = V.A[E.slots[s].own_e]; Aqs[s] = V.Aq[E.slots[s].own_e]; }
+    for (const Pattern& p : N.pats) {
+      const Matching& m = E.matchings[p.match];
+      T w = 1;
+      Poly<T> pw; pw.c[0] = 1;       // polynomial factor from self-energy children
+      bool haspoly = false;
+      auto child_poly = [&](int slot, int comp) -> const Poly<T>& { return nv[node_of_child(E.slots[slot].child)][comp]; };
+      for (auto& pr : m.pairs) {
+        w *= (T)(-0.5) * V.beta[E.slots[pr[0]].own_e * ne + E.slots[pr[1]].own_e];
+        for (int q = 0; q < 2; ++q) if (E.slots[pr[q]].child >= 0) { pw = pmul(pw, child_poly(pr[q], 1)); haspoly = true; }
+      }
+      for (int s : m.unmatched) {
+        bool isq = (s == p.qslot), inT = (p.tmask >> s) & 1;
+        if (isq) w *= Aqs[s]; else if (inT) w *= As[s];
+        if (E.slots[s].child >= 0) { pw = pmul(pw, child_poly(s, (isq || inT) ? 1 : 0)); haspoly = true; }
+      }
+      int mdeg = (int)m.pairs.size();
+      if (!haspoly) { acc0.c[mdeg] += w * (T)p.c[0]; acc1.c[mdeg] += w * (T)p.c[1]; }
+      else for (int d = 0; d + mdeg < 7; ++d) { acc0.c[d + mdeg] += w * (T)p.c[0] * pw.c[d]; acc1.c[d + mdeg] += w * (T)p.c[1] * pw.c[d]; }
+    }
+    for (int c : E.vc_children) { const Poly<T>& cp = nv[node_of_child(c)][0]; acc0 = pmul(acc0, cp); acc1 = pmul(acc1, cp); }
+    nv[nd][0] = acc0; nv[nd][1] = acc1;
+  }
+  T total = 0;
+  for (size_t ti = 0; ti < terms.size(); ++ti) {
+    const Term& t = terms[ti];
+    // assembly
+    T prodU2 = 1, WF = 0;
+    for (size_t k = 0; k < t.members.size(); ++k) { const GeomVal<T>& V = gv[term_geom[ti][k]]; prodU2 *= V.U * V.U; WF += V.W; }
+    const Poly<T>& P = nv[term_top[ti]][0];
+    T s = 0; T fact = 1;   // (n-m-1)!
+    // sum_{m=0}^{n-1} (n-m-1)! P_m / WF^{n-m}
+    std::vector<T> Winv(n + 1); Winv[0] = 1; for (int k = 1; k <= n; ++k) Winv[k] = Winv[k - 1] / WF;
+    for (int m = n - 1; m >= 0; --m) { int f = n - m - 1; fact = 1; for (int q = 2; q <= f; ++q) fact *= (T)(double)q; s += fact * P.c[m] * Winv[n - m]; }
+    T quarter = 1; for (int k = 0; k < n; ++k) quarter *= (T)(-0.25);
+    T val = (T)(double)t.sign * quarter * s / prodU2;
+    if (dbg) { dbg[ti] = (double)val; }
+    total += val;
+  }
+  if (dbg) dbg[terms.size()] = (double)nv[term_top[0]][0].c[n];   // P_n of the first term (pin: = 0)
+  if (merge) total *= zvars[g.x - 1];
+  return total;
+}
+
+// ------------------------------------------------------------------------------------------
+// O8  density
+// ------------------------------------------------------------------------------------------
+void Oracle::build_density(const double* deg_override) {
+  size_t nset = (size_t)1 << M; int n = g.n;
+  deg1.assign(nset, 0.0);
+  if (deg_override) { for (size_t s = 1; s + 1 < nset; ++s) deg1[s] = deg_override[s]; }
+  else {
+    // substitute rule (R-Deg): omega(s) = 2 loops(s) - e(s)/2 - gamma(s);
+    // subtract (omega(S)+1/2) for each maximal UV-divergent subgraph S inside s; clamp(-omega,1/2,3/2)
+    for (size_t s = 1; s + 1 < nset; ++s) {
+      std::vector<char> in(3 * n, 0);
+      for (int v = 0; v < M; ++v) if ((s >> v) & 1) for (int id : var_lines[v]) in[id] = 1;
+      int ne = 0, np = 0; std::vector<int> par(g.nv); for (int i = 0; i < g.nv; ++i) par[i] = i;
+      std::vector<char> touched(g.nv, 0);
+      auto find = [&](int a) { while (par[a] != a) a = par[a] = par[par[a]]; return a; };
+      int nl = 0, joins = 0;
+      for (int id = 0; id < 3 * n; ++id) if (in[id]) {
+        int a, b; if (id < 2 * n) { a = id; b = id + 1; ++ne; } else { a = g.ph[id - 2 * n][0]; b = g.ph[id - 2 * n][1]; ++np; }
+        touched[a] = touched[b] = 1; ++nl; int ra = find(a), rb = find(b); if (ra != rb) { par[ra] = rb; ++joins; }
+      }
+      int loops = nl - joins;
+      double omega = 2.0 * loops - 0.5 * ne - 1.0 * np;
+      std::vector<int> inside;
+      for (size_t k = 1; k < subs.size(); ++k) {
+        bool all = true;
+        for (int i = subs[k].a + 1; i <= subs[k].b; ++i) if (!in[i - 1]) all = false;
+        for (int q = 0; q < n; ++q) if (g.ph[q][0] >= subs[k].a && g.ph[q][1] <= subs[k].b && !in[2 * n + q]) all = false;
+        if (all) inside.push_back((int)k);
+      }
+      for (int k : inside) {
+        bool maximal = true;
+        for (int k2 : inside) if (k2 != k && subs[k2].a <= subs[k].a && subs[k].b <= subs[k2].b) maximal = false;
+        if (maximal) omega -= (subs[k].type == 1 ? 0.5 : 1.0);
+      }
+      double d = -omega; if (d < 0.5) d = 0.5; if (d > 1.5) d = 1.5;
+      deg1[s] = d;
+    }
+  }
+  auto buildZ = [&](double scale, std::vector<double>& Z) {
+    Z.assign(nset, 0.0); Z[0] = 1.0;
+    for (size_t s = 1; s < nset; ++s) {
+      double sum = 0.0;
+      for (int j = 0; j < M; ++j) if ((s >> j) & 1) sum = sum + Z[s ^ ((size_t)1 << j)];
+      if (s + 1 < nset) { double d = scale * deg1[s]; Z[s] = sum / d; } else Z[s] = sum;
+    }
+  };
+  buildZ(1.0, Z1); buildZ(D, Z3);
+  lnZfull[0] = std::log(Z1[nset - 1]); lnZfull[2] = std::log(Z3[nset - 1]);
+  // Deg = 1/2: Z_k = 2^k k! (k<M), Z(full) = M Z_{M-1};  Deg = |s|: Z = 1, Z(full) = M
+  double lz = 0; for (int k = 1; k < M; ++k) lz += std::log(2.0 * k);
+  lnZfull[1] = lz + std::log((double)M); lnZfull[3] = std::log((double)M);
+}
+
+struct SampleOut { int comp; uint8_t order[16]; double z[16]; double pdf_mant; int pdf_exp; bool bad; };
+
+static void sample_point(const Oracle& o, uint64_t sid, uint64_t seed, SampleOut& out) {
+  int M = o.M; size_t full = ((size_t)1 << M) - 1;
+  UniformStream us(sid, seed);
+  double uc = us.next();
+  int comp = 3; { double c = 0; for (int k = 0; k < 4; ++k) { c = c + o.C[k]; if (uc < c) { comp = k; break; } } }
+  out.comp = comp;
+  double zeta[16], deg_own[16], d1[16]; double lnu[16];
+  size_t s = full; double zprev = 1.0;
+  for (int l = 0; l < M; ++l) {
+    int cnt = __builtin_popcountll(s);
+    // Deg_1(s) = sum_j Z1(s\j) / Z1(s) for proper s
+    double tot1 = 0.0; for (int j = 0; j < M; ++j) if ((s >> j) & 1) tot1 = tot1 + o.Z1[s ^ ((size_t)1 << j)];
+    d1[l] = (l == 0) ? 0.0 : tot1 / o.Z1[s];
+    double usel = us.next();
+    int pick = -1;
+    if (comp == 0 || comp == 2) {
+      const std::vector<double>& Z = (comp == 0) ? o.Z1 : o.Z3;
+      double tot = 0.0; for (int j = 0; j < M; ++j) if ((s >> j) & 1) tot = tot + Z[s ^ ((size_t)1 << j)];
+      double r = usel * tot, cum = 0.0; int last = -1;
+      for (int j = 0; j < M; ++j) if ((s >> j) & 1) { cum = cum + Z[s ^ ((size_t)1 << j)]; last = j; if (cum > r) { pick = j; break; } }
+      if (pick < 0) pick = last;
+    } else {
+      int k = (int)(usel * (double)cnt); if (k >= cnt) k = cnt - 1;
+      for (int j = 0; j < M; ++j) if ((s >> j) & 1) { if (k == 0) { pick = j; break; } --k; }
+    }
+    double dg = (comp == 0) ? d1[l] : (comp == 1) ? 0.5 : (comp == 2) ? o.D * d1[l] : (double)cnt;
+    deg_own[l] = dg;
+    if (l == 0) { zeta[0] = 1.0; lnu[0] = 0; }
+    else { double u = us.next(); lnu[l] = std::log(u); double tau = std::pow(u, 1.0 / dg); zeta[l] = zprev * tau; }
+    zprev = zeta[l];
+    out.order[l] = (uint8_t)pick; s ^= ((size_t)1 << pick);
+  }
+  double sum = 0.0; for (int l = 0; l < M; ++l) sum = sum + zeta[l];
+  out.bad = false;
+  for (int l = 0; l < M; ++l) { double zz = zeta[l] / sum; out.z[out.order[l]] = zz; if (!(zz >= 2.2250738585072014e-308)) out.bad = true; }
+  // pdf: ln g_k = -ln Z_k(full) + sum_{l>=2} Deg_k(s_l) ln(z_l/z_{l-1}) - sum_j ln z_j
+  // with ln(z_l/z_{l-1}) = ln(tau_l) = ln(u_l)/Deg_own(s_l) and ln z_l = ln zeta_l - ln sum
+  double lnratio[16], lnz_sum = 0.0, lnzeta = 0.0;
+  for (int l = 0; l < M; ++l) { lnratio[l] = (l == 0) ? 0.0 : lnu[l] / deg_own[l]; lnzeta += lnratio[l]; lnz_sum += lnzeta; }
+  lnz_sum -= M * std::log(sum);
+  double lg[4];
+  for (int k = 0; k < 4; ++k) {
+    double e = 0.0; int cnt = M;
+    for (int l = 1; l < M; ++l) { --cnt; double dk = (k == 0) ? d1[l] : (k == 1) ? 0.5 : (k == 2) ? o.D * d1[l] : (double)cnt; e += dk * lnratio[l]; }
+    lg[k] = -o.lnZfull[k] + e - lnz_sum;
+  }
+  double mx = -1e300; for (int k = 0; k < 4; ++k) if (o.C[k] > 0 && lg[k] > mx) mx = lg[k];
+  double acc = 0.0; for (int k = 0; k < 4; ++k) if (o.C[k] > 0) acc += o.C[k] * std::exp(lg[k] - mx);
+  // g = acc * exp(mx) = mant * 2^e  with mant in [0.5,1)
+  double l2 = mx * 1.4426950408889634074; double fl = std::floor(l2);
+  int e2; double mant = std::frexp(acc * std::exp2(l2 - fl), &e2);
+  out.pdf_mant = mant; out.pdf_exp = e2 + (int)fl;
+  if (!std::isfinite(mant) || mant <= 0) out.bad = true;
+}
+
+// ------------------------------------------------------------------------------------------
+// C interface (ctypes)
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+void fgo_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
+double fgo_u01(uint32_t w0, uint32_t w1) { return u01(w0, w1); }
+
+int fgo_enumerate(int n, int* out, int cap) {   // out rows: x, then n photon pairs
+  std::vector<Graph> gs = enumerate_graphs(n);
+  int stride = 1 + 2 * n;
+  for (size_t i = 0; i < gs.size() && (int)i < cap; ++i) { out[i * stride] = gs[i].x; for (int k = 0; k < n; ++k) { out[i * stride + 1 + 2 * k] = gs[i].ph[k][0]; out[i * stride + 2 + 2 * k] = gs[i].ph[k][1]; } }
+  return (int)gs.size();
+}
+int fgo_count_undirected(int n) {
+  std::vector<Graph> gs = enumerate_graphs(n);
+  std::set<std::vector<int>> seen; int cnt = 0;
+  for (auto& g : gs) {
+    std::vector<int> a = {g.x}; for (auto& p : g.ph) { a.push_back(p[0]); a.push_back(p[1]); }
+    std::vector<std::array<int, 2>> rp; for (auto& p : g.ph) rp.push_back({2 * n - p[1], 2 * n - p[0]});
+    std::sort(rp.begin(), rp.end());
+    std::vector<int> b = {2 * n - g.x}; for (auto& p : rp) { b.push_back(p[0]); b.push_back(p[1]); }
+    std::vector<int> key = std::min(a, b);
+    if (!seen.count(key)) { seen.insert(key); ++cnt; }
+  }
+  return cnt;
+}
+
+void* fgo_create(int n, int x, const int* photons, int merge, const double* C, double D, const double* deg_override, int printed_projector, int structure_only) {
+  Oracle* o = new Oracle(); o->structure_only = structure_only != 0;
+  if (!graph_make(n, x, photons, o->g)) { delete o; return nullptr; }
+  o->merge = merge; o->printed_projector = printed_projector != 0;
+  if (C) for (int k = 0; k < 4; ++k) o->C[k] = C[k];
+  o->D = D;
+  o->build_structure();
+  if (!structure_only) o->build_density(deg_override);
+  return o;
+}
+void fgo_destroy(void* h) { delete (Oracle*)h; }
+
+// info: [M, n_subs, n_forests, n_terms, n_geoms, n_nums, total patterns]
+void fgo_info(void* h, long* out) {
+  Oracle* o = (Oracle*)h; out[0] = o->M; out[1] = (long)o->subs.size(); out[2] = (long)o->forests.size(); out[3] = (long)o->terms.size();
+  out[4] = (long)o->geoms.size(); out[5] = (long)o->nums.size(); long tp = 0; for (auto& N : o->nums) tp += (long)N.pats.size(); out[6] = tp;
+}
+void fgo_subs(void* h, int* out) { Oracle* o = (Oracle*)h; for (size_t k = 0; k < o->subs.size(); ++k) { out[4 * k] = o->subs[k].a; out[4 * k + 1] = o->subs[k].b; out[4 * k + 2] = o->subs[k].type; out[4 * k + 3] = o->subs[k].in_chain; } }
+// terms: for term t: sign, gprime, nmembers, then (member, op) pairs; returns ints written
+int fgo_terms(void* h, int* out, int cap) {
+  Oracle* o = (Oracle*)h; int w = 0;
+  for (auto& t : o->terms) { if (w + 3 + 2 * (int)t.members.size() > cap) return -1; out[w++] = t.sign; out[w++] = t.gprime; out[w++] = (int)t.members.size(); for (size_t k = 0; k < t.members.size(); ++k) { out[w++] = t.members[k]; out[w++] = t.ops[k]; } }
+  return w;
+}
+void fgo_tables(void* h, double* deg1, double* Z1) { Oracle* o = (Oracle*)h; size_t ns = (size_t)1 << o->M; for (size_t s = 0; s < ns; ++s) { if (deg1) deg1[s] = o->deg1[s]; if (Z1) Z1[s] = o->Z1[s]; } }
+
+// Kirchhoff debug: for geom gi at full-line z: U, W, and beta (ne x ne), A, Aq; returns ne
+int fgo_geom_eval(void* h, int gi, const double* zlines, double* U, double* W, double* beta, double* A, double* Aq,
+                  int* own_lines /* ne own_e ids then l own_ph ids */, int* nl_out, int* ends /* 2 per own line */, int* eta_rows_unused) {
+  Oracle* o = (Oracle*)h; (void)eta_rows_unused;
+  // evaluate through the generic path with merge disabled semantic: zlines are per LINE
+  Oracle tmp = *o; tmp.merge = 0; tmp.var_lines.clear(); for (int id = 0; id < 3 * o->g.n; ++id) tmp.var_lines.push_back({id}); tmp.M = 3 * o->g.n;
+  // replicate the geometry part of eval_point
+  const ElemGeom& E = tmp.geoms[gi]; int ne = (int)E.own_e.size();
+  auto zl = [&](int q) -> double { return q < ne ? zlines[E.own_e[q]] : zlines[E.own_ph[q - ne]]; };
+  double u = 0; for (auto& S : E.Usets) { double p = 1; for (int q : S) p *= zl(q); u += p; }
+  std::vector<double> Ub(ne * ne, 0.0);
+  for (auto& bs : E.Bsets) { double p = 1; for (int q : bs.lines) p *= zl(q); for (auto& pr : bs.pairs) Ub[pr[0] * ne + pr[1]] += pr[2] * p; }
+  for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) { beta[i * ne + j] = beta[j * ne + i] = Ub[i * ne + j] / u; }
+  std::vector<int> xiq(ne, 0); for (auto& s : E.slots) if (s.child < 0) xiq[s.own_e] = s.xiq;
+  double w = 0;
+  for (int j = 0; j < ne; ++j) { double s = 0, sq = 0; for (int e = 0; e < ne; ++e) { s += zl(e) * beta[j * ne + e]; sq += zl(e) * beta[j * ne + e] * 0.5 * xiq[e]; } A[j] = 1 - s; Aq[j] = 0.5 * xiq[j] - sq; w += zl(j) * s; }
+  *U = u; *W = w;
+  for (int q = 0; q < ne; ++q) own_lines[q] = E.own_e[q];
+  for (size_t q = 0; q < E.own_ph.size(); ++q) own_lines[ne + q] = E.own_ph[q];
+  *nl_out = (int)E.line_ends.size();
+  for (size_t q = 0; q < E.line_ends.size(); ++q) { ends[2 * q] = E.line_ends[q][0]; ends[2 * q + 1] = E.line_ends[q][1]; }
+  return ne;
+}
+
+// Dirac pin: max |fast - explicit| over up to `maxpat` patterns of every num of this oracle
+double fgo_dirac_selfcheck(void* h, int maxpat_per_num, long* n_checked) {
+  Oracle* o = (Oracle*)h; double worst = 0; long cnt = 0;
+  for (auto& N : o->nums) {
+    const ElemGeom& E = o->geoms[N.geom]; int st = o->subs[E.sub].type; int ns = (int)E.slots.size();
+    // also check a few zero coefficients: walk all (matching, T) for small cases
+    long step = std::max<long>(1, (long)N.pats.size() / std::max(1, maxpat_per_num));
+    for (size_t k = 0; k < N.pats.size(); k += step) {
+      const Pattern& p = N.pats[k];
+      for (int comp = 0; comp < (st == 0 ? 2 : 1); ++comp) {
+        auto pcs = pieces_for(N.op, st, comp, p.qslot >= 0, o->printed_projector);
+        double e = dirac_explicit(E.toks, ns, E.l, E.matchings[p.match], p.qslot, p.tmask, pcs);
+        worst = std::max(worst, std::fabs(e - p.c[comp])); ++cnt;
+      }
+    }
+  }
+  if (n_checked) *n_checked = cnt; return worst;
+}
+
+// integrand at n points (z over the M variables).  I_d: double evaluation; I_q: __float128 evaluation
+// rounded to double; flags bit0: |I_d - I_q| > max(rel_tol |I_q|, abs_tol); bit1: non-finite
+void fgo_eval(void* h, const double* z, long n, double rel_tol, double abs_tol, int do_quad, double* I_d, double* I_q, uint8_t* flags, double* term_dbg) {
+  Oracle* o = (Oracle*)h; int M = o->M; int nt = (int)o->terms.size();
+  #pragma omp parallel for schedule(dynamic, 16)
+  for (long i = 0; i < n; ++i) {
+    double d = o->eval_point<double>(z + i * M, term_dbg ? term_dbg + i * (nt + 1) : nullptr);
+    double q = d; uint8_t f = 0;
+    if (do_quad) { quad zq[16]; for (int v = 0; v < M; ++v) zq[v] = (quad)z[i * M + v]; q = (double)o->eval_point<quad>(zq, nullptr); }
+    if (!std::isfinite(d) || !std::isfinite(q)) f |= 2;
+    else if (std::fabs(d - q) > std::max(rel_tol * std::fabs(q), abs_tol)) f |= 1;
+    if (I_d) I_d[i] = d; if (I_q) I_q[i] = q; if (flags) flags[i] = f;
+  }
+}
+
+void fgo_sample(void* h, uint64_t seed, uint64_t first, long n, int32_t* comp, uint8_t* order, double* z, double* pdf_mant, int32_t* pdf_exp, uint8_t* bad) {
+  Oracle* o = (Oracle*)h; int M = o->M;
+  #pragma omp parallel for schedule(static)
+  for (long i = 0; i < n; ++i) {
+    SampleOut s; sample_point(*o, first + (uint64_t)i, seed, s);
+    if (comp) comp[i] = s.comp; for (int l = 0; l < M; ++l) { if (order) order[i * M + l] = s.order[l]; if (z) z[i * M + l] = s.z[l]; }
+    if (pdf_mant) pdf_mant[i] = s.pdf_mant; if (pdf_exp) pdf_exp[i] = s.pdf_exp; if (bad) bad[i] = s.bad;
+  }
+}
+
+// O10 estimator over samples [first, first+n): y = I/g.  use_quad: y from the __float128 integrand.
+// out: [sum_y, sum_y2, n_flagged, n_rejected, n_pdf_big_exp, mean, variance]
+void fgo_integrate(void* h, uint64_t seed, uint64_t first, long n, int use_quad, double rel_tol, double abs_tol, double* out) {
+  Oracle* o = (Oracle*)h; int M = o->M;
+  long double sy = 0, sy2 = 0; long nfl = 0, nrej = 0, nbig = 0;
+  #pragma omp parallel for schedule(dynamic, 64) reduction(+ : sy, sy2, nfl, nrej, nbig)
+  for (long i = 0; i < n; ++i) {
+    SampleOut s; sample_point(*o, first + (uint64_t)i, seed, s);
+    if (s.pdf_exp > 1023 || s.pdf_exp < -1021) ++nbig;
+    if (s.bad) { ++nrej; continue; }
+    double d = o->eval_point<double>(s.z, nullptr), val = d;
+    if (use_quad) {
+      quad zq[16]; for (int v = 0; v < M; ++v) zq[v] = (quad)s.z[v];
+      double q = (double)o->eval_point<quad>(zq, nullptr);
+      if (std::isfinite(q) && std::isfinite(d) && std::fabs(d - q) > std::max(rel_tol * std::fabs(q), abs_tol * std::ldexp(s.pdf_mant, s.pdf_exp))) ++nfl;
+      val = q;
+    }
+    if (!std::isfinite(val)) { ++nrej; continue; }
+    long double y = std::ldexp((long double)val / (long double)s.pdf_mant, -s.pdf_exp);
+    if (!std::isfinite((double)y)) { ++nrej; continue; }
+    sy += y; sy2 += y * y;
+  }
+  out[0] = (double)sy; out[1] = (double)sy2; out[2] = (double)nfl; out[3] = (double)nrej; out[4] = (double)nbig;
+  long double N = (long double)n;
+  out[5] = (double)(sy / N); out[6] = (double)(sy2 / (N * N) - sy * sy / (N * N * N));
+}
+
+int fgo_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"

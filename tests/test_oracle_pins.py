@@ -1,0 +1,332 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+Each test names the passage it pins.  PAPER.md = /root/reference/PAPER.md; "R-x" = reading x in DESIGN.md.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from conftest import golden, read_facts
+from oracle import oracle as O
+from paper_1909_08015_b200 import inputs
+
+FACTS = read_facts()
+
+
+# ---------------------------------------------------------------- O9 Philox
+def test_philox_known_answers():
+    with open(golden("philox4x32_10_kat.txt")) as f:
+        rows = [l.split() for l in f if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r if t != "->"]
+        out = O.philox(v[0:4], v[4:6])
+        assert [int(w) for w in out] == v[6:10]
+
+
+def test_uniform_mapping_open_interval():
+    assert O.u01(0, 0) == 0.5 * 2.0 ** -53
+    assert O.u01(0xFFFFFFFF, 0xFFFFFFFF) == 1.0 - 0.5 * 2.0 ** -53
+    assert O.u01(0x80000000, 0) == 0.5 + 0.5 * 2.0 ** -53
+
+
+# ---------------------------------------------------------------- O1 enumeration
+def test_graph_counts():
+    assert [len(O.enumerate_graphs(n)) for n in (1, 2, 3, 4)] == [1, 6, 50, 518]
+    assert [O.count_undirected(n) for n in (1, 2, 3, 4)] == [1, 4, 28, 269]
+
+
+def test_3213_five_loop_graphs():
+    assert len(O.enumerate_graphs(5)) == 6354
+    assert O.count_undirected(5) == int(FACTS["n_graphs_5loop_undirected"][0])
+
+
+def test_input_generator_agrees_with_oracle_enumeration():
+    for n in (1, 2, 3):
+        assert [(x, [tuple(p) for p in ph]) for x, ph in inputs.all_graphs(n)] == O.enumerate_graphs(n)
+
+
+# ---------------------------------------------------------------- O2-O3 forests: expression (11)
+def test_expression_11():
+    x = int(FACTS["eq11_x"][0])
+    ph = [tuple(int(t) for t in s.split("-")) for s in FACTS["eq11_photons"]]
+    o = O.Oracle(x, ph, structure_only=True)
+    subs = o.subs()
+    want = sorted(tuple(int(t) for t in s.split("-")) for s in FACTS["eq11_subgraphs"])
+    assert sorted((s["a"], s["b"]) for s in subs) == want
+    types = {(s["a"], s["b"]): s["type"] for s in subs}
+    assert types[(2, 3)] == "SE" and types[(5, 8)] == "SE" and types[(5, 7)] == "V" and types[(6, 8)] == "V"
+    assert types[(1, 9)] == "V" and types[(0, 10)] == "V"
+    assert o.n_forests == int(FACTS["eq11_forests"][0]) and o.n_terms == int(FACTS["eq11_terms"][0])
+    # expand (11) by hand: [A_G(1-U_b) - (L_G-U_G)A_b] (1-U_cd)(1-U_fghi)(1-U_fgh-U_ghi)
+    idx = {(s["a"], s["b"]): k for k, s in enumerate(subs)}
+    G, b, cd, fghi, fgh, ghi = (idx[k] for k in [(0, 10), (1, 9), (2, 3), (5, 8), (5, 7), (6, 8)])
+    head = [(+1, [(G, "A")]), (-1, [(G, "A"), (b, "U")]), (-1, [(G, "L-U"), (b, "A")])]
+    f1 = [(+1, []), (-1, [(cd, "U")])]
+    f2 = [(+1, []), (-1, [(fghi, "U")])]
+    f3 = [(+1, []), (-1, [(fgh, "U")]), (-1, [(ghi, "U")])]
+    want_terms = set()
+    for s0, m0 in head:
+        for s1, m1 in f1:
+            for s2, m2 in f2:
+                for s3, m3 in f3:
+                    want_terms.add((s0 * s1 * s2 * s3, tuple(sorted(m0 + m1 + m2 + m3))))
+    got = set((t["sign"], tuple(sorted(t["members"]))) for t in o.terms())
+    assert got == want_terms
+
+
+def test_four_loop_ladder_structure():          # 4 nested vertexlike, 8 forests, 20 terms
+    o = O.Oracle(4, [(0, 8), (1, 7), (2, 6), (3, 5)], structure_only=True)
+    assert o.n_subs == 4 and o.n_forests == 8 and o.n_terms == 20
+
+
+# ---------------------------------------------------------------- O4 Dirac algebra against explicit 4x4 matrices
+@pytest.mark.parametrize("n", [1, 2])
+def test_dirac_coefficients_vs_explicit_matrices(n):
+    for x, ph in inputs.all_graphs(n):
+        o = O.Oracle(x, ph)
+        worst, cnt = o.dirac_selfcheck(100000)
+        assert cnt > 0 and worst < 1e-12
+
+
+def test_dirac_coefficients_three_loop_sampled():
+    for x, ph in inputs.all_graphs(3)[::17]:
+        o = O.Oracle(x, ph, printed=False)
+        worst, cnt = o.dirac_selfcheck(12)
+        assert cnt > 0 and worst < 1e-11
+
+
+def test_projector_printed_equals_reduced():
+    # the A projector as stated (sum over mu != nu) against its rotationally reduced form
+    rng = np.random.default_rng(5)
+    for n, step in ((1, 1), (2, 1), (3, 13)):
+        for x, ph in inputs.all_graphs(n)[::step]:
+            a = O.Oracle(x, ph, printed=True); b = O.Oracle(x, ph, printed=False)
+            z = rng.dirichlet(np.ones(a.M), 8)
+            Ia = a.eval(z)[1]; Ib = b.eval(z)[1]
+            assert np.allclose(Ia, Ib, rtol=1e-12, atol=0)
+
+
+# ---------------------------------------------------------------- O5 Kirchhoff polynomials vs determinants
+def _loop_matrix(ends, ne, z):
+    """Textbook route: fundamental cycles of a spanning tree -> B = eta^T Z eta, U = det B, beta = eta B^-1 eta^T."""
+    nl = len(ends); nv = int(ends.max()) + 1
+    parent = {0: (None, None, 0)}; tree = set(); frontier = [0]
+    while frontier:
+        v = frontier.pop()
+        for q, (a, b) in enumerate(ends):
+            for (p, c, d) in ((a, b, +1), (b, a, -1)):
+                if p == v and c not in parent:
+                    parent[c] = (v, q, d); tree.add(q); frontier.append(c)
+    assert len(parent) == nv
+
+    def path_to_root(v):
+        res = {}
+        while parent[v][0] is not None:
+            p, q, d = parent[v]; res[q] = d; v = p      # line q traversed p->v has direction d
+        return res
+    chords = [q for q in range(nl) if q not in tree]
+    eta = np.zeros((nl, len(chords)))
+    for k, q in enumerate(chords):
+        a, b = ends[q]
+        eta[q, k] = 1.0                                   # a -> b along the chord, then b -> root -> a
+        pb = path_to_root(b); pa = path_to_root(a)
+        for line, d in pb.items():
+            eta[line, k] -= d
+        for line, d in pa.items():
+            eta[line, k] += d
+    B = eta.T @ np.diag(z) @ eta
+    return np.linalg.det(B), (eta @ np.linalg.inv(B) @ eta.T)[:ne, :ne]
+
+
+def test_matrix_tree_identity_and_beta():
+    rng = np.random.default_rng(11)
+    graphs = inputs.all_graphs(2) + inputs.all_graphs(3)[::7]
+    checked = 0
+    for x, ph in graphs:
+        o = O.Oracle(x, ph)
+        zl = rng.dirichlet(np.ones(3 * o.n))
+        for gi in range(o.n_geoms):
+            r = o.geom_eval(gi, zl)
+            z_own = zl[r["own"]]
+            U, beta = _loop_matrix(r["ends"], r["ne"], z_own)
+            assert abs(U - r["U"]) <= 1e-13 * abs(U)
+            assert np.allclose(beta, r["beta"], rtol=0, atol=1e-12 * np.abs(beta).max())
+            # weighted matrix-tree theorem: U = prod z * det(reduced Laplacian with weights 1/z)
+            nv = int(r["ends"].max()) + 1
+            Lap = np.zeros((nv, nv))
+            for (a, b), w in zip(r["ends"], 1.0 / z_own):
+                Lap[a, a] += w; Lap[b, b] += w; Lap[a, b] -= w; Lap[b, a] -= w
+            Umt = np.prod(z_own) * np.linalg.det(Lap[1:, 1:])
+            assert abs(Umt - r["U"]) <= 1e-11 * abs(Umt)
+            # A_j = 1 - sum_e z_e beta_je and W = sum z z beta ("element")
+            ze = z_own[:r["ne"]]
+            assert np.allclose(r["A"], 1 - beta @ ze, atol=1e-12)
+            assert abs(r["W"] - ze @ beta @ ze) < 1e-12
+            checked += 1
+    assert checked > 30
+
+
+# ---------------------------------------------------------------- O5-O6 integrand
+def test_one_loop_closed_form_and_merged_form():     # I = z_gamma/(1-z_gamma); merged: z_gamma
+    rng = np.random.default_rng(2)
+    o = O.Oracle(1, [(0, 2)]); z = rng.dirichlet(np.ones(3), 64)
+    Id, Iq, fl, td = o.eval(z, terms=True)
+    assert np.allclose(Iq, z[:, 2] / (1 - z[:, 2]), rtol=1e-14) and np.allclose(Id, Iq, rtol=1e-13) and not fl.any()
+    assert np.all(td[:, -1] == 0.0)                  # P_n = 0
+    om = O.Oracle(1, [(0, 2)], merge=True); zz = rng.dirichlet(np.ones(2), 64)
+    assert om.M == 2
+    assert np.allclose(om.eval(zz)[1], zz[:, 1], rtol=1e-14)
+
+
+def test_one_loop_value_is_one_half():
+    o = O.Oracle(1, [(0, 2)])
+    r = o.integrate(1, 0, 400000)
+    assert abs(r["mean"] - float(FACTS["A1_2"][0])) < 4 * math.sqrt(r["variance"])
+    assert math.sqrt(r["variance"]) < 2e-3
+
+
+def test_two_loop_sum():                             # PAPER.md:28 minus the closed-form VP-insertion graph
+    target = float(FACTS["A1_4"][0]) - (119.0 / 36.0 - math.pi ** 2 / 3.0)
+    assert abs((119.0 / 36.0 - math.pi ** 2 / 3.0) - float(FACTS["A1_4_vp_closed"][0])) < 1e-11
+    tot = var = 0.0
+    for x, ph in inputs.all_graphs(2):
+        r = O.Oracle(x, ph).integrate(1, 0, 1500000)
+        tot += r["mean"]; var += r["variance"]
+    assert math.sqrt(var) < 0.012
+    assert abs(tot - target) < 4 * math.sqrt(var)
+
+
+@pytest.mark.parametrize("n,step", [(2, 1), (3, 6)])
+def test_pointwise_invariants(n, step):
+    """Mirror symmetry, homogeneity of degree -3n, P_n = 0, affine-in-split and the exact merge (O7)."""
+    rng = np.random.default_rng(3)
+    for x, ph in inputs.all_graphs(n)[::step]:
+        o = O.Oracle(x, ph); xm, pm = inputs.mirror(x, ph); om = O.Oracle(xm, pm)
+        z = rng.dirichlet(np.ones(o.M), 6)
+        Id, Iq, fl, td = o.eval(z, terms=True)
+        ne = 2 * n
+        phs = sorted(ph); phm = [(2 * n - b, 2 * n - a) for a, b in phs]; order = sorted(range(n), key=lambda k: phm[k])
+        zm = np.concatenate([z[:, :ne][:, ::-1], z[:, ne:][:, order]], axis=1)
+        assert np.allclose(om.eval(zm)[1], Iq, rtol=1e-11)
+        assert np.allclose(o.eval(2 * z)[1] * 2.0 ** (3 * n), Iq, rtol=1e-13)
+        assert np.all(np.abs(td[:, -1]) < 1e-9 * np.abs(td[:, :-1]).max())
+        s = z[:, x - 1] + z[:, x]; vals = []
+        for f in (0.2, 0.5, 0.8):
+            zz = z.copy(); zz[:, x - 1] = f * s; zz[:, x] = (1 - f) * s; vals.append(o.eval(zz)[1])
+        assert np.all(np.abs(vals[0] - 2 * vals[1] + vals[2]) < 1e-11 * np.abs(vals[1]))
+        og = O.Oracle(x, ph, merge=True)
+        zg = np.delete(z, x, axis=1); zg[:, x - 1] = s
+        assert og.M == 3 * n - 1
+        assert np.allclose(og.eval(zg)[1], s * vals[1], rtol=1e-13)
+
+
+def test_merge_gives_the_same_integral():            # PAPER.md:222, fn.12; 3n-1 variables
+    x, ph = 2, [(0, 4), (1, 3)]
+    a = O.Oracle(x, ph).integrate(7, 0, 600000); b = O.Oracle(x, ph, merge=True).integrate(7, 0, 600000)
+    assert abs(a["mean"] - b["mean"]) < 4 * math.sqrt(a["variance"] + b["variance"])
+    assert O.Oracle(4, [(0, 10), (1, 9), (2, 3), (5, 7), (6, 8)], merge=True, structure_only=True).M - 1 == 13
+
+
+def test_subtracted_integrand_bounded_under_scaling_limits():
+    """|I| prod(z) ~ eps^d(s) with d(s) > 0 when the lines of any subset s are scaled by eps -> 0 (UV) —
+    and likewise when they are scaled up (IR), i.e. the complement scaled down."""
+    rng = np.random.default_rng(4)
+    for x, ph in inputs.all_graphs(2):
+        o = O.Oracle(x, ph); M = o.M
+        z0 = rng.dirichlet(np.ones(M))
+        pts = []
+        for s in range(1, (1 << M) - 1):
+            for eps in (1e-3, 1e-5):
+                z = z0.copy()
+                for j in range(M):
+                    if (s >> j) & 1:
+                        z[j] *= eps
+                pts.append(z / z.sum())
+        pts = np.array(pts)
+        Iq = o.eval(pts)[1]
+        f = np.abs(Iq) * np.prod(pts, axis=1)
+        f = f.reshape(-1, 2)
+        expo = np.log10(f[:, 0] / f[:, 1]) / 2.0
+        assert np.all(np.isfinite(expo)) and expo.min() > 0.4, (x, ph, expo.min())
+
+
+# ---------------------------------------------------------------- O8 density
+@pytest.mark.parametrize("x,ph,merge", [(1, [(0, 2)], False), (2, [(0, 3), (1, 4)], False), (1, [(0, 4), (2, 3)], True),
+                                        (3, [(0, 5), (1, 4), (2, 6)], True)])
+def test_density_integrates_to_one(x, ph, merge):
+    o = O.Oracle(x, ph, merge=merge); N = 400000
+    s = o.sample(3, 0, N)
+    assert not s["bad"].any()
+    w = math.factorial(o.M - 1) / (s["pdf_mant"] * np.exp2(s["pdf_exp"].astype(np.float64)))
+    assert abs(w.mean() - 1.0) < 5 * w.std() / math.sqrt(N)
+    assert np.allclose(s["z"].sum(axis=1), 1.0, atol=1e-14)
+    # the stored order is the descending order of z (Hepp sector)
+    zs = np.take_along_axis(s["z"], s["order"].astype(np.int64), axis=1)
+    assert np.all(np.diff(zs, axis=1) <= 0)
+    assert np.all((s["pdf_mant"] >= 0.5) & (s["pdf_mant"] < 1.0))
+
+
+def test_each_mixture_component_is_normalised():
+    x, ph = 2, [(0, 4), (1, 3)]
+    for k in range(4):
+        C4 = [0.0] * 4; C4[k] = 1.0
+        o = O.Oracle(x, ph, C4=C4); N = 300000
+        s = o.sample(9, 0, N)
+        assert np.all(s["comp"] == k)
+        w = math.factorial(o.M - 1) / (s["pdf_mant"] * np.exp2(s["pdf_exp"].astype(np.float64)))
+        assert abs(w.mean() - 1.0) < 5 * w.std() / math.sqrt(N)
+
+
+def test_sector_frequencies_follow_Z_table():
+    x, ph = 1, [(0, 3), (2, 4)]
+    o = O.Oracle(x, ph, C4=[1, 0, 0, 0]); N = 300000
+    deg, Z = o.tables(); M = o.M; full = (1 << M) - 1
+    s = o.sample(5, 0, N)
+    first = np.bincount(s["order"][:, 0], minlength=M) / N
+    want = np.array([Z[full ^ (1 << j)] for j in range(M)]) / Z[full]
+    assert np.allclose(first, want, atol=5 * np.sqrt(want / N))
+    # Z recursion (R-sampler): Z(s) = sum_j Z(s\j)/Deg(s)
+    for st in (0b000111, 0b101010, 0b011111):
+        tot = sum(Z[st ^ (1 << j)] for j in range(M) if (st >> j) & 1)
+        assert abs(Z[st] - tot / deg[st]) < 1e-15 * Z[st]
+
+
+def test_deg_equal_size_gives_Z_equal_one():
+    M = 6
+    table = np.array([bin(s).count("1") for s in range(1 << M)], dtype=np.float64)
+    o = O.Oracle(2, [(0, 3), (1, 4)], deg_table=table)
+    deg, Z = o.tables()
+    assert np.all(Z[:-1] == 1.0) and Z[-1] == M
+
+
+def test_mixture_constants_calc2():
+    Cs = [float(v) for v in FACTS["calc2_C"]]
+    assert abs(Cs[0] - (1 - Cs[1] - Cs[2] - Cs[3])) < 1e-15
+    o = O.Oracle(1, [(0, 2)]); s = o.sample(1, 0, 200000)
+    freq = np.bincount(s["comp"], minlength=4) / 200000
+    assert np.allclose(freq, Cs, atol=5 * np.sqrt(np.array(Cs) / 200000))
+
+
+# ---------------------------------------------------------------- O10 estimator (16)-(17)
+def test_estimator_formulas():
+    o = O.Oracle(1, [(0, 2)]); N = 50000
+    r = o.integrate(2, 100, N)
+    s = o.sample(2, 100, N); Iq = o.eval(s["z"])[0]
+    y = Iq / (s["pdf_mant"] * np.exp2(s["pdf_exp"].astype(np.float64)))
+    assert abs(r["sum_y"] - y.sum()) < 1e-9 * abs(y.sum())
+    assert abs(r["mean"] - y.sum() / N) < 1e-12
+    assert abs(r["variance"] - ((y ** 2).sum() / N ** 2 - y.sum() ** 2 / N ** 3)) < 1e-12 * r["variance"] + 1e-18
+    a = o.integrate(2, 100, N // 2); b = o.integrate(2, 100 + N // 2, N // 2)     # counter-based: ranges add up
+    assert abs(a["sum_y"] + b["sum_y"] - r["sum_y"]) < 1e-9 * abs(r["sum_y"])
+
+
+# ---------------------------------------------------------------- O11 precision
+def test_double_and_quad_agree_on_typical_points():
+    o = O.Oracle(4, [(0, 6), (1, 5), (2, 3)])
+    s = o.sample(1, 0, 3000)
+    Id, Iq, fl = o.eval(s["z"], rel_tol=1e-9)
+    assert fl.mean() < 0.2
+    ok = fl == 0
+    assert np.all(np.abs(Id[ok] - Iq[ok]) <= 1e-9 * np.abs(Iq[ok]))
