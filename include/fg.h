@@ -1,0 +1,143 @@
+/* fg.h — C ABI of the B200-native Monte-Carlo integrator for divergence-subtracted QED vertex graphs
+ * without lepton loops (hot path of arXiv:1909.08015; PAPER.md = /root/reference/PAPER.md).
+ *
+ * One path: graph -> plan (host combinatorics + tables) -> fg_integrate (one sm_100a kernel pass
+ * per precision rung: Philox -> Hepp-sector sample + pdf -> all forest terms of the integrand ->
+ * conditioning check -> y = I/g -> compensated sums -> block reduce) -> mean, variance, counters.
+ *
+ * Conventions
+ *  - every call returns int: 0 = FG_OK, negative = error code; fg_strerror(code) names it and
+ *    fg_last_error_message() (thread-local) has the detail.  No exception crosses the ABI.
+ *  - handles (fg_graph, fg_plan) are opaque, owned by the caller, released by *_destroy.
+ *  - pointer arguments are HOST pointers unless the name ends in _dev; inputs are borrowed for the
+ *    duration of the call only; outputs are written through caller-provided pointers.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls that return
+ *    results to host memory synchronise that stream before returning.
+ *  - there is NO CPU compute path: every entry point that evaluates anything launches CUDA kernels
+ *    and fails with FG_E_CUDA when no device is usable.
+ */
+#ifndef FG_H_
+#define FG_H_
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FG_OK 0
+#define FG_E_ARG -1       /* NULL / out-of-range argument */
+#define FG_E_COUNT -2     /* need 2n electron + n photon lines on 2n+1 vertices, 1 <= n <= 5 */
+#define FG_E_NOT_PATH -3  /* electron lines are not one simple open path v_0..v_2n (lepton loop or broken line) */
+#define FG_E_VERTEX -4    /* a vertex without exactly one photon (internal or the external one) */
+#define FG_E_NOT_1PI -5   /* an electron line not spanned by a photon: not 1PI / leg correction */
+#define FG_E_LOOPS -6     /* n > 5 */
+#define FG_E_CUDA -7      /* CUDA runtime error or no device */
+#define FG_E_LIMIT -8     /* an internal table limit was exceeded */
+#define FG_E_OPTS -9      /* invalid plan options */
+
+typedef struct fg_graph fg_graph;
+typedef struct fg_plan fg_plan;
+
+/* Internal line of the graph.  kind 0 = electron, 1 = photon.  Vertices are numbered along the electron path:
+ * electron line i (i = 1..2n) joins v_{i-1} and v_i.  The Feynman parameters z follow the canonical line order
+ * "electron lines e_1..e_2n, then photons sorted by their lower end" (eq. (12)). */
+typedef struct { int32_t u, v; int32_t kind; } fg_edge;
+
+/* Build a graph from its internal lines and the vertex of the external photon. */
+int fg_graph_create(const fg_edge* edges, int32_t n_edges, int32_t ext_photon_vertex, fg_graph** out);
+void fg_graph_destroy(fg_graph*);
+
+/* Plan options.  fg_plan_opts_default fills the Calc-2 constants of PAPER.md:370-377.
+ *  C[4]      mixture weights C_1..C_4 of g = sum C_k g_k; must be >= 0 and sum to 1
+ *  D         exponent scale of the third component
+ *  merge_ext_lines  1: the two electron lines at the external-photon vertex share one variable, M = 3n-1
+ *            (fn.12); 0: M = 3n
+ *  deg_table optional host array of 2^M doubles overriding Deg(s); NULL = built-in rule
+ *  rel_tol, abs_tol  a sample whose estimated round-off error exceeds max(rel_tol*|I|, abs_tol*g) is
+ *            re-evaluated in double-double (abs_tol plays the role of sigma/4 in (18))
+ *  err_factor safety factor of the running error estimate (0 = default)                                   */
+typedef struct {
+  double C[4];
+  double D;
+  int32_t merge_ext_lines;
+  int32_t reserved;
+  const double* deg_table;
+  double rel_tol, abs_tol;
+  double err_factor;
+} fg_plan_opts;
+void fg_plan_opts_default(fg_plan_opts* o);
+
+/* Host: UV-divergent subgraphs, forests, operator table, element instances, Dirac coefficient tables, Deg/Z
+ * tables; then uploads them to `device`.  "fg_plan" in BASELINE.json. */
+int fg_plan_create(const fg_graph*, const fg_plan_opts*, int32_t device, fg_plan** out);
+void fg_plan_destroy(fg_plan*);
+
+typedef struct {
+  int32_t n_loops, M;                 /* loops, number of Feynman variables */
+  int32_t n_subgraphs, n_forests, n_terms;       /* UV-divergent subgraphs incl. G; forests; (F,G') terms */
+  int32_t n_geoms, n_nums, n_nodes;   /* distinct element geometries, (geometry, operator) tables, value nodes */
+  int64_t n_records, n_coefs, n_coefs_nonzero;   /* numerator stream: records, stored and non-zero coefficients */
+  int64_t table_bytes;                /* device bytes of all plan tables */
+  int64_t stream_bytes;               /* bytes of the numerator coefficient stream (subset of table_bytes) */
+  double flops_per_sample;            /* algorithmic FP64 flops of a5-a7 + sampler (FMA = 2), non-zero coefs only */
+  double exec_flops_per_sample;       /* flops the double-precision kernel actually executes per sample */
+  double plan_seconds;                /* host time spent in fg_plan_create */
+} fg_plan_stats;
+int fg_plan_info(const fg_plan*, fg_plan_stats* out);
+
+/* Structure dump for tests (expression (11)).
+ *  subs: n_subgraphs rows (a, b, type 0 = self-energy / 1 = vertexlike, in_chain)
+ *  terms: flat ints: sign, index of G', n_members, then (sub index, op) pairs, op 0=A 1=U 2=L 3=L-U.
+ *  Returns the number of ints written to `terms`, or FG_E_LIMIT if cap is too small. */
+int fg_plan_structure(const fg_plan*, int32_t* subs, int32_t* terms, int32_t terms_cap);
+/* Copies Deg(s) and Z_1(s) (2^M doubles each; either may be NULL). */
+int fg_plan_tables(const fg_plan*, double* deg, double* Z1);
+
+typedef struct {
+  double mean;            /* (16): sum y / N */
+  double variance;        /* (17): sigma_down^2 = sum y^2 / N^2 - (sum y)^2 / N^3 */
+  double sum_y[2];        /* double-double (hi, lo) */
+  double sum_y2[2];
+  uint64_t n_samples;
+  uint64_t n_flagged;     /* samples re-evaluated in double-double */
+  uint64_t n_rejected;    /* samples that contributed 0 (non-finite or degenerate point) */
+  uint64_t n_pdf_big_exp; /* samples whose pdf left the double range, kept as x*2^j */
+} fg_result;
+
+/* Samples [0, n_samples) of the Philox stream `seed`.  Blocks until the result is on the host. */
+int fg_integrate(const fg_plan*, uint64_t n_samples, uint64_t seed, void* stream, fg_result* out);
+/* Samples [first_sample, first_sample + n_samples): sharding and checkpoint/resume. */
+int fg_integrate_range(const fg_plan*, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void* stream,
+                       fg_result* out);
+/* Asynchronous form: the result is left in device memory (`out_dev`, sizeof(fg_result) bytes, written by the
+ * final reduction kernel on `stream`); no host synchronisation. */
+int fg_integrate_async(const fg_plan*, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void* stream,
+                       void* out_dev);
+/* Exact combination of two shards (double-double sums add; mean/variance recomputed). */
+int fg_result_merge(const fg_result* a, const fg_result* b, fg_result* out);
+
+/* ---- parity / debug surface (device kernels; outputs are HOST arrays, any may be NULL) -------------------
+ * fg_sample_dump: for samples first..first+n-1: all Philox words (n * M * 4, call-major), mixture component (n),
+ * ordering j_1..j_M (n*M), z (n*M), pdf mantissa in [0.5,1) and exponent (n each), bad flag (n). */
+int fg_sample_dump(const fg_plan*, uint64_t first, uint64_t n, uint64_t seed, void* stream, uint32_t* philox_words,
+                   int32_t* comp, uint8_t* orderings, double* z, double* pdf_mant, int32_t* pdf_exp, uint8_t* bad);
+/* fg_eval_points: integrand at n given points (n*M doubles, on the simplex).  I = final value (double-double
+ * where flagged), I_double = plain double pass, err = its running error estimate, flags bit0 = flagged,
+ * bit1 = non-finite.  mode 0: as the integrator does; 1: double only; 2: double-double for every point. */
+int fg_eval_points(const fg_plan*, const double* z, uint64_t n, int32_t mode, void* stream, double* I,
+                   double* I_double, double* err, uint8_t* flags);
+/* fg_sample_eval_dump: what the integrator computes per sample, for samples first..first+n-1:
+ * I (final), y = I/g, flags as above. */
+int fg_sample_eval_dump(const fg_plan*, uint64_t first, uint64_t n, uint64_t seed, void* stream, double* I, double* y,
+                        uint8_t* flags);
+/* fg_dfma_peak: FP64-FMA micro-benchmark on the plan-independent device (the roofline denominator):
+ * returns achieved TFLOP/s (FMA = 2) over `iters` dependent-chain steps x 8 chains per thread on all SMs. */
+int fg_dfma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms);
+
+const char* fg_strerror(int code);
+const char* fg_last_error_message(void);
+const char* fg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

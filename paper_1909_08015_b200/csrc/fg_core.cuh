@@ -1,0 +1,286 @@
+// fg_core.cuh — per-sample arithmetic of the hot path, written once for T = double and T = dd.
+//   a1 Philox4x32-10 stream
+//   a2-a4 Hepp-sector sample, coordinates, pdf
+//   a5 element geometry: loop matrix, LDL^T, U, W, A, A^q, beta   PAPER.md:205 (method by reference)
+//   a6 numerator stream interpreter
+//   a7 forest sum
+// Everything here is device code; the FG_HD qualifier only lets a developer harness instantiate the same
+// templates on the host for debugging.  The library itself has no CPU compute path.
+#pragma once
+#include <float.h>
+#include <stdint.h>
+
+#include "fg_dd.cuh"
+#include "fg_tables.h"
+
+namespace fg {
+
+// ------------------------------------------------------------------------------------------------
+// a1  Philox4x32-10: counter = (sample_lo, sample_hi, call, 0), key = (seed_lo, seed_hi)
+// ------------------------------------------------------------------------------------------------
+FG_HD void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+// 53-bit uniform in the open interval (0,1)
+FG_HD double uniform53(uint32_t w0, uint32_t w1) { return ((double)((((uint64_t)w0 << 32) | w1) >> 11) + 0.5) * 0x1p-53; }
+
+struct UniformStream {
+  uint64_t sid, seed; uint32_t call, w[4]; int left;
+  FG_HD UniformStream(uint64_t sid_, uint64_t seed_) : sid(sid_), seed(seed_), call(0), left(0) {}
+  FG_HD double next() {
+    if (left == 0) { philox4x32_10((uint32_t)sid, (uint32_t)(sid >> 32), call++, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w); left = 2; }
+    double u = (left == 2) ? uniform53(w[0], w[1]) : uniform53(w[2], w[3]);
+    --left; return u;
+  }
+};
+
+// ------------------------------------------------------------------------------------------------
+// a2-a4  one sample of g = sum_k C_k g_k.  g_k has the form (14) with exponent table Deg_k:
+//   k=0: Deg_1 (graph table, through Z_1);  k=1: Deg = 1/2;  k=2: D*Deg_1 (through Z_3);  k=3: Deg(s) = |s| (uniform).
+// Sector j_1..j_M is drawn by M categorical draws with weights Z(s \ j); tau_l = u^(1/Deg(s_l)); z_{j_l} ~ prod tau.
+// The selection sums are evaluated in ascending line order without FMA contraction (bit-exact sectors).
+// ------------------------------------------------------------------------------------------------
+struct Sample { double z[FG_MAXM]; uint8_t order[FG_MAXM]; double mant; int ex; int comp; bool bad; };
+
+FG_HD void draw_sample(const FgPlanDev& P, const double* __restrict__ Z1, const double* __restrict__ Z3, uint64_t sid, uint64_t seed, Sample& r) {
+  const int M = P.M; const uint32_t full = (1u << M) - 1u;
+  UniformStream us(sid, seed);
+  double uc = us.next();
+  int comp = 3; { double c = 0.0; for (int k = 0; k < 4; ++k) { c = f_add(c, P.C[k]); if (uc < c) { comp = k; break; } } }
+  r.comp = comp;
+  double zeta[FG_MAXM], lnr[FG_MAXM], d1[FG_MAXM];
+  uint32_t s = full; double zprev = 1.0;
+  for (int l = 0; l < M; ++l) {
+    const int cnt = __builtin_popcount(s);
+    double tot1 = 0.0;
+    for (int j = 0; j < M; ++j) if ((s >> j) & 1u) tot1 = f_add(tot1, Z1[s ^ (1u << j)]);
+    d1[l] = (l == 0) ? 0.0 : tot1 / Z1[s];          // Deg_1(s) = sum_j Z_1(s\j) / Z_1(s)
+    const double usel = us.next();
+    int pick = -1;
+    if (comp == 0 || comp == 2) {
+      const double* Z = (comp == 0) ? Z1 : Z3;
+      double tot = tot1;
+      if (comp == 2) { tot = 0.0; for (int j = 0; j < M; ++j) if ((s >> j) & 1u) tot = f_add(tot, Z[s ^ (1u << j)]); }
+      const double thr = f_mul(usel, tot); double cum = 0.0; int last = -1;
+      for (int j = 0; j < M; ++j) if ((s >> j) & 1u) { cum = f_add(cum, Z[s ^ (1u << j)]); last = j; if (cum > thr) { pick = j; break; } }
+      if (pick < 0) pick = last;
+    } else {
+      int k = (int)f_mul(usel, (double)cnt); if (k >= cnt) k = cnt - 1;
+      for (int j = 0; j < M; ++j) if ((s >> j) & 1u) { if (k == 0) { pick = j; break; } --k; }
+    }
+    if (l == 0) { zeta[0] = 1.0; lnr[0] = 0.0; }
+    else {
+      const double dg = (comp == 0) ? d1[l] : (comp == 1) ? 0.5 : (comp == 2) ? f_mul(P.D, d1[l]) : (double)cnt;
+      const double u = us.next();
+      lnr[l] = log(u) / dg;                          // ln(z_{j_l} / z_{j_{l-1}})
+      zeta[l] = f_mul(zprev, pow(u, 1.0 / dg));
+    }
+    zprev = zeta[l];
+    r.order[l] = (uint8_t)pick; s ^= (1u << pick);
+  }
+  double sum = 0.0; for (int l = 0; l < M; ++l) sum = f_add(sum, zeta[l]);
+  bool bad = false;
+  for (int l = 0; l < M; ++l) { double zz = zeta[l] / sum; r.z[r.order[l]] = zz; if (!(zz >= DBL_MIN)) bad = true; }
+  // ln g_k = -ln Z_k(full) + sum_{l>=2} Deg_k(s_l) ln(z_{j_l}/z_{j_{l-1}}) - sum_j ln z_j      (14)
+  double lnzeta = 0.0, lnz_sum = 0.0;
+  for (int l = 0; l < M; ++l) { lnzeta += lnr[l]; lnz_sum += lnzeta; }
+  lnz_sum -= M * log(sum);
+  double lg[4];
+  for (int k = 0; k < 4; ++k) {
+    double e = 0.0;
+    for (int l = 1; l < M; ++l) { double dk = (k == 0) ? d1[l] : (k == 1) ? 0.5 : (k == 2) ? f_mul(P.D, d1[l]) : (double)(M - l); e += dk * lnr[l]; }
+    lg[k] = -P.lnZfull[k] + e - lnz_sum;
+  }
+  double mx = -DBL_MAX; for (int k = 0; k < 4; ++k) if (P.C[k] > 0.0 && lg[k] > mx) mx = lg[k];
+  double acc = 0.0; for (int k = 0; k < 4; ++k) if (P.C[k] > 0.0) acc += P.C[k] * exp(lg[k] - mx);
+  // g = acc * e^mx kept as mant * 2^ex with mant in [0.5,1)
+  const double l2 = mx * 1.4426950408889634074, fl = floor(l2);
+  int e2; const double mant = frexp(acc * exp2(l2 - fl), &e2);
+  r.mant = mant; r.ex = e2 + (int)fl;
+  if (!(mant > 0.0) || !(mant < 1.0)) bad = true;
+  r.bad = bad;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5  geometry of one element at one point.  Loop a = own photon a plus the own electron lines between its ends:
+//   B_ab = sum_j z_j eta_ja eta_jb + delta_ab z_gamma_a,  U = det B,  C_a = sum_j z_j eta_ja,  W = C^T B^-1 C,
+//   A_j = 1 - eta_j^T B^-1 C,  beta_ij = eta_i^T B^-1 eta_j,  A^q_j = xi^q_j - eta_j^T B^-1 C^q.
+// B = L D L^T (no square roots); growth = max_a B_aa / d_a measures the cancellation in the pivots.
+// V receives beta (upper triangle, row-major), then A, then A^q, element idx at V[idx * vs].
+// ------------------------------------------------------------------------------------------------
+template <class T>
+FG_HD void geom_eval(const FgGeomDev& E, const T* zl, T* V, int vs, T& U, T& W, double& growth) {
+  const int l = E.l, ne = E.ne;
+  T B[FG_MAXL][FG_MAXL], C[FG_MAXL], Cq[FG_MAXL], invd[FG_MAXL];
+  for (int a = 0; a < l; ++a) { C[a] = T(0.0); Cq[a] = T(0.0); for (int b = 0; b < l; ++b) B[a][b] = T(0.0); }
+  for (int q = 0; q < ne; ++q) {
+    const T z = zl[E.line_e[q]]; const unsigned m = E.eta[q]; const int xq = E.xiq[q];
+    const T zh = t_halve(z);
+    for (int a = 0; a < l; ++a) if ((m >> a) & 1u) {
+      C[a] = C[a] + z;
+      if (xq > 0) Cq[a] = Cq[a] + zh; else if (xq < 0) Cq[a] = Cq[a] - zh;
+      for (int b = 0; b <= a; ++b) if ((m >> b) & 1u) B[a][b] = B[a][b] + z;
+    }
+  }
+  for (int a = 0; a < l; ++a) B[a][a] = B[a][a] + zl[E.line_ph[a]];
+  U = T(1.0); double gr = 1.0;
+  for (int a = 0; a < l; ++a) {
+    T d = B[a][a];
+    for (int b = 0; b < a; ++b) d = d - B[a][b] * B[a][b] * B[b][b];     // B[b][b] now holds d_b, B[a][b] holds L_ab
+    const double g1 = to_double(B[a][a]) / to_double(d); if (g1 > gr || !(g1 == g1)) gr = g1;
+    invd[a] = T(1.0) / d; U = U * d;
+    for (int c = a + 1; c < l; ++c) {
+      T t = B[c][a];
+      for (int b = 0; b < a; ++b) t = t - B[c][b] * B[a][b] * B[b][b];
+      B[c][a] = t * invd[a];
+    }
+    B[a][a] = d;
+  }
+  growth = gr;
+  // x = L^-1 C, xq = L^-1 C^q
+  for (int a = 0; a < l; ++a) for (int b = 0; b < a; ++b) { C[a] = C[a] - B[a][b] * C[b]; Cq[a] = Cq[a] - B[a][b] * Cq[b]; }
+  T w = T(0.0); for (int a = 0; a < l; ++a) w = w + C[a] * C[a] * invd[a];
+  W = w;
+  T Y[FG_MAXNE][FG_MAXL];
+  const int nb = ne * (ne + 1) / 2;
+  for (int q = 0; q < ne; ++q) {
+    const unsigned m = E.eta[q];
+    for (int a = 0; a < l; ++a) { T y = ((m >> a) & 1u) ? T(1.0) : T(0.0); for (int b = 0; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
+    T sa = T(0.0), sq = T(0.0);
+    for (int a = 0; a < l; ++a) { T yd = Y[q][a] * invd[a]; sa = sa + yd * C[a]; sq = sq + yd * Cq[a]; }
+    V[(nb + q) * vs] = T(1.0) - sa;
+    V[(nb + ne + q) * vs] = T(0.5 * (double)E.xiq[q]) - sq;
+  }
+  int idx = 0;
+  for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) {
+    T b = T(0.0); for (int a = 0; a < l; ++a) b = b + Y[i][a] * Y[j][a] * invd[a];
+    V[idx * vs] = b; ++idx;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6  multilinear polynomial in K variables with a dense 2^K coefficient table (uniform across the block)
+// ------------------------------------------------------------------------------------------------
+template <class T, int S, int K> struct Horner {
+  static FG_HD void run(const double* __restrict__ c, const T (*a)[S], T* out) {
+    T lo[S], hi[S];
+    Horner<T, S, K - 1>::run(c, a, lo); Horner<T, S, K - 1>::run(c + (1 << (K - 1)), a, hi);
+#pragma unroll
+    for (int s = 0; s < S; ++s) out[s] = t_fma(a[K - 1][s], hi[s], lo[s]);
+  }
+};
+template <class T, int S> struct Horner<T, S, 0> {
+  static FG_HD void run(const double* __restrict__ c, const T (*)[S], T* out) {
+    const double c0 = c[0];
+#pragma unroll
+    for (int s = 0; s < S; ++s) out[s] = T(c0);
+  }
+};
+template <int S> struct Horner<double, S, 1> {   // leaf FMA takes both coefficients straight from the table
+  static FG_HD void run(const double* __restrict__ c, const double (*a)[S], double* out) {
+    const double c0 = c[0], c1 = c[1];
+#pragma unroll
+    for (int s = 0; s < S; ++s) out[s] = fma(a[0][s], c1, c0);
+  }
+};
+
+// One record: value[s] = prod_f V[fidx[f]] * sum_T coef[T] prod_{j in T} V[vidx[j]]
+template <class T, int S>
+FG_HD void eval_record(const FgRecHdr& h, const double* __restrict__ coef, const T* __restrict__ Vt, int vs, T (*q)[S], T* prod) {
+#pragma unroll
+  for (int s = 0; s < S; ++s) prod[s] = T(1.0);
+  for (int f = 0; f < h.nf; ++f) {
+    const T* p = Vt + (int)h.fidx[f] * vs;
+#pragma unroll
+    for (int s = 0; s < S; ++s) prod[s] = prod[s] * p[s];
+  }
+  T a[FG_KMAX][S];
+#pragma unroll
+  for (int j = 0; j < FG_KMAX; ++j) if (j < h.k) {
+    const T* p = Vt + (int)h.vidx[j] * vs;
+#pragma unroll
+    for (int s = 0; s < S; ++s) a[j][s] = p[s];
+  }
+  const int nc = h.ncomp;
+  switch (h.k) {
+#define FG_CASE(K) case K: Horner<T, S, K>::run(coef, a, q[0]); if (nc == 2) Horner<T, S, K>::run(coef + (1 << K), a, q[1]); break;
+    FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4) FG_CASE(5) FG_CASE(6)
+#undef FG_CASE
+    default: break;
+  }
+}
+
+// Scratch layout per sample (slot index; element at Sc[slot * ss]):
+//   [0, 2*ngeom)                U_g, W_g
+//   [rawv, rawv + raw_slots)    raw accumulators R[sig][deg][comp] of the running program; then their |.| sums
+//   node value polynomials [node][comp][deg], then node |.| polynomials
+struct ScratchMap {
+  int rawv, rawa, nodev, nodea;
+  FG_HD ScratchMap(const FgPlanDev& P) { rawv = 2 * P.ngeom; rawa = rawv + P.raw_slots; nodev = rawa + P.raw_slots; nodea = nodev + 2 * FG_NDEG * P.nnode; }
+};
+
+// a6 (cont.)  After the stream of a program: node polynomial = sum_sig R[sig] * prod_i (u or v of self-energy kid i),
+// times the scalar polynomials of the vertexlike kids.  Polynomials in t, degree < FG_NDEG.
+template <class T, bool ABS>
+FG_HD void finish_node(const FgPlanDev& P, const ScratchMap& sm, int node_id, T* Sc, int ss) {
+  const FgNodeDev nd = P.nodes[node_id];
+  const int nc = nd.ncomp, raw0 = ABS ? sm.rawa : sm.rawv, node0 = ABS ? sm.nodea : sm.nodev;
+  T out[2][FG_NDEG];
+  for (int c = 0; c < 2; ++c) for (int d = 0; d < FG_NDEG; ++d) out[c][d] = T(0.0);
+  for (int sig = 0; sig < (1 << nd.nse); ++sig) {
+    T f[FG_NDEG]; f[0] = T(1.0); for (int d = 1; d < FG_NDEG; ++d) f[d] = T(0.0);
+    for (int i = 0; i < nd.nse; ++i) {
+      const T* kp = Sc + (node0 + (nd.se_kid[i] * 2 + ((sig >> i) & 1)) * FG_NDEG) * ss;
+      T g[FG_NDEG]; for (int d = 0; d < FG_NDEG; ++d) g[d] = T(0.0);
+      for (int d1 = 0; d1 < FG_NDEG; ++d1) for (int d2 = 0; d1 + d2 < FG_NDEG; ++d2) g[d1 + d2] = g[d1 + d2] + f[d1] * kp[d2 * ss];
+      for (int d = 0; d < FG_NDEG; ++d) f[d] = g[d];
+    }
+    for (int c = 0; c < nc; ++c) for (int d1 = 0; d1 < FG_NDEG; ++d1) {
+      const T r = Sc[(raw0 + (sig * FG_NDEG + d1) * nc + c) * ss];
+      for (int d2 = 0; d1 + d2 < FG_NDEG; ++d2) out[c][d1 + d2] = out[c][d1 + d2] + r * f[d2];
+    }
+  }
+  for (int i = 0; i < nd.nvc; ++i) {
+    const T* kp = Sc + (node0 + (nd.vc_kid[i] * 2) * FG_NDEG) * ss;
+    for (int c = 0; c < nc; ++c) {
+      T g[FG_NDEG]; for (int d = 0; d < FG_NDEG; ++d) g[d] = T(0.0);
+      for (int d1 = 0; d1 < FG_NDEG; ++d1) for (int d2 = 0; d1 + d2 < FG_NDEG; ++d2) g[d1 + d2] = g[d1 + d2] + out[c][d1] * kp[d2 * ss];
+      for (int d = 0; d < FG_NDEG; ++d) out[c][d] = g[d];
+    }
+  }
+  for (int c = 0; c < nc; ++c) for (int d = 0; d < FG_NDEG; ++d) Sc[(node0 + (node_id * 2 + c) * FG_NDEG + d) * ss] = out[c][d];
+}
+
+// a7  I(z) = sum_{(F,G')} (-1)^{|F|-1} prod_S[(-1/4)^{l_S} / U_S^2] sum_{m<n} (n-m-1)! P_m / W_F^{n-m}
+template <class T, bool ABS>
+FG_HD void assemble(const FgPlanDev& P, const ScratchMap& sm, const T* Sc, int ss, T& I, T& Iabs) {
+  const int n = P.n;
+  T tot = T(0.0), tota = T(0.0);
+  for (int t = 0; t < P.nterm; ++t) {
+    const FgTermDev tm = P.terms[t];
+    T pu = T(1.0), wf = T(0.0);
+    for (int k = 0; k < tm.nmem; ++k) { const T u = Sc[(2 * tm.geom[k]) * ss]; pu = pu * u * u; wf = wf + Sc[(2 * tm.geom[k] + 1) * ss]; }
+    const T winv = T(1.0) / wf; T wp = winv, s = T(0.0), sa = T(0.0);
+    const T* pv = Sc + (sm.nodev + tm.top * 2 * FG_NDEG) * ss; const T* pa = Sc + (sm.nodea + tm.top * 2 * FG_NDEG) * ss;
+    for (int m = n - 1; m >= 0; --m) {
+      const T fw = wp * T(P.fact[n - m - 1]);
+      s = s + fw * pv[m * ss];
+      if (ABS) sa = sa + fw * pa[m * ss];
+      wp = wp * winv;
+    }
+    const T ipu = T(P.quarter_pow) / pu;
+    const T val = s * ipu;
+    tot = (tm.sign > 0) ? tot + val : tot - val;
+    if (ABS) { const T va = sa * ipu; tota = tota + T(t_abs_d(va)); }
+  }
+  I = tot; Iabs = tota;
+}
+
+}  // namespace fg

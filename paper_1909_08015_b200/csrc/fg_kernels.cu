@@ -1,0 +1,566 @@
+// fg_kernels.cu — sm_100a kernels of the hot path and the C ABI (include/fg.h).
+//
+// One persistent launch per precision rung (blocks of samples, deferred higher-precision passes):
+//   fg_eval_kernel<double>  draws a sample per Philox counter, evaluates every forest term, estimates the round-off
+//                           error, queues ill-conditioned samples, accumulates y = I/g in compensated FP64;
+//   fg_eval_kernel<dd>      re-evaluates the queued samples in double-double;
+//   fg_reduce_kernel        folds the per-block partial sums in a fixed order (deterministic).
+// The numerator coefficient stream is block-uniform: it is pulled through a two-stage shared-memory ring with
+// 1-D bulk TMA copies (cp.async.bulk + mbarrier) while the FP64 pipe works on the previous chunk.  Per-sample
+// operands (beta, A, A^q) live in shared memory, per-sample polynomials in an L2-resident scratch.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/fg.h"
+#include "fg_core.cuh"
+#include "fg_plan.hpp"
+
+namespace fg {
+
+struct RunArgs {
+  uint64_t first, n, seed;
+  const uint32_t* idlist; const unsigned long long* idcount;   // work list (ordinals relative to first) or NULL
+  const double* zin;                                           // points instead of samples, or NULL
+  double *outI, *outId, *outY, *outErr; uint8_t* outFlags;     // optional per-sample dumps, indexed by ordinal
+  uint32_t* flag_list; unsigned long long* flag_count;         // queue for the next rung
+  int do_flag;
+  double* partials;                                            // [gridDim.x][8]
+  void* scratch;
+};
+
+struct Accum { double sy[2], sy2[2]; unsigned long long nflag, nrej, nbig, n; };
+
+// ---- mbarrier / bulk-copy helpers (sm_90+ PTX; SASS: UBLKCP, SYNCS) -------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) { asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do { asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory"); } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2]; };
+
+// a6: run the record stream of one program for the S samples of this thread
+template <class T, int S, bool ABS>
+__device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const T* Vt, int vs, T* Sc, int ss) {
+  const int nslots = (1 << N.nse) * FG_NDEG * N.ncomp;
+  for (int i = 0; i < nslots; ++i) {
+#pragma unroll
+    for (int s = 0; s < S; ++s) { Sc[(sm.rawv + i) * ss + s] = T(0.0); if (ABS) Sc[(sm.rawa + i) * ss + s] = T(0.0); }
+  }
+  const int nch = N.chunk_count;
+  if (nch == 0) return;
+  const unsigned char* g0 = P.chunks + (size_t)N.chunk_begin * FG_CHUNK_BYTES;
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(&ring.bar[0], FG_CHUNK_BYTES); bulk_g2s(ring.buf, g0, FG_CHUNK_BYTES, &ring.bar[0]);
+    if (nch > 1) { mbar_expect_tx(&ring.bar[1], FG_CHUNK_BYTES); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[1]); }
+  }
+  int cur = -1; T acc[2][S], aab[2][S];
+  auto flush = [&]() {
+    if (cur < 0) return;
+    for (int c = 0; c < N.ncomp; ++c) {
+#pragma unroll
+      for (int s = 0; s < S; ++s) { Sc[(sm.rawv + cur * N.ncomp + c) * ss + s] = acc[c][s]; if (ABS) Sc[(sm.rawa + cur * N.ncomp + c) * ss + s] = aab[c][s]; }
+    }
+  };
+  for (int ch = 0; ch < nch; ++ch) {
+    const int b = ch & 1;
+    mbar_wait(&ring.bar[b], ring.phase[b]); ring.phase[b] ^= 1u;
+    const unsigned char* p = ring.buf + b * FG_CHUNK_BYTES;
+    const int nrec = ((const FgChunkHdr*)p)->nrec;
+    int off = sizeof(FgChunkHdr);
+    for (int r = 0; r < nrec; ++r) {
+      const FgRecHdr h = *(const FgRecHdr*)(p + off);
+      const double* coef = (const double*)(p + off + sizeof(FgRecHdr));
+      if ((int)h.dst != cur) {
+        flush(); cur = h.dst;
+#pragma unroll
+        for (int s = 0; s < S; ++s) { acc[0][s] = T(0.0); acc[1][s] = T(0.0); aab[0][s] = T(0.0); aab[1][s] = T(0.0); }
+      }
+      T q[2][S], prod[S];
+      eval_record<T, S>(h, coef, Vt, vs, q, prod);
+#pragma unroll
+      for (int s = 0; s < S; ++s) {
+        const T t0 = prod[s] * q[0][s]; acc[0][s] = acc[0][s] + t0; if (ABS) aab[0][s] = aab[0][s] + T(t_abs_d(t0));
+        if (h.ncomp == 2) { const T t1 = prod[s] * q[1][s]; acc[1][s] = acc[1][s] + t1; if (ABS) aab[1][s] = aab[1][s] + T(t_abs_d(t1)); }
+      }
+      off += (int)sizeof(FgRecHdr) + ((int)h.ncomp << h.k) * (int)sizeof(double);
+    }
+    __syncthreads();   // every thread is done with buffer b
+    if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], FG_CHUNK_BYTES); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[b]); }
+  }
+  flush();
+}
+
+// a5-a7 for the S points of this thread
+template <class T, int S, bool ABS>
+__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* growth) {
+  const ScratchMap sm(P);
+  T zl[S][FG_MAXLINES];
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    for (int v = 0; v < P.M; ++v) {
+      const int l0 = P.var_line0[v], l1 = P.var_line1[v];
+      if (l1 == 255) zl[s][l0] = T(z[s][v]); else { zl[s][l0] = T(0.5 * z[s][v]); zl[s][l1] = T(0.5 * z[s][v]); }
+    }
+    growth[s] = 1.0;
+  }
+  for (int g = 0; g < P.ngeom; ++g) {
+    const FgGeomDev E = P.geoms[g];
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      T U, W; double gr;
+      geom_eval<T>(E, zl[s], Vt + s, vs, U, W, gr);
+      Sc[(2 * g) * ss + s] = U; Sc[(2 * g + 1) * ss + s] = W;
+      if (gr > growth[s] || !(gr == gr)) growth[s] = gr;
+    }
+    for (int ni = P.geom_num_begin[g]; ni < P.geom_num_begin[g + 1]; ++ni) {
+      const FgNumDev N = P.nums[ni];
+      run_program<T, S, ABS>(P, N, sm, ring, Vt, vs, Sc, ss);
+      for (int k = 0; k < N.node_count; ++k) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) { finish_node<T, false>(P, sm, N.node_begin + k, Sc + s, ss); if (ABS) finish_node<T, true>(P, sm, N.node_begin + k, Sc + s, ss); }
+      }
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    T Iv, Ia; assemble<T, ABS>(P, sm, Sc + s, ss, Iv, Ia);
+    if (P.merge_var >= 0) { Iv = Iv * T(z[s][P.merge_var]); Ia = Ia * T(z[s][P.merge_var]); }
+    I[s] = Iv; Iabs[s] = to_double(Ia);
+  }
+}
+
+__device__ __forceinline__ dd shfl_dd(dd v, int off) { return dd(__shfl_down_sync(0xffffffffu, v.hi, off), __shfl_down_sync(0xffffffffu, v.lo, off)); }
+
+template <class T, int S, int NT>
+__global__ void __launch_bounds__(NT) fg_eval_kernel(const FgPlanDev P, const RunArgs A) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  ChunkRing ring; ring.buf = smem; ring.bar = (uint64_t*)(smem + 2 * FG_CHUNK_BYTES); ring.phase[0] = ring.phase[1] = 0u;
+  T* Vsm = (T*)(smem + 2 * FG_CHUNK_BYTES + 128);
+  const int tid = threadIdx.x;
+  if (tid == 0) { mbar_init(&ring.bar[0], 1); mbar_init(&ring.bar[1], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  __syncthreads();
+  const int vs = NT * S, ss = NT * S;
+  T* Vt = Vsm + tid * S;
+  T* Sc = (T*)A.scratch + (size_t)blockIdx.x * (size_t)P.scratch_slots * ss + tid * S;
+  const uint64_t nwork = A.idlist ? (uint64_t)*A.idcount : A.n;
+  const uint64_t per_batch = (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
+  dd sy(0.0), sy2(0.0); unsigned long long nflag = 0, nrej = 0, nbig = 0;
+  const int M = P.M;
+  for (uint64_t batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
+    double z[S][FG_MAXM], mant[S]; int ex[S]; bool valid[S], bad[S]; uint64_t oid[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      const uint64_t ord = batch * per_batch + (uint64_t)s * NT + tid;
+      valid[s] = ord < nwork; bad[s] = false; mant[s] = 0.5; ex[s] = 1; oid[s] = 0;
+      if (valid[s]) {
+        oid[s] = A.idlist ? (uint64_t)A.idlist[ord] : ord;
+        if (A.zin) { for (int v = 0; v < M; ++v) z[s][v] = A.zin[oid[s] * M + v]; }
+        else {
+          Sample sp; draw_sample(P, P.Z1, P.Z3, A.first + oid[s], A.seed, sp);
+          for (int v = 0; v < M; ++v) z[s][v] = sp.z[v];
+          mant[s] = sp.mant; ex[s] = sp.ex; bad[s] = sp.bad;
+        }
+      }
+      if (!valid[s] || bad[s]) for (int v = 0; v < M; ++v) z[s][v] = 1.0 / M;
+    }
+    T I[S]; double Iabs[S], growth[S];
+    eval_points<T, S, !is_dd<T>::value>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth);
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (!valid[s]) continue;
+      const double Id = to_double(I[s]);
+      const double err = is_dd<T>::value ? 0.0 : P.err_eps * growth[s] * Iabs[s];
+      uint8_t fl = 0; double y = 0.0;
+      if (ex[s] > 1023 || ex[s] < -1021) ++nbig;
+      if (bad[s]) { ++nrej; fl = 2; }
+      else {
+        const double tol = fmax(P.rel_tol * fabs(Id), ldexp(P.abs_tol * mant[s], ex[s]));
+        const bool flagged = A.do_flag && !(err <= tol);
+        if (flagged) {
+          fl = 1; ++nflag;
+          if (A.flag_list) { const unsigned long long pos = atomicAdd(A.flag_count, 1ull); A.flag_list[pos] = (uint32_t)oid[s]; }
+        } else {
+          const T yq = I[s] / T(mant[s]);
+          y = ldexp(to_double(yq), -ex[s]);
+          if (!isfinite(y)) { ++nrej; fl |= 2; y = 0.0; }
+          else {
+            const dd yd = is_dd<T>::value ? dd(ldexp(to_double(yq), -ex[s])) : dd(y);
+            sy = dd_add_d(sy, yd.hi); const dd y2 = two_prod(yd.hi, yd.hi); sy2 = sy2 + y2;
+          }
+        }
+      }
+      if (A.outI) A.outI[oid[s]] = Id;
+      if (A.outId) A.outId[oid[s]] = Id;
+      if (A.outY) A.outY[oid[s]] = y;
+      if (A.outErr) A.outErr[oid[s]] = err;
+      if (A.outFlags) A.outFlags[oid[s]] = is_dd<T>::value ? (uint8_t)(A.outFlags[oid[s]] | fl) : fl;
+    }
+  }
+  // a10: warp shuffle -> block -> one partial per block
+  double cnt[3] = {(double)nflag, (double)nrej, (double)nbig};
+  for (int off = 16; off > 0; off >>= 1) { sy = sy + shfl_dd(sy, off); sy2 = sy2 + shfl_dd(sy2, off); for (int k = 0; k < 3; ++k) cnt[k] += __shfl_down_sync(0xffffffffu, cnt[k], off); }
+  __syncthreads();
+  double* red = (double*)smem;   // the ring is idle now
+  if ((tid & 31) == 0) { double* r = red + (tid >> 5) * 8; r[0] = sy.hi; r[1] = sy.lo; r[2] = sy2.hi; r[3] = sy2.lo; r[4] = cnt[0]; r[5] = cnt[1]; r[6] = cnt[2]; }
+  __syncthreads();
+  if (tid == 0) {
+    dd a(0.0), b(0.0); double c[3] = {0, 0, 0};
+    for (int w = 0; w < NT / 32; ++w) { const double* r = red + w * 8; a = a + dd(r[0], r[1]); b = b + dd(r[2], r[3]); for (int k = 0; k < 3; ++k) c[k] += r[4 + k]; }
+    double* o = A.partials + (size_t)blockIdx.x * 8;
+    o[0] = a.hi; o[1] = a.lo; o[2] = b.hi; o[3] = b.lo; o[4] = c[0]; o[5] = c[1]; o[6] = c[2]; o[7] = 0.0;
+  }
+}
+
+__global__ void fg_reduce_kernel(const double* partials, int nparts, Accum* acc, unsigned long long n_add, int finalize, fg_result* out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  dd a(acc->sy[0], acc->sy[1]), b(acc->sy2[0], acc->sy2[1]);
+  double c[3] = {0, 0, 0};
+  for (int i = 0; i < nparts; ++i) { const double* r = partials + (size_t)i * 8; a = a + dd(r[0], r[1]); b = b + dd(r[2], r[3]); for (int k = 0; k < 3; ++k) c[k] += r[4 + k]; }
+  acc->sy[0] = a.hi; acc->sy[1] = a.lo; acc->sy2[0] = b.hi; acc->sy2[1] = b.lo;
+  acc->nflag += (unsigned long long)c[0]; acc->nrej += (unsigned long long)c[1]; acc->nbig += (unsigned long long)c[2]; acc->n += n_add;
+  if (finalize) {
+    const double N = (double)acc->n;
+    out->mean = to_double(a) / N;
+    const dd v = b / dd(N * N) - a * a / dd(N * N * N);   // (17)
+    out->variance = to_double(v);
+    out->sum_y[0] = a.hi; out->sum_y[1] = a.lo; out->sum_y2[0] = b.hi; out->sum_y2[1] = b.lo;
+    out->n_samples = acc->n; out->n_flagged = acc->nflag; out->n_rejected = acc->nrej; out->n_pdf_big_exp = acc->nbig;
+  }
+}
+
+__global__ void fg_sample_dump_kernel(const FgPlanDev P, uint64_t first, uint64_t n, uint64_t seed, uint32_t* words, int32_t* comp,
+                                      uint8_t* order, double* z, double* mant, int32_t* ex, uint8_t* bad) {
+  const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint64_t sid = first + i; const int M = P.M;
+  if (words) for (int c = 0; c < M; ++c) { uint32_t w[4]; philox4x32_10((uint32_t)sid, (uint32_t)(sid >> 32), (uint32_t)c, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w); for (int k = 0; k < 4; ++k) words[(i * M + c) * 4 + k] = w[k]; }
+  Sample sp; draw_sample(P, P.Z1, P.Z3, sid, seed, sp);
+  if (comp) comp[i] = sp.comp;
+  for (int v = 0; v < M; ++v) { if (order) order[i * M + v] = sp.order[v]; if (z) z[i * M + v] = sp.z[v]; }
+  if (mant) mant[i] = sp.mant; if (ex) ex[i] = sp.ex; if (bad) bad[i] = sp.bad ? 1 : 0;
+}
+
+// FP64-FMA peak: 8 independent chains per thread (the roofline denominator is measured, not quoted)
+__global__ void fg_dfma_kernel(double* out, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-9, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int i = 0; i < iters; ++i) {
+    x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+    x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+  }
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+}  // namespace fg
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+using namespace fg;
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string& m) { g_err = m; return code; }
+#define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail(FG_E_CUDA, std::string(#x) + ": " + cudaGetErrorString(e_)); } while (0)
+
+struct fg_graph { Graph g; };
+
+static const int NT_D = 128, S_D = 2;     // double pass: threads per block, samples per thread
+static const int NT_Q = 128, S_Q = 1;     // double-double pass
+static const uint64_t SLAB = 1ull << 24;  // samples per launch (bounds the re-evaluation queue)
+
+struct fg_plan {
+  HostPlan H; FgPlanDev D; int device = 0, sms = 0;
+  std::vector<void*> allocs;
+  void* scratch = nullptr; double* partials = nullptr; Accum* accum = nullptr; fg_result* result_dev = nullptr;
+  uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr;
+  int grid_d = 0, grid_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
+  int64_t table_bytes = 0;
+  std::mutex mu;
+};
+
+template <class T> static int upload(fg_plan* p, const std::vector<T>& v, const T** dst) {
+  void* d = nullptr; size_t bytes = std::max<size_t>(v.size() * sizeof(T), 16);
+  CU(cudaMalloc(&d, bytes)); p->allocs.push_back(d); p->table_bytes += (int64_t)bytes;
+  if (!v.empty()) CU(cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+  *dst = (const T*)d; return FG_OK;
+}
+
+extern "C" {
+
+const char* fg_version(void) { return "fg 0.1 (sm_100a)"; }
+const char* fg_last_error_message(void) { return g_err.c_str(); }
+const char* fg_strerror(int code) {
+  switch (code) {
+    case FG_OK: return "ok"; case FG_E_ARG: return "bad argument"; case FG_E_COUNT: return "wrong number of lines or vertices";
+    case FG_E_NOT_PATH: return "electron lines are not one open path"; case FG_E_VERTEX: return "vertex without exactly one photon";
+    case FG_E_NOT_1PI: return "graph is not one-particle irreducible"; case FG_E_LOOPS: return "more than 5 loops";
+    case FG_E_CUDA: return "CUDA error"; case FG_E_LIMIT: return "internal limit exceeded"; case FG_E_OPTS: return "invalid plan options";
+    default: return "unknown error";
+  }
+}
+
+int fg_graph_create(const fg_edge* edges, int32_t n_edges, int32_t ext_photon_vertex, fg_graph** out) {
+  if (!out) return fail(FG_E_ARG, "out is NULL");
+  *out = nullptr;
+  if (!edges) return fail(FG_E_ARG, "edges is NULL");
+  fg_graph* G = new fg_graph(); std::string msg;
+  int rc = graph_from_edges((const int32_t*)edges, n_edges, ext_photon_vertex, G->g, msg);
+  if (rc != FG_OK) { delete G; return fail(rc, msg); }
+  *out = G; return FG_OK;
+}
+void fg_graph_destroy(fg_graph* g) { delete g; }
+
+void fg_plan_opts_default(fg_plan_opts* o) {
+  if (!o) return;
+  std::memset(o, 0, sizeof(*o));
+  o->C[0] = 0.9; o->C[1] = 0.03; o->C[2] = 0.01; o->C[3] = 0.06; o->D = 0.75;   // Calc 2
+  o->merge_ext_lines = 0; o->deg_table = nullptr; o->rel_tol = 1e-12; o->abs_tol = 0.0; o->err_factor = 0.0;
+}
+
+void fg_plan_destroy(fg_plan* p) {
+  if (!p) return;
+  cudaSetDevice(p->device);
+  for (void* a : p->allocs) cudaFree(a);
+  delete p;
+}
+
+int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, fg_plan** out) {
+  if (!out) return fail(FG_E_ARG, "out is NULL");
+  *out = nullptr;
+  if (!g) return fail(FG_E_ARG, "graph is NULL");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(FG_E_CUDA, "no CUDA device: this library has no CPU path");
+  if (device < 0 || device >= ndev) return fail(FG_E_ARG, "device out of range");
+  fg_plan_opts o; if (opts) o = *opts; else fg_plan_opts_default(&o);
+  PlanOpts po; for (int k = 0; k < 4; ++k) po.C[k] = o.C[k]; po.D = o.D; po.merge = o.merge_ext_lines ? 1 : 0;
+  po.rel_tol = o.rel_tol; po.abs_tol = o.abs_tol; po.err_factor = o.err_factor;
+  int M = 3 * g->g.n - (po.merge ? 1 : 0);
+  if (o.deg_table) po.deg_override.assign(o.deg_table, o.deg_table + ((size_t)1 << M));
+  fg_plan* p = new fg_plan(); std::string msg;
+  int rc = build_plan(g->g, po, p->H, msg);
+  if (rc != FG_OK) { delete p; return fail(rc, msg); }
+  p->device = device;
+  cudaError_t e = cudaSetDevice(device); if (e != cudaSuccess) { delete p; return fail(FG_E_CUDA, cudaGetErrorString(e)); }
+  cudaDeviceProp prop; cudaGetDeviceProperties(&prop, device); p->sms = prop.multiProcessorCount;
+  HostPlan& H = p->H; FgPlanDev& D = p->D; std::memset(&D, 0, sizeof(D));
+  D.n = H.g.n; D.M = H.M; D.nlines = 3 * H.g.n; D.merge_var = H.merge_var;
+  D.ngeom = (int)H.d_geoms.size(); D.nnum = (int)H.d_nums.size(); D.nnode = (int)H.d_nodes.size(); D.nterm = (int)H.d_terms.size();
+  D.raw_slots = H.raw_slots; D.scratch_slots = H.scratch_slots;
+  for (int v = 0; v < H.M; ++v) { D.var_line0[v] = (uint8_t)H.var_lines[v][0]; D.var_line1[v] = H.var_lines[v].size() > 1 ? (uint8_t)H.var_lines[v][1] : 255; }
+  for (int k = 0; k < 4; ++k) { D.C[k] = H.opts.C[k]; D.lnZfull[k] = H.lnZfull[k]; }
+  D.D = H.opts.D; D.rel_tol = po.rel_tol; D.abs_tol = po.abs_tol;
+  D.err_eps = (po.err_factor > 0 ? po.err_factor : 64.0) * 0x1p-53;
+  D.quarter_pow = std::pow(-0.25, H.g.n); D.fact[0] = 1; for (int k = 1; k < FG_NDEG; ++k) D.fact[k] = D.fact[k - 1] * k;
+#define UP(vec, field) do { int rc_ = upload(p, vec, &D.field); if (rc_ != FG_OK) { fg_plan_destroy(p); return rc_; } } while (0)
+  UP(H.d_geoms, geoms); UP(H.d_nums, nums); UP(H.d_nodes, nodes); UP(H.d_terms, terms); UP(H.d_geom_num_begin, geom_num_begin);
+  UP(H.d_chunks, chunks); UP(H.Z1, Z1); UP(H.Z3, Z3);
+#undef UP
+  int vmax = 1; for (auto& E : H.geoms) vmax = std::max(vmax, E.ne * (E.ne + 1) / 2 + 2 * E.ne);
+  p->vmax = vmax;
+  p->smem_d = 2 * FG_CHUNK_BYTES + 128 + (size_t)vmax * NT_D * S_D * sizeof(double);
+  p->smem_q = 2 * FG_CHUNK_BYTES + 128 + (size_t)vmax * NT_Q * S_Q * sizeof(dd);
+  p->grid_d = p->sms; p->grid_q = p->sms;
+  auto setattr = [&](const void* f, size_t sm) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); };
+  e = setattr((const void*)fg_eval_kernel<double, S_D, NT_D>, p->smem_d); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>, p->smem_q);
+  if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("shared memory: ") + cudaGetErrorString(e)); }
+  size_t sc = (size_t)H.scratch_slots * std::max((size_t)NT_D * S_D * sizeof(double) * p->grid_d, (size_t)NT_Q * S_Q * sizeof(dd) * p->grid_q);
+  auto dmalloc = [&](void** d, size_t bytes) { cudaError_t e2 = cudaMalloc(d, bytes); if (e2 == cudaSuccess) { p->allocs.push_back(*d); cudaMemset(*d, 0, bytes); } return e2; };
+  e = dmalloc(&p->scratch, sc);
+  if (e == cudaSuccess) e = dmalloc((void**)&p->partials, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->accum, sizeof(Accum));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->result_dev, sizeof(fg_result));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->flag_list, SLAB * sizeof(uint32_t));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->flag_count, sizeof(unsigned long long));
+  if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
+  *out = p; return FG_OK;
+}
+
+int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
+  if (!p || !s) return fail(FG_E_ARG, "NULL argument");
+  const HostPlan& H = p->H; std::memset(s, 0, sizeof(*s));
+  s->n_loops = H.g.n; s->M = H.M; s->n_subgraphs = (int)H.subs.size(); s->n_forests = (int)H.forests.size(); s->n_terms = (int)H.terms.size();
+  s->n_geoms = (int)H.geoms.size(); s->n_nums = (int)H.nums.size(); s->n_nodes = (int)H.nodes.size();
+  s->n_records = H.n_records; s->n_coefs = H.n_coefs; s->n_coefs_nonzero = H.n_nonzero;
+  s->table_bytes = p->table_bytes; s->stream_bytes = (int64_t)H.d_chunks.size();
+  s->flops_per_sample = H.algo_flops; s->exec_flops_per_sample = H.exec_flops; s->plan_seconds = H.plan_seconds;
+  return FG_OK;
+}
+
+int fg_plan_structure(const fg_plan* p, int32_t* subs, int32_t* terms, int32_t cap) {
+  if (!p) return fail(FG_E_ARG, "NULL plan");
+  const HostPlan& H = p->H;
+  if (subs) for (size_t k = 0; k < H.subs.size(); ++k) { subs[4 * k] = H.subs[k].a; subs[4 * k + 1] = H.subs[k].b; subs[4 * k + 2] = H.subs[k].type; subs[4 * k + 3] = H.subs[k].chain; }
+  int w = 0;
+  if (terms) for (auto& t : H.terms) {
+    if (w + 3 + 2 * (int)t.members.size() > cap) return fail(FG_E_LIMIT, "terms buffer too small");
+    terms[w++] = t.sign; terms[w++] = t.gprime; terms[w++] = (int)t.members.size();
+    for (size_t k = 0; k < t.members.size(); ++k) { terms[w++] = t.members[k]; terms[w++] = t.ops[k]; }
+  }
+  return w;
+}
+
+int fg_plan_tables(const fg_plan* p, double* deg, double* Z1) {
+  if (!p) return fail(FG_E_ARG, "NULL plan");
+  if (deg) std::memcpy(deg, p->H.deg.data(), p->H.deg.size() * sizeof(double));
+  if (Z1) std::memcpy(Z1, p->H.Z1.data(), p->H.Z1.size() * sizeof(double));
+  return FG_OK;
+}
+
+// one slab: double pass, double-double pass over its queue, fold partials
+static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaStream_t st, const double* zin, int mode,
+                    double* dI, double* dId, double* dY, double* dErr, uint8_t* dFl, bool finalize, fg_result* out_dev) {
+  RunArgs A; std::memset(&A, 0, sizeof(A));
+  A.first = first; A.n = n; A.seed = seed; A.zin = zin; A.outI = dI; A.outId = dId; A.outY = dY; A.outErr = dErr; A.outFlags = dFl;
+  A.scratch = p->scratch;
+  int nparts = 0;
+  if (mode != 2) {
+    CU(cudaMemsetAsync(p->flag_count, 0, sizeof(unsigned long long), st));
+    A.flag_list = p->flag_list; A.flag_count = p->flag_count; A.do_flag = (mode == 0); A.partials = p->partials;
+    uint64_t nbatch = (n + (uint64_t)NT_D * S_D - 1) / ((uint64_t)NT_D * S_D);
+    int grid = (int)std::min<uint64_t>((uint64_t)p->grid_d, std::max<uint64_t>(nbatch, 1));
+    CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
+    fg_eval_kernel<double, S_D, NT_D><<<grid, NT_D, p->smem_d, st>>>(p->D, A);
+    CU(cudaGetLastError());
+    nparts = p->grid_d;
+  } else CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
+  if (mode == 0 || mode == 2) {
+    RunArgs B = A; B.do_flag = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
+    if (mode == 0) { B.idlist = p->flag_list; B.idcount = p->flag_count; }
+    fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, NT_Q, p->smem_q, st>>>(p->D, B);
+    CU(cudaGetLastError());
+    nparts = p->grid_d + p->grid_q;
+  }
+  fg_reduce_kernel<<<1, 32, 0, st>>>(p->partials, nparts, p->accum, (unsigned long long)n, finalize ? 1 : 0, out_dev);
+  CU(cudaGetLastError());
+  return FG_OK;
+}
+
+int fg_integrate_async(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, void* out_dev) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
+  if (!p || !out_dev) return fail(FG_E_ARG, "NULL argument");
+  if (n == 0) return fail(FG_E_ARG, "n_samples must be > 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaSetDevice(p->device));
+  CU(cudaMemsetAsync(p->accum, 0, sizeof(Accum), st));
+  for (uint64_t done = 0; done < n; done += SLAB) {
+    uint64_t m = std::min<uint64_t>(SLAB, n - done);
+    int rc = run_slab(p, first + done, m, seed, st, nullptr, 0, nullptr, nullptr, nullptr, nullptr, nullptr, done + m >= n, (fg_result*)out_dev);
+    if (rc != FG_OK) return rc;
+  }
+  return FG_OK;
+}
+
+int fg_integrate_range(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, fg_result* out) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
+  if (!p || !out) return fail(FG_E_ARG, "NULL argument");
+  std::lock_guard<std::mutex> lk(p->mu);
+  int rc = fg_integrate_async(p, first, n, seed, stream, p->result_dev);
+  if (rc != FG_OK) return rc;
+  CU(cudaMemcpyAsync(out, p->result_dev, sizeof(fg_result), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  return FG_OK;
+}
+int fg_integrate(const fg_plan* p, uint64_t n, uint64_t seed, void* stream, fg_result* out) { return fg_integrate_range(p, 0, n, seed, stream, out); }
+
+int fg_result_merge(const fg_result* a, const fg_result* b, fg_result* out) {
+  if (!a || !b || !out) return fail(FG_E_ARG, "NULL argument");
+  fg_result r; std::memset(&r, 0, sizeof(r));
+  dd sy = dd(a->sum_y[0], a->sum_y[1]) + dd(b->sum_y[0], b->sum_y[1]);
+  dd s2 = dd(a->sum_y2[0], a->sum_y2[1]) + dd(b->sum_y2[0], b->sum_y2[1]);
+  r.n_samples = a->n_samples + b->n_samples; r.n_flagged = a->n_flagged + b->n_flagged; r.n_rejected = a->n_rejected + b->n_rejected;
+  r.n_pdf_big_exp = a->n_pdf_big_exp + b->n_pdf_big_exp;
+  r.sum_y[0] = sy.hi; r.sum_y[1] = sy.lo; r.sum_y2[0] = s2.hi; r.sum_y2[1] = s2.lo;
+  double N = (double)r.n_samples;
+  if (N > 0) { r.mean = to_double(sy) / N; r.variance = to_double(s2 / dd(N * N) - sy * sy / dd(N * N * N)); }
+  *out = r; return FG_OK;
+}
+
+// ---- debug / parity surface -----------------------------------------------------------------------------------
+struct DevBuf {
+  void* d = nullptr; size_t bytes = 0;
+  ~DevBuf() { if (d) cudaFree(d); }
+  cudaError_t alloc(size_t b) { bytes = b; return cudaMalloc(&d, std::max<size_t>(b, 16)); }
+};
+#define CUB(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail(FG_E_CUDA, std::string(#x) + ": " + cudaGetErrorString(e_)); } while (0)
+
+int fg_sample_dump(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, uint32_t* words, int32_t* comp,
+                   uint8_t* order, double* z, double* mant, int32_t* ex, uint8_t* bad) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
+  if (!p) return fail(FG_E_ARG, "NULL plan");
+  if (n == 0) return FG_OK;
+  cudaStream_t st = (cudaStream_t)stream; CU(cudaSetDevice(p->device));
+  const int M = p->D.M;
+  DevBuf bw, bc, bo, bz, bm, be, bb;
+  if (words) CUB(bw.alloc(n * M * 4 * sizeof(uint32_t))); if (comp) CUB(bc.alloc(n * sizeof(int32_t))); if (order) CUB(bo.alloc(n * M));
+  if (z) CUB(bz.alloc(n * M * sizeof(double))); if (mant) CUB(bm.alloc(n * sizeof(double))); if (ex) CUB(be.alloc(n * sizeof(int32_t))); if (bad) CUB(bb.alloc(n));
+  fg_sample_dump_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(p->D, first, n, seed, (uint32_t*)bw.d, (int32_t*)bc.d, (uint8_t*)bo.d, (double*)bz.d, (double*)bm.d, (int32_t*)be.d, (uint8_t*)bb.d);
+  CU(cudaGetLastError());
+  auto back = [&](void* h, DevBuf& b) { return h ? cudaMemcpyAsync(h, b.d, b.bytes, cudaMemcpyDeviceToHost, st) : cudaSuccess; };
+  CU(back(words, bw)); CU(back(comp, bc)); CU(back(order, bo)); CU(back(z, bz)); CU(back(mant, bm)); CU(back(ex, be)); CU(back(bad, bb));
+  CU(cudaStreamSynchronize(st));
+  return FG_OK;
+}
+
+static int eval_common(fg_plan* p, const double* z_host, uint64_t first, uint64_t n, uint64_t seed, int mode, cudaStream_t st,
+                       double* I, double* Id, double* Y, double* err, uint8_t* flags) {
+  if (n == 0) return FG_OK;
+  if (n > SLAB) return fail(FG_E_ARG, "at most 2^24 points per call");
+  std::lock_guard<std::mutex> lk(p->mu);
+  CU(cudaSetDevice(p->device));
+  const int M = p->D.M;
+  DevBuf bz, bI, bId, bY, bE, bF;
+  if (z_host) { CUB(bz.alloc(n * M * sizeof(double))); CU(cudaMemcpyAsync(bz.d, z_host, bz.bytes, cudaMemcpyHostToDevice, st)); }
+  CUB(bI.alloc(n * sizeof(double))); CUB(bId.alloc(n * sizeof(double))); CUB(bY.alloc(n * sizeof(double))); CUB(bE.alloc(n * sizeof(double))); CUB(bF.alloc(n));
+  CU(cudaMemsetAsync(bF.d, 0, n, st)); CU(cudaMemsetAsync(bE.d, 0, n * sizeof(double), st)); CU(cudaMemsetAsync(bId.d, 0, n * sizeof(double), st));
+  CU(cudaMemsetAsync(p->accum, 0, sizeof(Accum), st));
+  int rc = run_slab(p, first, n, seed, st, (const double*)bz.d, mode, (double*)bI.d, (double*)bId.d, (double*)bY.d, (double*)bE.d, (uint8_t*)bF.d, true, p->result_dev);
+  if (rc != FG_OK) return rc;
+  auto back = [&](void* h, DevBuf& b) { return h ? cudaMemcpyAsync(h, b.d, b.bytes, cudaMemcpyDeviceToHost, st) : cudaSuccess; };
+  CU(back(I, bI)); CU(back(Id, bId)); CU(back(Y, bY)); CU(back(err, bE)); CU(back(flags, bF));
+  CU(cudaStreamSynchronize(st));
+  return FG_OK;
+}
+
+int fg_eval_points(const fg_plan* cp, const double* z, uint64_t n, int32_t mode, void* stream, double* I, double* I_double, double* err, uint8_t* flags) {
+  if (!cp || (!z && n)) return fail(FG_E_ARG, "NULL argument");
+  if (mode < 0 || mode > 2) return fail(FG_E_ARG, "mode must be 0, 1 or 2");
+  return eval_common(const_cast<fg_plan*>(cp), z, 0, n, 0, mode, (cudaStream_t)stream, I, I_double, nullptr, err, flags);
+}
+
+int fg_sample_eval_dump(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, double* I, double* y, uint8_t* flags) {
+  if (!cp) return fail(FG_E_ARG, "NULL plan");
+  return eval_common(const_cast<fg_plan*>(cp), nullptr, first, n, seed, 0, (cudaStream_t)stream, I, nullptr, y, nullptr, flags);
+}
+
+int fg_dfma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms_out) {
+  if (!tflops || iters <= 0) return fail(FG_E_ARG, "bad argument");
+  int ndev = 0; if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(FG_E_CUDA, "no CUDA device");
+  CU(cudaSetDevice(device));
+  cudaDeviceProp prop; CU(cudaGetDeviceProperties(&prop, device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const int threads = 256, blocks = prop.multiProcessorCount * 8;
+  DevBuf out; CUB(out.alloc((size_t)threads * blocks * sizeof(double)));
+  cudaEvent_t e0, e1; CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  fg_dfma_kernel<<<blocks, threads, 0, st>>>((double*)out.d, iters / 8 + 1, 0.999999, 1e-7);   // warm-up
+  CU(cudaEventRecord(e0, st));
+  fg_dfma_kernel<<<blocks, threads, 0, st>>>((double*)out.d, iters, 0.999999, 1e-7);
+  CU(cudaEventRecord(e1, st)); CU(cudaEventSynchronize(e1));
+  float ms = 0; CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  double flops = 2.0 * 8.0 * (double)iters * threads * blocks;
+  *tflops = flops / (ms * 1e-3) / 1e12; if (ms_out) *ms_out = ms;
+  return FG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,557 @@
+// fg_plan.cpp — host planner (see fg_plan.hpp).  All citations: PAPER.md = /root/reference/PAPER.md.
+//
+// What is built here, in the paper's order:
+//   graph validity (1PI, no lepton loops)
+//   UV-divergent subgraphs: self-energy (N_e=2,N_gamma=0), vertexlike (N_e=2,N_gamma=1)   PAPER.md:139, fn.7
+//   forests F[G] and the chain I[G]
+//   operator table of R^new: A on G', U below, L above, (L-U) on G     PAPER.md:184-198, example (11) at 200-203
+//   per element: loop basis, slot string, Dirac traces of the projectors A, U, L
+//   Hepp-sector density tables Deg(s), Z(s)
+// The numerator of every (element, operator) is flattened into a stream of "records"
+//   value = prod_f V[f] * sum_{T subset of k free slots} coef[T] prod_{j in T} A_j
+// that the CUDA kernel interprets.
+#include "fg_plan.hpp"
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <numeric>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#include "../../include/fg.h"
+
+namespace fg {
+
+// ------------------------------------------------------------------------------------------------
+// graph
+// ------------------------------------------------------------------------------------------------
+static bool spanned(const Graph& g, int lo, int hi, int i) {   // electron line e_i spanned by a photon inside [lo,hi]
+  for (auto& p : g.ph) if (p[0] >= lo && p[1] <= hi && p[0] <= i - 1 && p[1] >= i) return true;
+  return false;
+}
+
+int graph_from_edges(const int32_t* edges, int n_edges, int ext_vertex, Graph& g, std::string& msg) {
+  if (!edges || n_edges <= 0) { msg = "no edges"; return FG_E_ARG; }
+  if (n_edges % 3 != 0) { msg = "need 3n internal lines"; return FG_E_COUNT; }
+  int n = n_edges / 3;
+  if (n > FG_MAXL) { msg = "more than 5 loops"; return FG_E_LOOPS; }
+  int nv = 2 * n + 1;
+  std::vector<std::array<int, 2>> el, pl;
+  for (int k = 0; k < n_edges; ++k) {
+    int u = edges[3 * k], v = edges[3 * k + 1], kind = edges[3 * k + 2];
+    if (u < 0 || v < 0 || u >= nv || v >= nv || u == v) { msg = "vertex out of range (need vertices 0..2n)"; return FG_E_COUNT; }
+    if (kind == 0) el.push_back({u, v}); else if (kind == 1) pl.push_back({u, v}); else { msg = "edge kind must be 0 or 1"; return FG_E_ARG; }
+  }
+  if ((int)el.size() != 2 * n || (int)pl.size() != n) { msg = "need 2n electron and n photon lines"; return FG_E_COUNT; }
+  if (ext_vertex < 0 || ext_vertex >= nv) { msg = "external-photon vertex out of range"; return FG_E_ARG; }
+  // electron lines must form one open path; follow it u -> v
+  std::vector<int> out(nv, -1), indeg(nv, 0), outdeg(nv, 0);
+  for (auto& e : el) { if (out[e[0]] >= 0) { msg = "two electron lines leave one vertex"; return FG_E_NOT_PATH; } out[e[0]] = e[1]; ++outdeg[e[0]]; ++indeg[e[1]]; }
+  int start = -1;
+  for (int v = 0; v < nv; ++v) { if (indeg[v] > 1) { msg = "two electron lines enter one vertex"; return FG_E_NOT_PATH; } if (indeg[v] == 0) { if (start >= 0) { msg = "electron lines are not one path"; return FG_E_NOT_PATH; } start = v; } }
+  if (start < 0) { msg = "electron lines close a loop (lepton loop)"; return FG_E_NOT_PATH; }
+  std::vector<int> pos(nv, -1); int cur = start, cnt = 0;
+  while (cur >= 0 && pos[cur] < 0) { pos[cur] = cnt++; cur = out[cur]; }
+  if (cnt != nv) { msg = "electron lines are not one open path through all vertices"; return FG_E_NOT_PATH; }
+  g = Graph(); g.n = n; g.nv = nv; g.x = pos[ext_vertex]; g.partner.assign(nv, -1);
+  std::vector<int> used(nv, 0); used[g.x] = 1;
+  for (auto& p : pl) {
+    int a = pos[p[0]], b = pos[p[1]]; if (a > b) std::swap(a, b);
+    if (used[a] || used[b]) { msg = "a vertex carries more than one photon"; return FG_E_VERTEX; }
+    used[a] = used[b] = 1; g.partner[a] = b; g.partner[b] = a; g.ph.push_back({a, b});
+  }
+  for (int v = 0; v < nv; ++v) if (!used[v]) { msg = "a vertex carries no photon"; return FG_E_VERTEX; }
+  std::sort(g.ph.begin(), g.ph.end());
+  for (int i = 1; i <= 2 * n; ++i) if (!spanned(g, 0, 2 * n, i)) { msg = "electron line e_" + std::to_string(i) + " is not spanned by a photon"; return FG_E_NOT_1PI; }
+  return FG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// UV-divergent subgraphs (fn.7 at 155): with no lepton loops each is the induced subgraph on a
+// vertex interval whose electron lines are all spanned by internal photons; the number of vertices whose photon
+// leaves the interval (v_x counts) is 0 (self-energy) or 1 (vertexlike).
+// ------------------------------------------------------------------------------------------------
+static bool classify(const Graph& g, int a, int b, Sub& s) {
+  int leaving = 0, inside = 0;
+  for (int v = a; v <= b; ++v) { int p = g.partner[v]; if (p < 0 || p < a || p > b) ++leaving; else ++inside; }
+  if (inside < 2 || leaving > 1) return false;
+  for (int i = a + 1; i <= b; ++i) if (!spanned(g, a, b, i)) return false;
+  s.a = a; s.b = b; s.type = leaving; s.chain = (leaving == 1 && g.x >= a && g.x <= b);
+  return true;
+}
+static bool contains(const Sub& p, const Sub& q) { return p.a <= q.a && q.b <= p.b; }
+static bool overlap(const Sub& p, const Sub& q) {   // share a line, neither contains the other
+  return std::max(p.a, q.a) < std::min(p.b, q.b) && !contains(p, q) && !contains(q, p);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Clifford monomials: s * gamma^mask, gamma^mask = ascending product; {g^mu,g^nu} = 2 diag(+,-,-,-)
+// ------------------------------------------------------------------------------------------------
+struct CliffTab {
+  uint8_t flip[16][4];   // sign flip when gamma^mu is multiplied on the right of gamma^mask
+  uint8_t parsp[16];     // parity of the number of spatial gammas = parity of popcount(mask & 0b1110)
+  CliffTab() {
+    for (int m = 0; m < 16; ++m) {
+      parsp[m] = __builtin_popcount(m & 14) & 1;
+      for (int mu = 0; mu < 4; ++mu) {
+        int f = __builtin_popcount(m >> (mu + 1)) & 1;      // hop over the gammas with larger index
+        if (((m >> mu) & 1) && mu != 0) f ^= 1;             // gamma^i gamma^i = -1
+        flip[m][mu] = (uint8_t)f;
+      }
+    }
+  }
+};
+static const CliffTab CT;
+
+static int trace_of(const std::vector<int>& F, int p0, int mask) {   // Tr[ prod F * gamma0^p0 * gamma^mask ]
+  int s = 0, m = 0;
+  auto mul = [&](int mu) { s ^= CT.flip[m][mu]; m ^= (1 << mu); };
+  for (int mu : F) mul(mu);
+  if (p0) mul(0);
+  for (int mu = 0; mu < 4; ++mu) if ((mask >> mu) & 1) mul(mu);
+  return m == 0 ? (s ? -4 : 4) : 0;
+}
+
+// One run: sum over the Lorentz indices of all chords (photon chords and Wick pairs) of the signed monomial of the
+// string, resolved by the parity pattern `cb` that a gamma^0 placed at each gap would pick up when moved to the front.
+struct DiracRun {
+  int ntok = 0;
+  int8_t kind[48];   // 0 first end of chord, 1 second end, 2 fixed gamma, 3 gap
+  int8_t arg[48];
+  int8_t val[16];
+  int64_t* N = nullptr;
+  void go(int pos, unsigned sgn, unsigned mask, unsigned cb) {
+    for (;;) {
+      if (pos == ntok) { N[cb] += sgn ? -1 : 1; return; }
+      int a = arg[pos];
+      switch (kind[pos]) {
+        case 0:
+          for (int mu = 0; mu < 4; ++mu) { val[a] = (int8_t)mu; go(pos + 1, sgn ^ CT.flip[mask][mu], mask ^ (1u << mu), cb); }
+          return;
+        case 1: { int mu = val[a]; sgn ^= CT.flip[mask][mu] ^ (mu != 0 ? 1u : 0u); mask ^= (1u << mu); break; }   // gamma_rho = g_rr gamma^rho
+        case 2: sgn ^= CT.flip[mask][a]; mask ^= (1u << a); break;
+        default: cb |= (unsigned)CT.parsp[mask] << a; break;
+      }
+      ++pos;
+    }
+  }
+};
+
+struct Piece { double w; std::vector<int> F; int ext; bool q; };
+
+static std::vector<Piece> pieces_of(int op, int type, int comp) {
+  // Rest frame p = (1,0,0,0), p^2 = m^2 = 1.
+  std::vector<Piece> P;
+  if (type == 0) {                       // U on a self-energy Sigma = u + v p-hat: u = Tr[Sigma]/4, v = Tr[g0 Sigma]/4
+    if (comp == 0) P.push_back({0.25, {}, -1, false}); else P.push_back({0.25, {0}, -1, false});
+    return P;
+  }
+  // Gamma_mu(p,0) = a g_mu + b p_mu + c p-hat p_mu + d(p-hat g_mu - g_mu p-hat)   (10)
+  auto addU = [&](double s) { P.push_back({-0.25 * s, {3}, 3, false}); };                      // a = Tr[g^3 Gamma_3]/4, Gamma_3 = -Gamma^3
+  auto addL = [&](double s) { P.push_back({0.25 * s, {}, 0, false}); P.push_back({0.25 * s, {0}, 0, false}); };   // a+b+c = Tr[(1+g0)Gamma_0]/4
+  if (op == FG_OP_U) addU(1);
+  else if (op == FG_OP_L) addL(1);
+  else if (op == FG_OP_LMU) { addL(1); addU(-1); }
+  else {
+    // A: Pauli form factor at q = 0 from Gamma^mu = V^mu + q_nu T^{nu mu}:
+    //   (1/12) Tr[g_mu V^mu - (4 g0 + 3) V^0]  =  -(1/4) { Tr[g0 V^0] + Tr[g3 V^3] + Tr[V^0] }   (isotropy)
+    //   (1/48) sum_{mu != nu} Tr[(g0+1)[g_mu,g_nu](g0+1) T^{nu mu}] = (1/2) Tr[g1 g2 (1+g0) T^{21}]
+    P.push_back({-0.25, {0}, 0, false}); P.push_back({-0.25, {3}, 3, false}); P.push_back({-0.25, {}, 0, false});
+    P.push_back({0.5, {1, 2}, 1, true}); P.push_back({0.5, {1, 2, 0}, 1, true});
+  }
+  return P;
+}
+
+// ------------------------------------------------------------------------------------------------
+// element geometry
+// ------------------------------------------------------------------------------------------------
+static HGeom make_geom(const Graph& g, const std::vector<Sub>& subs, int si, const std::vector<int>& kids) {
+  HGeom E; E.sub = si; E.kids = kids;
+  const Sub& S = subs[si];
+  int n2 = 2 * g.n;
+  struct Site { int kind, v, kid; };   // kind 0 plain vertex, 1 vertexlike child, 2 self-energy child
+  std::vector<Site> sites; std::vector<int> site_of(g.nv, -1);
+  for (int v = S.a; v <= S.b; ++v) {
+    int kid = -1; for (int c : kids) if (subs[c].a == v) kid = c;
+    int s = (int)sites.size();
+    if (kid >= 0) { sites.push_back({subs[kid].type == 1 ? 1 : 2, v, kid}); for (int w = subs[kid].a; w <= subs[kid].b; ++w) site_of[w] = s; v = subs[kid].b; }
+    else { sites.push_back({0, v, -1}); site_of[v] = s; }
+    if (v < S.b) E.own_e.push_back(v);   // line e_{v+1} = (v_v, v_{v+1}) has id v; it joins site s and site s+1
+  }
+  E.ne = (int)E.own_e.size();
+  std::vector<int> chord(g.n, -1); std::vector<std::array<int, 2>> ph_sites;
+  for (int k = 0; k < g.n; ++k) {
+    int a = g.ph[k][0], b = g.ph[k][1];
+    if (a < S.a || b > S.b || site_of[a] == site_of[b]) continue;
+    chord[k] = (int)E.own_ph.size(); E.own_ph.push_back(n2 + k); ph_sites.push_back({site_of[a], site_of[b]});
+  }
+  E.l = (int)E.own_ph.size();
+  E.eta.assign(E.ne, 0);
+  for (int q = 0; q < E.ne; ++q) for (int a = 0; a < E.l; ++a) if (ph_sites[a][0] <= q && q < ph_sites[a][1]) E.eta[q] |= (1 << a);
+  E.has_x = (g.x >= S.a && g.x <= S.b);
+  int xsite = E.has_x ? site_of[g.x] : -1;
+  E.xiq.assign(E.ne, 0);
+  if (E.has_x) for (int q = 0; q < E.ne; ++q) E.xiq[q] = (q + 1 <= xsite) ? -1 : +1;
+  int ext_site = -1;
+  if (S.type == 1) for (int w = S.a; w <= S.b; ++w) { int p = g.partner[w]; if (p < 0 || p < S.a || p > S.b) ext_site = site_of[w]; }
+  for (auto& st : sites) { if (st.kind == 2) E.se_kids.push_back(st.kid); if (st.kind == 1) E.vc_kids.push_back(st.kid); }
+  // tokens in path order: site, line, site, ...; reversed below (the matrix string reads from v_b back to v_a)
+  std::vector<Tok> fw; std::vector<Slot> fslots;
+  for (int s = 0; s < (int)sites.size(); ++s) {
+    const Site& st = sites[s];
+    if (st.kind == 2) {
+      int idx = (int)(std::find(E.se_kids.begin(), E.se_kids.end(), st.kid) - E.se_kids.begin());
+      fw.push_back({2, (int)fslots.size()}); fslots.push_back({s - 1, idx, E.has_x ? (s < xsite ? -1 : +1) : 0});
+    } else if (s == ext_site) fw.push_back({1, 0});
+    else {
+      int k = -1;   // the photon attached here: a plain vertex's own photon, or the one photon leaving a vertexlike child
+      for (int q = 0; q < g.n; ++q) {
+        if (st.kind == 0) { if (g.ph[q][0] == st.v || g.ph[q][1] == st.v) k = q; }
+        else { const Sub& K = subs[st.kid]; bool ia = g.ph[q][0] >= K.a && g.ph[q][0] <= K.b, ib = g.ph[q][1] >= K.a && g.ph[q][1] <= K.b; if (ia != ib) k = q; }
+      }
+      fw.push_back({0, chord[k]});
+    }
+    if (s + 1 < (int)sites.size()) { fw.push_back({2, (int)fslots.size()}); fslots.push_back({s, -1, E.xiq[s]}); }
+  }
+  int ns = (int)fslots.size();
+  for (int i = (int)fw.size() - 1; i >= 0; --i) { Tok t = fw[i]; if (t.kind == 2) t.id = ns - 1 - t.id; E.toks.push_back(t); }
+  E.slots.assign(fslots.rbegin(), fslots.rend());
+  return E;
+}
+
+// ------------------------------------------------------------------------------------------------
+// numerator records of one (geometry, operator)
+// ------------------------------------------------------------------------------------------------
+struct Matching { std::vector<std::array<int, 2>> pairs; std::vector<int> unmatched; };
+static void enum_matchings(int ns, std::vector<Matching>& out) {
+  std::vector<int> used(ns, 0); Matching cur;
+  struct R { static void go(int i, int ns, std::vector<int>& used, Matching& cur, std::vector<Matching>& out) {
+    while (i < ns && used[i]) ++i;
+    if (i == ns) { out.push_back(cur); return; }
+    used[i] = 1;
+    cur.unmatched.push_back(i); go(i + 1, ns, used, cur, out); cur.unmatched.pop_back();
+    for (int j = i + 1; j < ns; ++j) if (!used[j]) { used[j] = 1; cur.pairs.push_back({i, j}); go(i + 1, ns, used, cur, out); cur.pairs.pop_back(); used[j] = 0; }
+    used[i] = 0;
+  } };
+  R::go(0, ns, used, cur, out);
+  for (auto& m : out) std::sort(m.unmatched.begin(), m.unmatched.end());
+}
+
+// table over subsets T of `gaps` (bit g of T = gaps[g] carries gamma^0) of the coefficient of this matching
+static void matching_table(const HGeom& E, int type, int op, int comp, const Matching& m, int qslot, bool qpart,
+                           const std::vector<int>& gaps, std::vector<double>& out) {
+  int ng = (int)gaps.size(); size_t nT = (size_t)1 << ng;
+  out.assign(nT, 0.0);
+  std::vector<Piece> pcs = pieces_of(op, type, comp);
+  std::vector<int> exts;
+  for (auto& p : pcs) if (p.q == qpart && std::find(exts.begin(), exts.end(), p.ext) == exts.end()) exts.push_back(p.ext);
+  int ns = (int)E.slots.size();
+  std::vector<int> role(ns, -1), gapidx(ns, -1);
+  for (size_t k = 0; k < m.pairs.size(); ++k) { role[m.pairs[k][0]] = (int)k; role[m.pairs[k][1]] = (int)k; }
+  for (int gi = 0; gi < ng; ++gi) gapidx[gaps[gi]] = gi;
+  const int NU = 2;
+  std::vector<int64_t> N(nT);
+  for (int ext : exts) {
+    DiracRun R; R.N = N.data(); std::fill(N.begin(), N.end(), 0);
+    std::vector<int> seen(E.l + m.pairs.size(), 0);
+    int fm = 0;
+    for (const Tok& t : E.toks) {
+      int chord = -1;
+      if (t.kind == 1) { R.kind[R.ntok] = 2; R.arg[R.ntok++] = (int8_t)ext; fm ^= (1 << ext); continue; }
+      if (t.kind == 0) chord = t.id;
+      else if (t.id == qslot) { R.kind[R.ntok] = 2; R.arg[R.ntok++] = NU; fm ^= (1 << NU); continue; }
+      else if (role[t.id] < 0) { R.kind[R.ntok] = 3; R.arg[R.ntok++] = (int8_t)gapidx[t.id]; continue; }
+      else chord = E.l + role[t.id];
+      R.kind[R.ntok] = (int8_t)(seen[chord] ? 1 : 0); R.arg[R.ntok++] = (int8_t)chord; seen[chord] = 1;
+    }
+    R.go(0, 0u, 0u, 0u);
+    // Walsh-Hadamard: H[T] = sum_cb N[cb] (-1)^{|T & cb|}
+    for (size_t h = 1; h < nT; h <<= 1) for (size_t i = 0; i < nT; i += (h << 1)) for (size_t j = i; j < i + h; ++j) { int64_t a = N[j], b = N[j + h]; N[j] = a + b; N[j + h] = a - b; }
+    for (auto& p : pcs) if (p.q == qpart && p.ext == ext) {
+      int tr[2] = {trace_of(p.F, 0, fm), trace_of(p.F, 1, fm)};
+      for (size_t T = 0; T < nT; ++T) { int t = tr[__builtin_popcountll(T) & 1]; if (t) out[T] += p.w * (double)t * (double)N[T]; }
+    }
+  }
+  double pref = 1.0; for (size_t k = 0; k < m.pairs.size(); ++k) pref *= -0.5;   // <kappa_i^mu kappa_j^nu> = -(1/2) beta_ij g^{mu nu} t
+  for (auto& c : out) c *= pref;
+}
+
+static void build_records(const HGeom& E, int type, HNum& N) {
+  int ns = (int)E.slots.size(), ne = E.ne, nb = ne * (ne + 1) / 2;
+  auto bidx = [&](int i, int j) { if (i > j) std::swap(i, j); return i * ne - i * (i - 1) / 2 + (j - i); };
+  std::vector<Matching> ms; enum_matchings(ns, ms);
+  std::vector<std::vector<HRecord>> per(ms.size());
+  int ncomp = N.ncomp;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long mi = 0; mi < (long)ms.size(); ++mi) {
+    const Matching& m = ms[mi];
+    int npairs = (int)m.pairs.size();
+    std::vector<int> qchoices = {-1};
+    if (N.op == FG_OP_A && type == 1) for (int s : m.unmatched) qchoices.push_back(s);
+    for (int q : qchoices) {
+      std::vector<int> gaps; for (int s : m.unmatched) if (s != q) gaps.push_back(s);
+      std::vector<double> tab[2];
+      for (int c = 0; c < ncomp; ++c) matching_table(E, type, N.op, c, m, q, q >= 0, gaps, tab[c]);
+      bool any = false; for (int c = 0; c < ncomp; ++c) for (double v : tab[c]) if (v != 0.0) any = true;
+      if (!any) continue;
+      // split the gaps: pseudo-slots (self-energy children) and own lines beyond FG_KMAX are enumerated
+      std::vector<int> en, fr;   // positions in `gaps`
+      for (int gi = 0; gi < (int)gaps.size(); ++gi) { if (E.slots[gaps[gi]].se >= 0) en.push_back(gi); else fr.push_back(gi); }
+      while ((int)fr.size() > FG_KMAX) { en.push_back(fr.back()); fr.pop_back(); }
+      int sig0 = 0; std::vector<int> f0;
+      for (auto& pr : m.pairs) { f0.push_back(bidx(E.slots[pr[0]].e, E.slots[pr[1]].e)); for (int t = 0; t < 2; ++t) if (E.slots[pr[t]].se >= 0) sig0 |= 1 << E.slots[pr[t]].se; }
+      if (q >= 0) { f0.push_back(nb + ne + E.slots[q].e); if (E.slots[q].se >= 0) sig0 |= 1 << E.slots[q].se; }
+      for (unsigned eb = 0; eb < (1u << en.size()); ++eb) {
+        HRecord r; r.ncomp = ncomp; r.k = (int)fr.size(); int sig = sig0; std::vector<int> f = f0; size_t Tbase = 0;
+        for (size_t t = 0; t < en.size(); ++t) if ((eb >> t) & 1) { const Slot& sl = E.slots[gaps[en[t]]]; f.push_back(nb + sl.e); if (sl.se >= 0) sig |= 1 << sl.se; Tbase |= (size_t)1 << en[t]; }
+        r.nf = (int)f.size(); r.dst = sig * FG_NDEG + npairs;
+        std::memset(r.fidx, 0, sizeof(r.fidx)); std::memset(r.vidx, 0, sizeof(r.vidx));
+        for (int t = 0; t < r.nf; ++t) r.fidx[t] = (uint8_t)f[t];
+        for (int t = 0; t < r.k; ++t) r.vidx[t] = (uint8_t)(nb + E.slots[gaps[fr[t]]].e);
+        r.coef.assign((size_t)ncomp << r.k, 0.0); bool nz = false;
+        for (int c = 0; c < ncomp; ++c) for (size_t sub = 0; sub < ((size_t)1 << r.k); ++sub) {
+          size_t T = Tbase; for (int t = 0; t < r.k; ++t) if ((sub >> t) & 1) T |= (size_t)1 << fr[t];
+          double v = tab[c][T]; r.coef[((size_t)c << r.k) + sub] = v; if (v != 0.0) nz = true;
+        }
+        if (nz) per[mi].push_back(std::move(r));
+      }
+    }
+  }
+  for (auto& v : per) for (auto& r : v) N.recs.push_back(std::move(r));
+  std::stable_sort(N.recs.begin(), N.recs.end(), [](const HRecord& a, const HRecord& b) { if (a.dst != b.dst) return a.dst < b.dst; return a.k > b.k; });
+  for (auto& r : N.recs) {
+    long nc = (long)r.coef.size(), nz = 0; for (double v : r.coef) if (v != 0.0) ++nz;
+    N.n_coefs += nc; N.n_nonzero += nz;
+    N.exec_flops += std::max(0, r.nf - 1) + r.ncomp * (2.0 * ((1 << r.k) - 1) + 2.0);
+    N.algo_flops += std::max(0, r.nf - 1) + 2.0 * nz;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// density tables.  Deg(s): the paper's algorithm (constants (15)) is only in
+// its Refs. [42],[32]; reading R-Deg is used unless the caller supplies a table.
+// ------------------------------------------------------------------------------------------------
+static void build_density(HostPlan& P) {
+  const Graph& g = P.g; int n = g.n, M = P.M; size_t nset = (size_t)1 << M;
+  P.deg.assign(nset, 0.0);
+  if (!P.opts.deg_override.empty()) { for (size_t s = 1; s + 1 < nset; ++s) P.deg[s] = P.opts.deg_override[s]; }
+  else {
+    for (size_t s = 1; s + 1 < nset; ++s) {
+      std::vector<char> in(3 * n, 0);
+      for (int v = 0; v < M; ++v) if ((s >> v) & 1) for (int id : P.var_lines[v]) in[id] = 1;
+      std::vector<int> root(g.nv); std::iota(root.begin(), root.end(), 0);
+      auto find = [&](int a) { while (root[a] != a) a = root[a] = root[root[a]]; return a; };
+      int ne = 0, np = 0, indep = 0;
+      for (int id = 0; id < 3 * n; ++id) if (in[id]) {
+        int a = id < 2 * n ? id : g.ph[id - 2 * n][0], b = id < 2 * n ? id + 1 : g.ph[id - 2 * n][1];
+        (id < 2 * n ? ne : np)++;
+        int ra = find(a), rb = find(b); if (ra != rb) { root[ra] = rb; ++indep; }
+      }
+      int loops = ne + np - indep;
+      double omega = 2.0 * loops - 0.5 * ne - 1.0 * np;          // superficial degree of the line set
+      std::vector<int> inside;
+      for (size_t k = 1; k < P.subs.size(); ++k) {
+        const Sub& S = P.subs[k]; bool all = true;
+        for (int i = S.a; i < S.b; ++i) if (!in[i]) all = false;
+        for (int q = 0; q < n; ++q) if (g.ph[q][0] >= S.a && g.ph[q][1] <= S.b && !in[2 * n + q]) all = false;
+        if (all) inside.push_back((int)k);
+      }
+      for (int k : inside) {
+        bool maximal = true; for (int k2 : inside) if (k2 != k && contains(P.subs[k2], P.subs[k])) maximal = false;
+        if (maximal) omega -= (P.subs[k].type == 1 ? 0.0 : 0.5) + 0.5;   // remove omega(S) + 1/2 of a subtracted subgraph
+      }
+      P.deg[s] = std::min(1.5, std::max(0.5, -omega));
+    }
+  }
+  auto buildZ = [&](double scale, std::vector<double>& Z) {
+    Z.assign(nset, 0.0); Z[0] = 1.0;
+    for (size_t s = 1; s < nset; ++s) {
+      double sum = 0.0;
+      for (int j = 0; j < M; ++j) if ((s >> j) & 1) sum = sum + Z[s ^ ((size_t)1 << j)];
+      Z[s] = (s + 1 < nset) ? sum / (scale * P.deg[s]) : sum;
+    }
+  };
+  buildZ(1.0, P.Z1); buildZ(P.opts.D, P.Z3);
+  P.lnZfull[0] = std::log(P.Z1[nset - 1]); P.lnZfull[2] = std::log(P.Z3[nset - 1]);
+  double lz = 0.0; for (int k = 1; k < M; ++k) lz += std::log(2.0 * k);   // Deg = 1/2: Z(s) = 2^|s| |s|!
+  P.lnZfull[1] = lz + std::log((double)M); P.lnZfull[3] = std::log((double)M);   // Deg = |s|: Z = 1
+}
+
+// ------------------------------------------------------------------------------------------------
+// the plan
+// ------------------------------------------------------------------------------------------------
+int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& msg) {
+  auto t0 = std::chrono::steady_clock::now();
+  P = HostPlan(); P.g = g; P.opts = opts;
+  int n = g.n;
+  double csum = 0; for (int k = 0; k < 4; ++k) { if (!(opts.C[k] >= 0)) { msg = "C_k must be >= 0"; return FG_E_OPTS; } csum += opts.C[k]; }
+  if (std::fabs(csum - 1.0) > 1e-12 || !(opts.D > 0)) { msg = "C must sum to 1 and D must be > 0"; return FG_E_OPTS; }
+  // variables (the two electron lines at v_x may share one variable)
+  for (int id = 0; id < 3 * n; ++id) {
+    if (opts.merge && id == g.x - 1) { P.merge_var = (int)P.var_lines.size(); P.var_lines.push_back({g.x - 1, g.x}); }
+    else if (opts.merge && id == g.x) continue;
+    else P.var_lines.push_back({id});
+  }
+  P.M = (int)P.var_lines.size();
+  if (!opts.deg_override.empty() && opts.deg_override.size() != ((size_t)1 << P.M)) { msg = "deg_table must have 2^M entries"; return FG_E_OPTS; }
+  // subgraphs
+  Sub G; if (!classify(g, 0, 2 * n, G) || !G.chain) { msg = "graph is not a vertex graph"; return FG_E_NOT_1PI; }
+  P.subs.push_back(G);
+  for (int a = 0; a <= 2 * n; ++a) for (int b = a + 1; b <= 2 * n; ++b) { if (a == 0 && b == 2 * n) continue; Sub s; if (classify(g, a, b, s)) P.subs.push_back(s); }
+  int np = (int)P.subs.size() - 1;
+  if (np > 20) { msg = "too many subgraphs"; return FG_E_LIMIT; }
+  // forests
+  for (uint32_t mask = 0; mask < (1u << np); ++mask) {
+    std::vector<int> mem = {0}; bool ok = true;
+    for (int i = 0; i < np && ok; ++i) if ((mask >> i) & 1) { for (int j : mem) if (j && overlap(P.subs[i + 1], P.subs[j])) ok = false; mem.push_back(i + 1); }
+    if (ok) P.forests.push_back(mem);
+  }
+  // terms
+  for (auto& F : P.forests) {
+    if ((int)F.size() > FG_MAXMEM) { msg = "forest too large"; return FG_E_LIMIT; }
+    std::vector<int> chain; for (int m : F) if (P.subs[m].chain) chain.push_back(m);
+    std::sort(chain.begin(), chain.end(), [&](int p, int q) { return P.subs[p].b - P.subs[p].a > P.subs[q].b - P.subs[q].a; });
+    for (size_t r = 0; r < chain.size(); ++r) {
+      HTerm t; t.members = F; t.gprime = chain[r]; t.sign = (F.size() % 2 == 1) ? +1 : -1;
+      for (int m : F) {
+        size_t pos = std::find(chain.begin(), chain.end(), m) - chain.begin();
+        int op;
+        if (pos == chain.size()) op = FG_OP_U;            // not in I[G]
+        else if (pos == r) op = FG_OP_A;                  // G'
+        else if (pos > r) op = FG_OP_U;                   // inside G'
+        else op = (m == 0) ? FG_OP_LMU : FG_OP_L;         // contains G'
+        t.ops.push_back(op);
+      }
+      P.terms.push_back(t);
+    }
+  }
+  // geometries, programs, nodes
+  std::map<std::vector<int>, int> gmap, nmap, ndmap;
+  for (auto& t : P.terms) {
+    std::map<int, std::vector<int>> kids_of; std::map<int, int> op_of;
+    for (size_t k = 0; k < t.members.size(); ++k) {
+      int m = t.members[k]; op_of[m] = t.ops[k];
+      std::vector<int> ch;
+      for (int c : t.members) if (c != m && contains(P.subs[m], P.subs[c])) {
+        bool maximal = true;
+        for (int d : t.members) if (d != m && d != c && contains(P.subs[d], P.subs[c]) && contains(P.subs[m], P.subs[d])) maximal = false;
+        if (maximal) ch.push_back(c);
+      }
+      std::sort(ch.begin(), ch.end(), [&](int p, int q) { return P.subs[p].a < P.subs[q].a; });
+      kids_of[m] = ch;
+    }
+    std::map<int, int> geom_of;
+    struct R { static int go(HostPlan& P, int m, std::map<int, std::vector<int>>& kids_of, std::map<int, int>& op_of, std::map<int, int>& geom_of,
+                             std::map<std::vector<int>, int>& gmap, std::map<std::vector<int>, int>& nmap, std::map<std::vector<int>, int>& ndmap) {
+      std::vector<int> gk = {m}; for (int c : kids_of[m]) gk.push_back(c);
+      int gi; auto it = gmap.find(gk);
+      if (it == gmap.end()) { gi = (int)P.geoms.size(); P.geoms.push_back(make_geom(P.g, P.subs, m, kids_of[m])); gmap[gk] = gi; } else gi = it->second;
+      geom_of[m] = gi;
+      std::vector<int> nk = {gi, op_of[m]}; int ni; auto it2 = nmap.find(nk);
+      if (it2 == nmap.end()) { ni = (int)P.nums.size(); HNum N; N.geom = gi; N.op = op_of[m]; N.ncomp = P.subs[m].type == 0 ? 2 : 1; N.nse = (int)P.geoms[gi].se_kids.size(); P.nums.push_back(N); nmap[nk] = ni; } else ni = it2->second;
+      HNode nd; nd.num = ni; std::vector<int> key = {ni};
+      const HGeom& E = P.geoms[gi];
+      for (int c : E.se_kids) { int id = go(P, c, kids_of, op_of, geom_of, gmap, nmap, ndmap); nd.se_kid.push_back(id); key.push_back(id); }
+      key.push_back(-1);
+      for (int c : E.vc_kids) { int id = go(P, c, kids_of, op_of, geom_of, gmap, nmap, ndmap); nd.vc_kid.push_back(id); key.push_back(id); }
+      auto it3 = ndmap.find(key); if (it3 != ndmap.end()) return it3->second;
+      int id = (int)P.nodes.size(); P.nodes.push_back(nd); ndmap[key] = id; return id;
+    } };
+    t.top = R::go(P, 0, kids_of, op_of, geom_of, gmap, nmap, ndmap);
+    for (int m : t.members) t.geoms.push_back(geom_of[m]);
+  }
+  for (auto& E : P.geoms) if ((int)E.se_kids.size() > FG_MAXSE || (int)E.vc_kids.size() > FG_MAXVC || E.ne > FG_MAXNE || E.l > FG_MAXL) { msg = "element limit exceeded"; return FG_E_LIMIT; }
+  // evaluation order: children (shorter intervals) first.  Renumber geoms, nums, nodes accordingly.
+  {
+    int ng = (int)P.geoms.size();
+    std::vector<int> order(ng); std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int p, int q) { const Sub& a = P.subs[P.geoms[p].sub]; const Sub& b = P.subs[P.geoms[q].sub]; return a.b - a.a < b.b - b.a; });
+    std::vector<int> gnew(ng); std::vector<HGeom> G2; for (int i = 0; i < ng; ++i) { gnew[order[i]] = i; G2.push_back(P.geoms[order[i]]); }
+    P.geoms.swap(G2);
+    for (auto& N : P.nums) N.geom = gnew[N.geom];
+    for (auto& t : P.terms) for (int& q : t.geoms) q = gnew[q];
+    int nn = (int)P.nums.size();
+    std::vector<int> norder(nn); std::iota(norder.begin(), norder.end(), 0);
+    std::stable_sort(norder.begin(), norder.end(), [&](int p, int q) { return P.nums[p].geom < P.nums[q].geom; });
+    std::vector<int> nnew(nn); std::vector<HNum> N2; for (int i = 0; i < nn; ++i) { nnew[norder[i]] = i; N2.push_back(P.nums[norder[i]]); }
+    P.nums.swap(N2);
+    for (auto& nd : P.nodes) nd.num = nnew[nd.num];
+    int nd_n = (int)P.nodes.size();
+    std::vector<int> dorder(nd_n); std::iota(dorder.begin(), dorder.end(), 0);
+    std::stable_sort(dorder.begin(), dorder.end(), [&](int p, int q) { return P.nodes[p].num < P.nodes[q].num; });
+    std::vector<int> dnew(nd_n); std::vector<HNode> D2; for (int i = 0; i < nd_n; ++i) { dnew[dorder[i]] = i; D2.push_back(P.nodes[dorder[i]]); }
+    P.nodes.swap(D2);
+    for (auto& nd : P.nodes) { for (int& k : nd.se_kid) k = dnew[k]; for (int& k : nd.vc_kid) k = dnew[k]; }
+    for (auto& t : P.terms) t.top = dnew[t.top];
+    for (int i = 0; i < nd_n; ++i) P.nums[P.nodes[i].num].nodes.push_back(i);
+  }
+  // Dirac tables -> records
+  for (auto& N : P.nums) build_records(P.geoms[N.geom], P.subs[P.geoms[N.geom].sub].type, N);
+  // flatten
+  P.d_geoms.resize(P.geoms.size());
+  for (size_t i = 0; i < P.geoms.size(); ++i) {
+    const HGeom& E = P.geoms[i]; FgGeomDev d; std::memset(&d, 0, sizeof(d));
+    d.ne = (uint8_t)E.ne; d.l = (uint8_t)E.l; d.has_x = E.has_x;
+    for (int q = 0; q < E.ne; ++q) { d.line_e[q] = (uint8_t)E.own_e[q]; d.eta[q] = (uint8_t)E.eta[q]; d.xiq[q] = (int8_t)E.xiq[q]; }
+    for (int a = 0; a < E.l; ++a) d.line_ph[a] = (uint8_t)E.own_ph[a];
+    P.d_geoms[i] = d;
+  }
+  P.d_geom_num_begin.assign(P.geoms.size() + 1, 0);
+  int raw_max = 0;
+  for (size_t i = 0; i < P.nums.size(); ++i) {
+    HNum& N = P.nums[i]; FgNumDev d; std::memset(&d, 0, sizeof(d));
+    d.geom = N.geom; d.op = N.op; d.ncomp = N.ncomp; d.nse = N.nse;
+    d.node_begin = N.nodes.empty() ? 0 : N.nodes.front(); d.node_count = (int)N.nodes.size();
+    d.chunk_begin = (int)(P.d_chunks.size() / FG_CHUNK_BYTES);
+    // pack records into chunks
+    size_t cur = 0; bool open = false; int nrec = 0; size_t base = 0;
+    auto close_chunk = [&]() { if (open) { FgChunkHdr h = {nrec, 0}; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
+    for (auto& r : N.recs) {
+      size_t need = sizeof(FgRecHdr) + r.coef.size() * sizeof(double);
+      if (!open || cur + need > FG_CHUNK_BYTES) { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); nrec = 0; open = true; }
+      FgRecHdr h; std::memset(&h, 0, sizeof(h)); h.nf = (uint8_t)r.nf; h.k = (uint8_t)r.k; h.dst = (uint8_t)r.dst; h.ncomp = (uint8_t)r.ncomp;
+      std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx));
+      std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h);
+      std::memcpy(&P.d_chunks[base + cur], r.coef.data(), r.coef.size() * sizeof(double)); cur += r.coef.size() * sizeof(double);
+      ++nrec;
+    }
+    close_chunk();
+    d.chunk_count = (int)(P.d_chunks.size() / FG_CHUNK_BYTES) - d.chunk_begin;
+    P.d_nums.push_back(d);
+    P.d_geom_num_begin[N.geom + 1] = (int)i + 1;
+    raw_max = std::max(raw_max, (1 << N.nse) * FG_NDEG * N.ncomp);
+    P.n_records += (long)N.recs.size(); P.n_coefs += N.n_coefs; P.n_nonzero += N.n_nonzero;
+    P.exec_flops += N.exec_flops; P.algo_flops += N.algo_flops;
+    std::vector<HRecord>().swap(N.recs);   // the stream is the product; drop the host copy
+  }
+  for (size_t gi = 1; gi <= P.geoms.size(); ++gi) if (P.d_geom_num_begin[gi] < P.d_geom_num_begin[gi - 1]) P.d_geom_num_begin[gi] = P.d_geom_num_begin[gi - 1];
+  for (auto& nd : P.nodes) {
+    FgNodeDev d; std::memset(&d, 0, sizeof(d)); d.num = nd.num; d.ncomp = P.nums[nd.num].ncomp; d.nse = (int)nd.se_kid.size(); d.nvc = (int)nd.vc_kid.size();
+    for (int k = 0; k < d.nse; ++k) d.se_kid[k] = nd.se_kid[k];
+    for (int k = 0; k < d.nvc; ++k) d.vc_kid[k] = nd.vc_kid[k];
+    P.d_nodes.push_back(d);
+  }
+  for (auto& t : P.terms) {
+    FgTermDev d; std::memset(&d, 0, sizeof(d)); d.top = t.top; d.sign = t.sign; d.nmem = (int)t.geoms.size();
+    for (int k = 0; k < d.nmem; ++k) d.geom[k] = t.geoms[k];
+    P.d_terms.push_back(d);
+  }
+  P.raw_slots = raw_max;
+  // scratch per sample: [U,W per geom][raw value][raw abs][node value 2*NDEG][node abs 2*NDEG]
+  P.scratch_slots = 2 * (int)P.geoms.size() + 2 * raw_max + 4 * FG_NDEG * (int)P.nodes.size();
+  build_density(P);
+  // algorithmic flops outside the numerator stream (rough, per sample): geometry + node products + assembly + sampler
+  double extra = 0;
+  for (auto& E : P.geoms) extra += 2.0 * (E.l * E.l * E.l / 3.0 + E.ne * E.l * E.l + E.ne * (E.ne + 1) / 2.0 * E.l + 4.0 * E.ne * E.l);
+  extra += (double)P.nodes.size() * 2.0 * FG_NDEG * FG_NDEG + (double)P.terms.size() * 4.0 * n + 60.0 * P.M;
+  P.algo_flops += extra; P.exec_flops += extra;
+  P.plan_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+  return FG_OK;
+}
+
+}  // namespace fg

@@ -1,0 +1,84 @@
+// fg_tables.h — plain-old-data tables the host planner writes and the sm_100a kernels read.
+// Notation follows PAPER.md (arXiv:1909.08015) Sec. II-III and DESIGN.md.
+#pragma once
+#include <stdint.h>
+
+#define FG_MAXL 5          // loops n <= 5
+#define FG_MAXNE 10        // own electron lines of one element <= 2n
+#define FG_MAXLINES 15     // 3n
+#define FG_MAXM 15         // Feynman variables (3n, or 3n-1 after the merge of PAPER.md:222)
+#define FG_NDEG 6          // polynomial in t: degrees 0..5
+#define FG_KMAX 6          // free variables of one numerator record (dense 2^k table)
+#define FG_MAXF 10         // product factors of one record
+#define FG_CHUNK_BYTES 8192   // numerator stream is cut into chunks of this size (records never straddle)
+#define FG_MAXSE 4         // self-energy children of one element
+#define FG_MAXVC 5         // vertexlike children of one element
+#define FG_MAXMEM 8        // members of one forest
+#define FG_VMAX (FG_MAXNE * (FG_MAXNE + 1) / 2 + 2 * FG_MAXNE)   // beta (upper triangle), A, A^q
+
+// Operators of the forest formula R^new
+enum { FG_OP_A = 0, FG_OP_U = 1, FG_OP_L = 2, FG_OP_LMU = 3 };
+
+// Element geometry: forest member S with its children shrunk.
+struct FgGeomDev {
+  uint8_t ne, l, has_x, pad;
+  uint8_t line_e[FG_MAXNE];   // global line id of own electron line q (path order)
+  uint8_t line_ph[FG_MAXL];   // global line id of own photon a
+  uint8_t eta[FG_MAXNE];      // bit a set: own electron line q lies on loop a
+  int8_t xiq[FG_MAXNE];       // -1 before the site of v_x, +1 after, 0 if v_x is not in S
+};
+
+// (geometry, operator): one numerator program.  Its raw accumulators are R[sig][comp][deg].
+struct FgNumDev {
+  int32_t geom, op, ncomp, nse;        // ncomp 2 for self-energy elements (u, v), else 1; nse = # self-energy children
+  int32_t chunk_begin, chunk_count;    // range in the chunk stream
+  int32_t node_begin, node_count;      // nodes that use this program
+};
+
+// Value node: a program together with the complete subtree below it.
+struct FgNodeDev {
+  int32_t num, ncomp, nse, nvc;
+  int32_t se_kid[FG_MAXSE];   // node ids, order = signature bits
+  int32_t vc_kid[FG_MAXVC];   // node ids
+};
+
+// One (F, G') term of the forest formula.
+struct FgTermDev {
+  int32_t top;                // node of G
+  int32_t sign;               // (-1)^{|F|-1}
+  int32_t nmem;
+  int32_t geom[FG_MAXMEM];    // geometries of the members (for prod U_S^2 and sum W_S)
+};
+
+// Record header inside a chunk (24 bytes, followed by ncomp * 2^k doubles):
+//   value = prod_{f<nf} V[fidx[f]] * sum_T coef[T] prod_{j in T} V[vidx[j]]   added to accumulator dst
+struct alignas(8) FgRecHdr {
+  uint8_t nf, k, dst, ncomp;
+  uint8_t fidx[FG_MAXF];
+  uint8_t vidx[FG_KMAX];
+  uint8_t pad[4];
+};
+// Chunk header (8 bytes): number of records in the chunk.
+struct FgChunkHdr { int32_t nrec; int32_t pad; };
+
+// Everything the kernels need, passed by value.
+struct FgPlanDev {
+  int32_t n, M, nlines, merge_var;    // merge_var: variable holding the two merged lines, or -1
+  int32_t ngeom, nnum, nnode, nterm;
+  int32_t raw_slots, scratch_slots;   // per-sample scratch doubles: raw accumulators; total
+  uint8_t var_line0[FG_MAXM], var_line1[FG_MAXM];   // lines of each variable (line1 = 255 if single)
+  const FgGeomDev* geoms;
+  const FgNumDev* nums;
+  const FgNodeDev* nodes;
+  const FgTermDev* terms;
+  const int32_t* geom_num_begin;      // nums are sorted by geometry: nums of geom g are [begin[g], begin[g+1])
+  const unsigned char* chunks;        // nchunk * FG_CHUNK_BYTES
+  // density
+  const double* Z1;                   // 2^M
+  const double* Z3;                   // 2^M
+  double C[4], D, lnZfull[4];
+  // precision control
+  double rel_tol, abs_tol, err_eps;
+  double quarter_pow;                 // (-1/4)^n
+  double fact[FG_NDEG];               // k!
+};
