@@ -1,0 +1,228 @@
+"""Thin ctypes binding of the C ABI in include/fg.h (argument marshalling only; every step runs in the CUDA
+kernels of libfg.so).  Names follow the C calls: fg_graph_create -> Graph, fg_plan_create -> Plan,
+fg_integrate -> Plan.integrate, ...  There is no CPU fallback: without libfg.so or without a CUDA device the
+calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfg.so")
+
+EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
+           "fg_plan_info", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
+           "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
+           "fg_dfma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
+
+
+class FgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("fg error %d: %s" % (code, msg))
+        self.code = code
+
+
+class fg_edge(C.Structure):
+    _fields_ = [("u", C.c_int32), ("v", C.c_int32), ("kind", C.c_int32)]
+
+
+class fg_plan_opts(C.Structure):
+    _fields_ = [("C", C.c_double * 4), ("D", C.c_double), ("merge_ext_lines", C.c_int32), ("reserved", C.c_int32),
+                ("deg_table", C.c_void_p), ("rel_tol", C.c_double), ("abs_tol", C.c_double), ("err_factor", C.c_double)]
+
+
+class fg_plan_stats(C.Structure):
+    _fields_ = [("n_loops", C.c_int32), ("M", C.c_int32), ("n_subgraphs", C.c_int32), ("n_forests", C.c_int32),
+                ("n_terms", C.c_int32), ("n_geoms", C.c_int32), ("n_nums", C.c_int32), ("n_nodes", C.c_int32),
+                ("n_records", C.c_int64), ("n_coefs", C.c_int64), ("n_coefs_nonzero", C.c_int64),
+                ("table_bytes", C.c_int64), ("stream_bytes", C.c_int64), ("flops_per_sample", C.c_double),
+                ("exec_flops_per_sample", C.c_double), ("plan_seconds", C.c_double)]
+
+
+class fg_result(C.Structure):
+    _fields_ = [("mean", C.c_double), ("variance", C.c_double), ("sum_y", C.c_double * 2), ("sum_y2", C.c_double * 2),
+                ("n_samples", C.c_uint64), ("n_flagged", C.c_uint64), ("n_rejected", C.c_uint64),
+                ("n_pdf_big_exp", C.c_uint64)]
+
+    def as_dict(self):
+        return dict(mean=self.mean, variance=self.variance, sum_y=(self.sum_y[0], self.sum_y[1]),
+                    sum_y2=(self.sum_y2[0], self.sum_y2[1]), n_samples=int(self.n_samples),
+                    n_flagged=int(self.n_flagged), n_rejected=int(self.n_rejected),
+                    n_pdf_big_exp=int(self.n_pdf_big_exp))
+
+
+_lib = None
+
+
+def lib():
+    """Loads libfg.so (built by paper_1909_08015_b200.build).  Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FgError(-7, "libfg.so is not built (run `python -m paper_1909_08015_b200.build`); there is no CPU path")
+        L = C.CDLL(LIB_PATH)
+        vp = C.c_void_p
+        L.fg_graph_create.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(vp)]
+        L.fg_graph_destroy.argtypes = [vp]
+        L.fg_plan_opts_default.argtypes = [C.POINTER(fg_plan_opts)]
+        L.fg_plan_create.argtypes = [vp, C.POINTER(fg_plan_opts), C.c_int32, C.POINTER(vp)]
+        L.fg_plan_destroy.argtypes = [vp]
+        L.fg_plan_info.argtypes = [vp, C.POINTER(fg_plan_stats)]
+        L.fg_plan_structure.argtypes = [vp, vp, vp, C.c_int32]
+        L.fg_plan_tables.argtypes = [vp, vp, vp]
+        L.fg_integrate.argtypes = [vp, C.c_uint64, C.c_uint64, vp, C.POINTER(fg_result)]
+        L.fg_integrate_range.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp, C.POINTER(fg_result)]
+        L.fg_integrate_async.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp, vp]
+        L.fg_result_merge.argtypes = [C.POINTER(fg_result), C.POINTER(fg_result), C.POINTER(fg_result)]
+        L.fg_sample_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp] + [vp] * 7
+        L.fg_eval_points.argtypes = [vp, vp, C.c_uint64, C.c_int32, vp] + [vp] * 4
+        L.fg_sample_eval_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp] + [vp] * 3
+        L.fg_dfma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        for f in ("fg_strerror", "fg_last_error_message", "fg_version"):
+            getattr(L, f).restype = C.c_char_p
+        L.fg_strerror.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc < 0:
+        raise FgError(rc, "%s: %s" % (lib().fg_strerror(rc).decode(), lib().fg_last_error_message().decode()))
+    return rc
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _stream(stream):
+    if stream is None:
+        return None
+    return C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+
+
+def version():
+    return lib().fg_version().decode()
+
+
+class Graph:
+    """fg_graph_create: edge list (u, v, kind) with kind 0 = electron, 1 = photon; vertex of the external photon."""
+
+    def __init__(self, edges, ext_photon_vertex):
+        arr = (fg_edge * len(edges))(*[fg_edge(int(u), int(v), int(k)) for u, v, k in edges])
+        h = C.c_void_p()
+        _check(lib().fg_graph_create(arr, len(edges), int(ext_photon_vertex), C.byref(h)))
+        self.h = h
+
+    def __del__(self):
+        try:
+            if getattr(self, "h", None):
+                lib().fg_graph_destroy(self.h); self.h = None
+        except Exception:
+            pass
+
+
+class Plan:
+    """fg_plan_create (+ fg_plan_info, fg_integrate, ... on the plan)."""
+
+    def __init__(self, graph, merge_ext_lines=False, C4=None, D=None, deg_table=None, rel_tol=1e-12, abs_tol=0.0,
+                 err_factor=0.0, device=0):
+        o = fg_plan_opts(); lib().fg_plan_opts_default(C.byref(o))
+        if C4 is not None:
+            for k in range(4):
+                o.C[k] = float(C4[k])
+        if D is not None:
+            o.D = float(D)
+        o.merge_ext_lines = int(bool(merge_ext_lines)); o.rel_tol = float(rel_tol); o.abs_tol = float(abs_tol)
+        o.err_factor = float(err_factor)
+        self._deg = None
+        if deg_table is not None:
+            self._deg = np.ascontiguousarray(deg_table, dtype=np.float64); o.deg_table = self._deg.ctypes.data
+        h = C.c_void_p()
+        _check(lib().fg_plan_create(graph.h, C.byref(o), int(device), C.byref(h)))
+        self.h = h
+        self.stats = self.info()
+        self.M = self.stats["M"]
+
+    def __del__(self):
+        try:
+            if getattr(self, "h", None):
+                lib().fg_plan_destroy(self.h); self.h = None
+        except Exception:
+            pass
+
+    def info(self):
+        s = fg_plan_stats(); _check(lib().fg_plan_info(self.h, C.byref(s)))
+        return {k: getattr(s, k) for k, _ in fg_plan_stats._fields_}
+
+    def structure(self):
+        ns = self.stats["n_subgraphs"]
+        subs = np.zeros((ns, 4), dtype=np.int32); buf = np.zeros(1 << 16, dtype=np.int32)
+        w = _check(lib().fg_plan_structure(self.h, _p(subs), _p(buf), len(buf)))
+        ops = {0: "A", 1: "U", 2: "L", 3: "L-U"}
+        terms, i = [], 0
+        while i < w:
+            sign, gp, nm = int(buf[i]), int(buf[i + 1]), int(buf[i + 2]); i += 3
+            terms.append(dict(sign=sign, gprime=gp, members=[(int(buf[i + 2 * k]), ops[int(buf[i + 2 * k + 1])]) for k in range(nm)]))
+            i += 2 * nm
+        return [dict(a=int(r[0]), b=int(r[1]), type="V" if r[2] else "SE", in_chain=bool(r[3])) for r in subs], terms
+
+    def tables(self):
+        d = np.zeros(1 << self.M); z = np.zeros(1 << self.M)
+        _check(lib().fg_plan_tables(self.h, _p(d), _p(z)))
+        return d, z
+
+    def integrate(self, n_samples, seed, stream=None):
+        r = fg_result(); _check(lib().fg_integrate(self.h, int(n_samples), int(seed), _stream(stream), C.byref(r)))
+        return r.as_dict()
+
+    def integrate_range(self, first_sample, n_samples, seed, stream=None, raw=False):
+        r = fg_result()
+        _check(lib().fg_integrate_range(self.h, int(first_sample), int(n_samples), int(seed), _stream(stream), C.byref(r)))
+        return r if raw else r.as_dict()
+
+    def integrate_async(self, first_sample, n_samples, seed, out_dev_ptr, stream=None):
+        """Result (sizeof(fg_result) = 80 bytes) is left at device address out_dev_ptr; no synchronisation."""
+        _check(lib().fg_integrate_async(self.h, int(first_sample), int(n_samples), int(seed), _stream(stream),
+                                        C.c_void_p(int(out_dev_ptr))))
+
+    def sample_dump(self, first, n, seed, stream=None, words=True):
+        M = self.M
+        w = np.zeros((n, M, 4), dtype=np.uint32) if words else None
+        comp = np.zeros(n, dtype=np.int32); order = np.zeros((n, M), dtype=np.uint8); z = np.zeros((n, M))
+        pm = np.zeros(n); pe = np.zeros(n, dtype=np.int32); bad = np.zeros(n, dtype=np.uint8)
+        _check(lib().fg_sample_dump(self.h, int(first), int(n), int(seed), _stream(stream), _p(w), _p(comp), _p(order),
+                                    _p(z), _p(pm), _p(pe), _p(bad)))
+        return dict(words=w, comp=comp, order=order, z=z, pdf_mant=pm, pdf_exp=pe, bad=bad)
+
+    def eval_points(self, z, mode=0, stream=None):
+        z = np.ascontiguousarray(z, dtype=np.float64).reshape(-1, self.M); n = len(z)
+        I = np.zeros(n); Id = np.zeros(n); err = np.zeros(n); fl = np.zeros(n, dtype=np.uint8)
+        _check(lib().fg_eval_points(self.h, _p(z), n, int(mode), _stream(stream), _p(I), _p(Id), _p(err), _p(fl)))
+        return dict(I=I, I_double=Id, err=err, flags=fl)
+
+    def sample_eval_dump(self, first, n, seed, stream=None):
+        I = np.zeros(n); y = np.zeros(n); fl = np.zeros(n, dtype=np.uint8)
+        _check(lib().fg_sample_eval_dump(self.h, int(first), int(n), int(seed), _stream(stream), _p(I), _p(y), _p(fl)))
+        return dict(I=I, y=y, flags=fl)
+
+
+def result_merge(a, b):
+    """fg_result_merge on two raw fg_result structs."""
+    out = fg_result(); _check(lib().fg_result_merge(C.byref(a), C.byref(b), C.byref(out)))
+    return out
+
+
+def dfma_peak(device=0, iters=200000, stream=None):
+    """fg_dfma_peak: measured FP64-FMA throughput (TFLOP/s, FMA = 2) and kernel time in ms."""
+    t = C.c_double(); ms = C.c_double()
+    _check(lib().fg_dfma_peak(int(device), int(iters), _stream(stream), C.byref(t), C.byref(ms)))
+    return t.value, ms.value
+
+
+def plan_for(x, photons, **kw):
+    """Convenience: (x, photons) in the notation of paper_1909_08015_b200.inputs -> Plan."""
+    from . import inputs
+    g = Graph(inputs.edge_list(x, photons), x)
+    return Plan(g, **kw)
