@@ -54,7 +54,7 @@ void fg_graph_destroy(fg_graph*);
  *  deg_table optional host array of 2^M doubles overriding Deg(s); NULL = built-in rule
  *  rel_tol, abs_tol  a sample whose estimated round-off error exceeds max(rel_tol*|I|, abs_tol*g) is
  *            re-evaluated in double-double (abs_tol plays the role of sigma/4 in (18))
- *  err_factor safety factor of the running error estimate (0 = default)                                   */
+ *  err_factor safety factor K of the running error estimate K*2^-53*sum|terms| (0 = default 8)                                 */
 typedef struct {
   double C[4];
   double D;
@@ -70,6 +70,15 @@ void fg_plan_opts_default(fg_plan_opts* o);
  * tables; then uploads them to `device`.  "fg_plan" in BASELINE.json. */
 int fg_plan_create(const fg_graph*, const fg_plan_opts*, int32_t device, fg_plan** out);
 void fg_plan_destroy(fg_plan*);
+
+/* Changes the acceptance tolerances of an existing plan (e.g. after a pilot run has measured sigma). */
+int fg_plan_set_tol(fg_plan*, double rel_tol, double abs_tol);
+
+/* Per-kernel device timing (CUDA events on the launching stream).  While enabled every slab of an integration
+ * ends with an event synchronisation.  fg_plan_timing returns the milliseconds accumulated since fg_plan_profile:
+ * ms3[0] double-precision pass, ms3[1] double-double pass, ms3[2] final reduction; and the kernels launched. */
+int fg_plan_profile(fg_plan*, int32_t enable);
+int fg_plan_timing(const fg_plan*, double* ms3, int64_t* launches);
 
 typedef struct {
   int32_t n_loops, M;                 /* loops, number of Feynman variables */

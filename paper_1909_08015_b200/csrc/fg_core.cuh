@@ -112,56 +112,65 @@ FG_HD void draw_sample(const FgPlanDev& P, const double* __restrict__ Z1, const 
 // a5  geometry of one element at one point.  Loop a = own photon a plus the own electron lines between its ends:
 //   B_ab = sum_j z_j eta_ja eta_jb + delta_ab z_gamma_a,  U = det B,  C_a = sum_j z_j eta_ja,  W = C^T B^-1 C,
 //   A_j = 1 - eta_j^T B^-1 C,  beta_ij = eta_i^T B^-1 eta_j,  A^q_j = xi^q_j - eta_j^T B^-1 C^q.
-// B = L D L^T (no square roots); growth = max_a B_aa / d_a measures the cancellation in the pivots.
-// V receives beta (upper triangle, row-major), then A, then A^q, element idx at V[idx * vs].
+// B = L D L^T (no square roots).  This step is always carried out in double-double, whatever the precision of the
+// numerator pass: it is a few per cent of the work at 5 loops and it removes the cancellations of the pivots,
+// of 1 - sum and of the beta dot products from the double-precision pass.
+// V receives beta (upper triangle, row-major), then A, then A^q, element idx at V[idx * vs]; amax = max(1,|A|,|A^q|).
 // ------------------------------------------------------------------------------------------------
+template <class T> FG_HD T from_dd(dd a);
+template <> FG_HD double from_dd<double>(dd a) { return a.hi + a.lo; }
+template <> FG_HD dd from_dd<dd>(dd a) { return a; }
+
 template <class T>
-FG_HD void geom_eval(const FgGeomDev& E, const T* zl, T* V, int vs, T& U, T& W, double& growth) {
+FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T& W, double& amax) {
   const int l = E.l, ne = E.ne;
-  T B[FG_MAXL][FG_MAXL], C[FG_MAXL], Cq[FG_MAXL], invd[FG_MAXL];
-  for (int a = 0; a < l; ++a) { C[a] = T(0.0); Cq[a] = T(0.0); for (int b = 0; b < l; ++b) B[a][b] = T(0.0); }
+  dd B[FG_MAXL][FG_MAXL], C[FG_MAXL], Cq[FG_MAXL], invd[FG_MAXL];
+  for (int a = 0; a < l; ++a) { C[a] = dd(0.0); Cq[a] = dd(0.0); for (int b = 0; b < l; ++b) B[a][b] = dd(0.0); }
   for (int q = 0; q < ne; ++q) {
-    const T z = zl[E.line_e[q]]; const unsigned m = E.eta[q]; const int xq = E.xiq[q];
-    const T zh = t_halve(z);
+    const double z = zl[E.line_e[q]]; const unsigned m = E.eta[q]; const int xq = E.xiq[q];
+    const double zh = xq > 0 ? 0.5 * z : -0.5 * z;
     for (int a = 0; a < l; ++a) if ((m >> a) & 1u) {
-      C[a] = C[a] + z;
-      if (xq > 0) Cq[a] = Cq[a] + zh; else if (xq < 0) Cq[a] = Cq[a] - zh;
-      for (int b = 0; b <= a; ++b) if ((m >> b) & 1u) B[a][b] = B[a][b] + z;
+      C[a] = dd_add_d(C[a], z);
+      if (xq != 0) Cq[a] = dd_add_d(Cq[a], zh);
+      for (int b = 0; b <= a; ++b) if ((m >> b) & 1u) B[a][b] = dd_add_d(B[a][b], z);
     }
   }
-  for (int a = 0; a < l; ++a) B[a][a] = B[a][a] + zl[E.line_ph[a]];
-  U = T(1.0); double gr = 1.0;
+  for (int a = 0; a < l; ++a) B[a][a] = dd_add_d(B[a][a], zl[E.line_ph[a]]);
+  dd u(1.0);
   for (int a = 0; a < l; ++a) {
-    T d = B[a][a];
-    for (int b = 0; b < a; ++b) d = d - B[a][b] * B[a][b] * B[b][b];     // B[b][b] now holds d_b, B[a][b] holds L_ab
-    const double g1 = to_double(B[a][a]) / to_double(d); if (g1 > gr || !(g1 == g1)) gr = g1;
-    invd[a] = T(1.0) / d; U = U * d;
+    dd d = B[a][a];
+    for (int b = 0; b < a; ++b) d = d - B[a][b] * B[a][b] * B[b][b];     // B[b][b] holds d_b, B[a][b] holds L_ab
+    invd[a] = dd(1.0) / d; u = u * d;
     for (int c = a + 1; c < l; ++c) {
-      T t = B[c][a];
+      dd t = B[c][a];
       for (int b = 0; b < a; ++b) t = t - B[c][b] * B[a][b] * B[b][b];
       B[c][a] = t * invd[a];
     }
     B[a][a] = d;
   }
-  growth = gr;
-  // x = L^-1 C, xq = L^-1 C^q
-  for (int a = 0; a < l; ++a) for (int b = 0; b < a; ++b) { C[a] = C[a] - B[a][b] * C[b]; Cq[a] = Cq[a] - B[a][b] * Cq[b]; }
-  T w = T(0.0); for (int a = 0; a < l; ++a) w = w + C[a] * C[a] * invd[a];
-  W = w;
-  T Y[FG_MAXNE][FG_MAXL];
-  const int nb = ne * (ne + 1) / 2;
+  U = from_dd<T>(u);
+  for (int a = 0; a < l; ++a) for (int b = 0; b < a; ++b) { C[a] = C[a] - B[a][b] * C[b]; Cq[a] = Cq[a] - B[a][b] * Cq[b]; }   // L^-1 C, L^-1 C^q
+  dd w(0.0); for (int a = 0; a < l; ++a) { w = w + C[a] * C[a] * invd[a]; C[a] = C[a] * invd[a]; Cq[a] = Cq[a] * invd[a]; }
+  W = from_dd<T>(w);
+  dd Y[FG_MAXNE][FG_MAXL];
+  const int nb = ne * (ne + 1) / 2; double am = 1.0;
   for (int q = 0; q < ne; ++q) {
     const unsigned m = E.eta[q];
-    for (int a = 0; a < l; ++a) { T y = ((m >> a) & 1u) ? T(1.0) : T(0.0); for (int b = 0; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
-    T sa = T(0.0), sq = T(0.0);
-    for (int a = 0; a < l; ++a) { T yd = Y[q][a] * invd[a]; sa = sa + yd * C[a]; sq = sq + yd * Cq[a]; }
-    V[(nb + q) * vs] = T(1.0) - sa;
-    V[(nb + ne + q) * vs] = T(0.5 * (double)E.xiq[q]) - sq;
+    for (int a = 0; a < l; ++a) { dd y = ((m >> a) & 1u) ? dd(1.0) : dd(0.0); for (int b = 0; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
+    dd sa(0.0), sq(0.0);
+    for (int a = 0; a < l; ++a) { sa = sa + Y[q][a] * C[a]; sq = sq + Y[q][a] * Cq[a]; }
+    const dd A = dd(1.0) - sa, Aq = dd(0.5 * (double)E.xiq[q]) - sq;
+    V[(nb + q) * vs] = from_dd<T>(A); V[(nb + ne + q) * vs] = from_dd<T>(Aq);
+    am = fmax(am, fmax(fabs(A.hi), fabs(Aq.hi)));
   }
+  amax = am;
   int idx = 0;
-  for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) {
-    T b = T(0.0); for (int a = 0; a < l; ++a) b = b + Y[i][a] * Y[j][a] * invd[a];
-    V[idx * vs] = b; ++idx;
+  for (int i = 0; i < ne; ++i) {
+    dd yd[FG_MAXL]; for (int a = 0; a < l; ++a) yd[a] = Y[i][a] * invd[a];
+    for (int j = i; j < ne; ++j) {
+      dd b(0.0); for (int a = 0; a < l; ++a) b = b + yd[a] * Y[j][a];
+      V[idx * vs] = from_dd<T>(b); ++idx;
+    }
   }
 }
 
@@ -190,30 +199,97 @@ template <int S> struct Horner<double, S, 1> {   // leaf FMA takes both coeffici
     for (int s = 0; s < S; ++s) out[s] = fma(a[0][s], c1, c0);
   }
 };
+// q-extension: q += sum_j aq[j] * (multilinear in the K-1 variables other than j)
+template <class T, int S, int K> struct QExt {
+  static FG_HD void run(const double* __restrict__ cq, const T (*a)[S], const T (*aq)[S], T* q) {
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+      T b[K > 1 ? K - 1 : 1][S], sub[S];
+#pragma unroll
+      for (int i = 0; i + 1 < K; ++i) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) b[i][s] = a[i < j ? i : i + 1][s];
+      }
+      Horner<T, S, K - 1>::run(cq + j * (1 << (K - 1)), b, sub);
+#pragma unroll
+      for (int s = 0; s < S; ++s) q[s] = t_fma(aq[j][s], sub[s], q[s]);
+    }
+  }
+};
+template <class T, int S> struct QExt<T, S, 0> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
-// One record: value[s] = prod_f V[fidx[f]] * sum_T coef[T] prod_{j in T} V[vidx[j]]
-template <class T, int S>
-FG_HD void eval_record(const FgRecHdr& h, const double* __restrict__ coef, const T* __restrict__ Vt, int vs, T (*q)[S], T* prod) {
+// Running state of one program: prefix products of the factor list, accumulators of the current destination.
+template <class T, int S> struct RecState { T p[FG_MAXF][S]; T acc[2][S]; double aab[2][S]; int cur; };
+
+FG_HD int rec_ncoef(int k, int flags) {
+  const int n = (flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k;
+  return (n + 1) & ~1;
+}
+
+// All records of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
+template <class T, int S, bool ABS, class Flush>
+FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st, Flush&& flush) {
+#if defined(__CUDA_ARCH__)
+  __builtin_assume(__isShared(chunk)); __builtin_assume(__isShared(Vt));   // LDS instead of generic loads
+#endif
+  const int nrec = ((const FgChunkHdr*)chunk)->nrec;
+  int off = (int)sizeof(FgChunkHdr);
+  for (int r = 0; r < nrec; ++r) {
+    const FgRecHdr h = *(const FgRecHdr*)(chunk + off);
+    const double* __restrict__ coef = (const double*)(chunk + off + sizeof(FgRecHdr));
+    const int nf = h.nf, k = h.k, flags = h.flags, keep = flags >> 4;
+    if ((int)h.dst != st.cur) {
+      if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
+      st.cur = h.dst;
 #pragma unroll
-  for (int s = 0; s < S; ++s) prod[s] = T(1.0);
-  for (int f = 0; f < h.nf; ++f) {
-    const T* p = Vt + (int)h.fidx[f] * vs;
+      for (int s = 0; s < S; ++s) { st.acc[0][s] = T(0.0); st.acc[1][s] = T(0.0); st.aab[0][s] = 0.0; st.aab[1][s] = 0.0; }
+    }
+    T prod[S];
 #pragma unroll
-    for (int s = 0; s < S; ++s) prod[s] = prod[s] * p[s];
-  }
-  T a[FG_KMAX][S];
+    for (int s = 0; s < S; ++s) prod[s] = T(1.0);
 #pragma unroll
-  for (int j = 0; j < FG_KMAX; ++j) if (j < h.k) {
-    const T* p = Vt + (int)h.vidx[j] * vs;
+    for (int f = 0; f < FG_MAXF; ++f) if (f < nf) {
+      if (f >= keep) {
+        const T* pv = Vt + (int)h.fidx[f] * vs;
 #pragma unroll
-    for (int s = 0; s < S; ++s) a[j][s] = p[s];
-  }
-  const int nc = h.ncomp;
-  switch (h.k) {
-#define FG_CASE(K) case K: Horner<T, S, K>::run(coef, a, q[0]); if (nc == 2) Horner<T, S, K>::run(coef + (1 << K), a, q[1]); break;
-    FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4) FG_CASE(5) FG_CASE(6)
+        for (int s = 0; s < S; ++s) st.p[f][s] = (f == 0) ? pv[s] : st.p[f > 0 ? f - 1 : 0][s] * pv[s];
+      }
+      if (f == nf - 1) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) prod[s] = st.p[f][s];
+      }
+    }
+    T a[FG_KMAX][S], aq[FG_KMAX][S];
+#pragma unroll
+    for (int j = 0; j < FG_KMAX; ++j) if (j < k) {
+      const T* pv = Vt + (int)h.vidx[j] * vs;
+#pragma unroll
+      for (int s = 0; s < S; ++s) a[j][s] = pv[s];
+      if (flags & FG_REC_QEXT) {
+        const T* pq = pv + ne * vs;
+#pragma unroll
+        for (int s = 0; s < S; ++s) aq[j][s] = pq[s];
+      }
+    }
+    T q[2][S];
+    switch (k) {
+#define FG_CASE(K) case K: Horner<T, S, K>::run(coef, a, q[0]); \
+                           if (flags & FG_REC_TWO) Horner<T, S, K>::run(coef + (1 << K), a, q[1]); \
+                           else if (flags & FG_REC_QEXT) QExt<T, S, K>::run(coef + (1 << K), a, aq, q[0]); break;
+      FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4) FG_CASE(5) FG_CASE(6)
 #undef FG_CASE
-    default: break;
+      default: break;
+    }
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      st.acc[0][s] = t_fma(prod[s], q[0][s], st.acc[0][s]);
+      if (ABS) st.aab[0][s] = fma(t_abs_d(prod[s]), (double)h.cabs[0], st.aab[0][s]);
+      if (flags & FG_REC_TWO) {
+        st.acc[1][s] = t_fma(prod[s], q[1][s], st.acc[1][s]);
+        if (ABS) st.aab[1][s] = fma(t_abs_d(prod[s]), (double)h.cabs[1], st.aab[1][s]);
+      }
+    }
+    off += (int)sizeof(FgRecHdr) + rec_ncoef(k, flags) * (int)sizeof(double);
   }
 }
 

@@ -52,7 +52,7 @@ struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2]; };
 
 // a6: run the record stream of one program for the S samples of this thread
 template <class T, int S, bool ABS>
-__device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const T* Vt, int vs, T* Sc, int ss) {
+__device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const T* Vt, int vs, int ne, T* Sc, int ss) {
   const int nslots = (1 << N.nse) * FG_NDEG * N.ncomp;
   for (int i = 0; i < nslots; ++i) {
 #pragma unroll
@@ -65,68 +65,49 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     mbar_expect_tx(&ring.bar[0], FG_CHUNK_BYTES); bulk_g2s(ring.buf, g0, FG_CHUNK_BYTES, &ring.bar[0]);
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], FG_CHUNK_BYTES); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[1]); }
   }
-  int cur = -1; T acc[2][S], aab[2][S];
-  auto flush = [&]() {
-    if (cur < 0) return;
-    for (int c = 0; c < N.ncomp; ++c) {
+  RecState<T, S> st; st.cur = -1;
+  const int nc = N.ncomp, rawv = sm.rawv, rawa = sm.rawa;
+  auto flush = [&](int dst, const T (*acc)[S], const double (*aab)[S]) {
+    for (int c = 0; c < nc; ++c) {
 #pragma unroll
-      for (int s = 0; s < S; ++s) { Sc[(sm.rawv + cur * N.ncomp + c) * ss + s] = acc[c][s]; if (ABS) Sc[(sm.rawa + cur * N.ncomp + c) * ss + s] = aab[c][s]; }
+      for (int s = 0; s < S; ++s) { Sc[(rawv + dst * nc + c) * ss + s] = acc[c][s]; if (ABS) Sc[(rawa + dst * nc + c) * ss + s] = T(aab[c][s]); }
     }
   };
   for (int ch = 0; ch < nch; ++ch) {
     const int b = ch & 1;
     mbar_wait(&ring.bar[b], ring.phase[b]); ring.phase[b] ^= 1u;
-    const unsigned char* p = ring.buf + b * FG_CHUNK_BYTES;
-    const int nrec = ((const FgChunkHdr*)p)->nrec;
-    int off = sizeof(FgChunkHdr);
-    for (int r = 0; r < nrec; ++r) {
-      const FgRecHdr h = *(const FgRecHdr*)(p + off);
-      const double* coef = (const double*)(p + off + sizeof(FgRecHdr));
-      if ((int)h.dst != cur) {
-        flush(); cur = h.dst;
-#pragma unroll
-        for (int s = 0; s < S; ++s) { acc[0][s] = T(0.0); acc[1][s] = T(0.0); aab[0][s] = T(0.0); aab[1][s] = T(0.0); }
-      }
-      T q[2][S], prod[S];
-      eval_record<T, S>(h, coef, Vt, vs, q, prod);
-#pragma unroll
-      for (int s = 0; s < S; ++s) {
-        const T t0 = prod[s] * q[0][s]; acc[0][s] = acc[0][s] + t0; if (ABS) aab[0][s] = aab[0][s] + T(t_abs_d(t0));
-        if (h.ncomp == 2) { const T t1 = prod[s] * q[1][s]; acc[1][s] = acc[1][s] + t1; if (ABS) aab[1][s] = aab[1][s] + T(t_abs_d(t1)); }
-      }
-      off += (int)sizeof(FgRecHdr) + ((int)h.ncomp << h.k) * (int)sizeof(double);
-    }
+    run_chunk<T, S, ABS>(ring.buf + b * FG_CHUNK_BYTES, Vt, vs, ne, st, flush);
     __syncthreads();   // every thread is done with buffer b
     if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], FG_CHUNK_BYTES); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[b]); }
   }
-  flush();
+  if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
 }
 
 // a5-a7 for the S points of this thread
 template <class T, int S, bool ABS>
-__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* growth) {
+__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* amp) {
   const ScratchMap sm(P);
-  T zl[S][FG_MAXLINES];
+  double zl[S][FG_MAXLINES];
 #pragma unroll
   for (int s = 0; s < S; ++s) {
     for (int v = 0; v < P.M; ++v) {
       const int l0 = P.var_line0[v], l1 = P.var_line1[v];
-      if (l1 == 255) zl[s][l0] = T(z[s][v]); else { zl[s][l0] = T(0.5 * z[s][v]); zl[s][l1] = T(0.5 * z[s][v]); }
+      if (l1 == 255) zl[s][l0] = z[s][v]; else { zl[s][l0] = 0.5 * z[s][v]; zl[s][l1] = 0.5 * z[s][v]; }
     }
-    growth[s] = 1.0;
+    amp[s] = 1.0;
   }
   for (int g = 0; g < P.ngeom; ++g) {
     const FgGeomDev E = P.geoms[g];
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      T U, W; double gr;
-      geom_eval<T>(E, zl[s], Vt + s, vs, U, W, gr);
+      T U, W; double am;
+      geom_eval<T>(E, zl[s], Vt + s, vs, U, W, am);
       Sc[(2 * g) * ss + s] = U; Sc[(2 * g + 1) * ss + s] = W;
-      if (gr > growth[s] || !(gr == gr)) growth[s] = gr;
+      if (am > amp[s] || !(am == am)) amp[s] = am;
     }
     for (int ni = P.geom_num_begin[g]; ni < P.geom_num_begin[g + 1]; ++ni) {
       const FgNumDev N = P.nums[ni];
-      run_program<T, S, ABS>(P, N, sm, ring, Vt, vs, Sc, ss);
+      run_program<T, S, ABS>(P, N, sm, ring, Vt, vs, (int)E.ne, Sc, ss);
       for (int k = 0; k < N.node_count; ++k) {
 #pragma unroll
         for (int s = 0; s < S; ++s) { finish_node<T, false>(P, sm, N.node_begin + k, Sc + s, ss); if (ABS) finish_node<T, true>(P, sm, N.node_begin + k, Sc + s, ss); }
@@ -181,7 +162,8 @@ __global__ void __launch_bounds__(NT) fg_eval_kernel(const FgPlanDev P, const Ru
     for (int s = 0; s < S; ++s) {
       if (!valid[s]) continue;
       const double Id = to_double(I[s]);
-      const double err = is_dd<T>::value ? 0.0 : P.err_eps * growth[s] * Iabs[s];
+      double af = growth[s] * growth[s]; af = af * af * af;      // |A|, |A^q| <= 1 is assumed by cabs; amax^6 otherwise
+      const double err = is_dd<T>::value ? 0.0 : P.err_eps * af * Iabs[s];
       uint8_t fl = 0; double y = 0.0;
       if (ex[s] > 1023 || ex[s] < -1021) ++nbig;
       if (bad[s]) { ++nrej; fl = 2; }
@@ -286,6 +268,7 @@ struct fg_plan {
   uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr;
   int grid_d = 0, grid_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
   int64_t table_bytes = 0;
+  int profile = 0; cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; double ms[3] = {0, 0, 0}; long long launches = 0, flagged_last = 0;
   std::mutex mu;
 };
 
@@ -332,6 +315,7 @@ void fg_plan_destroy(fg_plan* p) {
   if (!p) return;
   cudaSetDevice(p->device);
   for (void* a : p->allocs) cudaFree(a);
+  for (int k = 0; k < 4; ++k) if (p->ev[k]) cudaEventDestroy(p->ev[k]);
   delete p;
 }
 
@@ -360,7 +344,7 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   for (int v = 0; v < H.M; ++v) { D.var_line0[v] = (uint8_t)H.var_lines[v][0]; D.var_line1[v] = H.var_lines[v].size() > 1 ? (uint8_t)H.var_lines[v][1] : 255; }
   for (int k = 0; k < 4; ++k) { D.C[k] = H.opts.C[k]; D.lnZfull[k] = H.lnZfull[k]; }
   D.D = H.opts.D; D.rel_tol = po.rel_tol; D.abs_tol = po.abs_tol;
-  D.err_eps = (po.err_factor > 0 ? po.err_factor : 64.0) * 0x1p-53;
+  D.err_eps = (po.err_factor > 0 ? po.err_factor : 8.0) * 0x1p-53;
   D.quarter_pow = std::pow(-0.25, H.g.n); D.fact[0] = 1; for (int k = 1; k < FG_NDEG; ++k) D.fact[k] = D.fact[k - 1] * k;
 #define UP(vec, field) do { int rc_ = upload(p, vec, &D.field); if (rc_ != FG_OK) { fg_plan_destroy(p); return rc_; } } while (0)
   UP(H.d_geoms, geoms); UP(H.d_nums, nums); UP(H.d_nodes, nodes); UP(H.d_terms, terms); UP(H.d_geom_num_begin, geom_num_begin);
@@ -384,6 +368,27 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   if (e == cudaSuccess) e = dmalloc((void**)&p->flag_count, sizeof(unsigned long long));
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
   *out = p; return FG_OK;
+}
+
+int fg_plan_set_tol(fg_plan* p, double rel_tol, double abs_tol) {
+  if (!p || !(rel_tol >= 0) || !(abs_tol >= 0)) return fail(FG_E_ARG, "bad tolerance");
+  std::lock_guard<std::mutex> lk(p->mu);
+  p->D.rel_tol = rel_tol; p->D.abs_tol = abs_tol; return FG_OK;
+}
+
+int fg_plan_profile(fg_plan* p, int32_t enable) {
+  if (!p) return fail(FG_E_ARG, "NULL plan");
+  std::lock_guard<std::mutex> lk(p->mu);
+  CU(cudaSetDevice(p->device));
+  if (enable) for (int k = 0; k < 4; ++k) if (!p->ev[k]) CU(cudaEventCreate(&p->ev[k]));
+  p->profile = enable ? 1 : 0; p->ms[0] = p->ms[1] = p->ms[2] = 0; p->launches = 0;
+  return FG_OK;
+}
+int fg_plan_timing(const fg_plan* p, double* ms3, int64_t* launches) {
+  if (!p) return fail(FG_E_ARG, "NULL plan");
+  if (ms3) for (int k = 0; k < 3; ++k) ms3[k] = p->ms[k];
+  if (launches) *launches = p->launches;
+  return FG_OK;
 }
 
 int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
@@ -430,19 +435,27 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
     uint64_t nbatch = (n + (uint64_t)NT_D * S_D - 1) / ((uint64_t)NT_D * S_D);
     int grid = (int)std::min<uint64_t>((uint64_t)p->grid_d, std::max<uint64_t>(nbatch, 1));
     CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
+    if (p->profile) CU(cudaEventRecord(p->ev[0], st));
     fg_eval_kernel<double, S_D, NT_D><<<grid, NT_D, p->smem_d, st>>>(p->D, A);
-    CU(cudaGetLastError());
+    CU(cudaGetLastError()); ++p->launches;
+    if (p->profile) CU(cudaEventRecord(p->ev[1], st));
     nparts = p->grid_d;
   } else CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
   if (mode == 0 || mode == 2) {
     RunArgs B = A; B.do_flag = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
     if (mode == 0) { B.idlist = p->flag_list; B.idcount = p->flag_count; }
+    if (p->profile && mode == 2) { CU(cudaEventRecord(p->ev[0], st)); CU(cudaEventRecord(p->ev[1], st)); }
     fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, NT_Q, p->smem_q, st>>>(p->D, B);
-    CU(cudaGetLastError());
+    CU(cudaGetLastError()); ++p->launches;
     nparts = p->grid_d + p->grid_q;
   }
+  if (p->profile) CU(cudaEventRecord(p->ev[2], st));
   fg_reduce_kernel<<<1, 32, 0, st>>>(p->partials, nparts, p->accum, (unsigned long long)n, finalize ? 1 : 0, out_dev);
-  CU(cudaGetLastError());
+  CU(cudaGetLastError()); ++p->launches;
+  if (p->profile) {
+    CU(cudaEventRecord(p->ev[3], st)); CU(cudaEventSynchronize(p->ev[3]));
+    for (int k = 0; k < 3; ++k) { float t = 0; CU(cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1])); p->ms[k] += t; }
+  }
   return FG_OK;
 }
 

@@ -281,18 +281,49 @@ static void matching_table(const HGeom& E, int type, int op, int comp, const Mat
   for (auto& c : out) c *= pref;
 }
 
-static void build_records(const HGeom& E, int type, HNum& N) {
+static void finish_record(HRecord& r) {
+  r.cabs[0] = r.cabs[1] = 0.f;
+  if (r.flags & FG_REC_TWO) { size_t h = (size_t)1 << r.k; double a0 = 0, a1 = 0; for (size_t i = 0; i < h; ++i) { a0 += std::fabs(r.coef[i]); a1 += std::fabs(r.coef[h + i]); } r.cabs[0] = (float)(a0 * 1.0000002); r.cabs[1] = (float)(a1 * 1.0000002); }
+  else { double a0 = 0; for (double v : r.coef) a0 += std::fabs(v); r.cabs[0] = (float)(a0 * 1.0000002); }
+  if (r.coef.size() & 1) r.coef.push_back(0.0);
+}
+
+static void build_records(const HGeom& E, int type, HNum& N, bool& limit_hit) {
   int ns = (int)E.slots.size(), ne = E.ne, nb = ne * (ne + 1) / 2;
   auto bidx = [&](int i, int j) { if (i > j) std::swap(i, j); return i * ne - i * (i - 1) / 2 + (j - i); };
   std::vector<Matching> ms; enum_matchings(ns, ms);
   std::vector<std::vector<HRecord>> per(ms.size());
-  int ncomp = N.ncomp;
+  int ncomp = N.ncomp; bool over = false;
 #pragma omp parallel for schedule(dynamic, 1)
   for (long mi = 0; mi < (long)ms.size(); ++mi) {
     const Matching& m = ms[mi];
     int npairs = (int)m.pairs.size();
+    int sig0 = 0; std::vector<int> f0;
+    for (auto& pr : m.pairs) { f0.push_back(bidx(E.slots[pr[0]].e, E.slots[pr[1]].e)); for (int t = 0; t < 2; ++t) if (E.slots[pr[t]].se >= 0) sig0 |= 1 << E.slots[pr[t]].se; }
+    bool wantq = (N.op == FG_OP_A && type == 1);
+    bool pseudo = false; for (int s : m.unmatched) if (E.slots[s].se >= 0) pseudo = true;
+    int k = (int)m.unmatched.size();
+    if (wantq && !pseudo && k >= 1 && k <= FG_KMAX) {
+      // one record for the whole matching: main table + one table per slot that may carry gamma^nu A^q
+      std::vector<double> main_t; matching_table(E, type, N.op, 0, m, -1, false, m.unmatched, main_t);
+      HRecord r; r.nf = npairs; r.k = k; r.dst = sig0 * FG_NDEG + npairs; r.flags = 0;
+      std::memset(r.fidx, 0, sizeof(r.fidx)); std::memset(r.vidx, 0, sizeof(r.vidx));
+      for (int t = 0; t < r.nf; ++t) r.fidx[t] = (uint8_t)f0[t];
+      for (int t = 0; t < k; ++t) r.vidx[t] = (uint8_t)(nb + E.slots[m.unmatched[t]].e);
+      r.coef = main_t; bool nz = false, nzq = false; for (double v : main_t) if (v != 0.0) nz = true;
+      std::vector<double> qall;
+      for (int j = 0; j < k; ++j) {
+        std::vector<int> gaps; for (int s : m.unmatched) if (s != m.unmatched[j]) gaps.push_back(s);
+        std::vector<double> qt; matching_table(E, type, N.op, 0, m, m.unmatched[j], true, gaps, qt);
+        for (double v : qt) if (v != 0.0) nzq = true;
+        qall.insert(qall.end(), qt.begin(), qt.end());
+      }
+      if (nzq) { r.flags |= FG_REC_QEXT; r.coef.insert(r.coef.end(), qall.begin(), qall.end()); }
+      if (nz || nzq) { finish_record(r); per[mi].push_back(std::move(r)); }
+      continue;
+    }
     std::vector<int> qchoices = {-1};
-    if (N.op == FG_OP_A && type == 1) for (int s : m.unmatched) qchoices.push_back(s);
+    if (wantq) for (int s : m.unmatched) qchoices.push_back(s);
     for (int q : qchoices) {
       std::vector<int> gaps; for (int s : m.unmatched) if (s != q) gaps.push_back(s);
       std::vector<double> tab[2];
@@ -303,12 +334,12 @@ static void build_records(const HGeom& E, int type, HNum& N) {
       std::vector<int> en, fr;   // positions in `gaps`
       for (int gi = 0; gi < (int)gaps.size(); ++gi) { if (E.slots[gaps[gi]].se >= 0) en.push_back(gi); else fr.push_back(gi); }
       while ((int)fr.size() > FG_KMAX) { en.push_back(fr.back()); fr.pop_back(); }
-      int sig0 = 0; std::vector<int> f0;
-      for (auto& pr : m.pairs) { f0.push_back(bidx(E.slots[pr[0]].e, E.slots[pr[1]].e)); for (int t = 0; t < 2; ++t) if (E.slots[pr[t]].se >= 0) sig0 |= 1 << E.slots[pr[t]].se; }
-      if (q >= 0) { f0.push_back(nb + ne + E.slots[q].e); if (E.slots[q].se >= 0) sig0 |= 1 << E.slots[q].se; }
+      int sigq = sig0; std::vector<int> fq = f0;
+      if (q >= 0) { fq.push_back(nb + ne + E.slots[q].e); if (E.slots[q].se >= 0) sigq |= 1 << E.slots[q].se; }
       for (unsigned eb = 0; eb < (1u << en.size()); ++eb) {
-        HRecord r; r.ncomp = ncomp; r.k = (int)fr.size(); int sig = sig0; std::vector<int> f = f0; size_t Tbase = 0;
+        HRecord r; r.flags = (ncomp == 2) ? FG_REC_TWO : 0; r.k = (int)fr.size(); int sig = sigq; std::vector<int> f = fq; size_t Tbase = 0;
         for (size_t t = 0; t < en.size(); ++t) if ((eb >> t) & 1) { const Slot& sl = E.slots[gaps[en[t]]]; f.push_back(nb + sl.e); if (sl.se >= 0) sig |= 1 << sl.se; Tbase |= (size_t)1 << en[t]; }
+        if ((int)f.size() > FG_MAXF) { over = true; continue; }
         r.nf = (int)f.size(); r.dst = sig * FG_NDEG + npairs;
         std::memset(r.fidx, 0, sizeof(r.fidx)); std::memset(r.vidx, 0, sizeof(r.vidx));
         for (int t = 0; t < r.nf; ++t) r.fidx[t] = (uint8_t)f[t];
@@ -318,17 +349,20 @@ static void build_records(const HGeom& E, int type, HNum& N) {
           size_t T = Tbase; for (int t = 0; t < r.k; ++t) if ((sub >> t) & 1) T |= (size_t)1 << fr[t];
           double v = tab[c][T]; r.coef[((size_t)c << r.k) + sub] = v; if (v != 0.0) nz = true;
         }
-        if (nz) per[mi].push_back(std::move(r));
+        if (nz) { finish_record(r); per[mi].push_back(std::move(r)); }
       }
     }
   }
+  if (over) limit_hit = true;
   for (auto& v : per) for (auto& r : v) N.recs.push_back(std::move(r));
-  std::stable_sort(N.recs.begin(), N.recs.end(), [](const HRecord& a, const HRecord& b) { if (a.dst != b.dst) return a.dst < b.dst; return a.k > b.k; });
+  std::stable_sort(N.recs.begin(), N.recs.end(), [](const HRecord& a, const HRecord& b) { return a.dst < b.dst; });
   for (auto& r : N.recs) {
     long nc = (long)r.coef.size(), nz = 0; for (double v : r.coef) if (v != 0.0) ++nz;
+    int nco = (r.flags & FG_REC_TWO) ? 2 : 1;
     N.n_coefs += nc; N.n_nonzero += nz;
-    N.exec_flops += std::max(0, r.nf - 1) + r.ncomp * (2.0 * ((1 << r.k) - 1) + 2.0);
-    N.algo_flops += std::max(0, r.nf - 1) + 2.0 * nz;
+    N.exec_flops += nco * (2.0 * ((1 << r.k) - 1) + 4.0);
+    if (r.flags & FG_REC_QEXT) N.exec_flops += r.k * (2.0 * ((1 << r.k) / 2 - 1) + 2.0);
+    N.algo_flops += 2.0 * nz;
   }
 }
 
@@ -491,7 +525,8 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     for (int i = 0; i < nd_n; ++i) P.nums[P.nodes[i].num].nodes.push_back(i);
   }
   // Dirac tables -> records
-  for (auto& N : P.nums) build_records(P.geoms[N.geom], P.subs[P.geoms[N.geom].sub].type, N);
+  { bool limit_hit = false; for (auto& N : P.nums) build_records(P.geoms[N.geom], P.subs[P.geoms[N.geom].sub].type, N, limit_hit);
+    if (limit_hit) { msg = "a numerator record needs more than FG_MAXF product factors"; return FG_E_LIMIT; } }
   // flatten
   P.d_geoms.resize(P.geoms.size());
   for (size_t i = 0; i < P.geoms.size(); ++i) {
@@ -508,17 +543,20 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     d.geom = N.geom; d.op = N.op; d.ncomp = N.ncomp; d.nse = N.nse;
     d.node_begin = N.nodes.empty() ? 0 : N.nodes.front(); d.node_count = (int)N.nodes.size();
     d.chunk_begin = (int)(P.d_chunks.size() / FG_CHUNK_BYTES);
-    // pack records into chunks
-    size_t cur = 0; bool open = false; int nrec = 0; size_t base = 0;
-    auto close_chunk = [&]() { if (open) { FgChunkHdr h = {nrec, 0}; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
+    // pack records into chunks; keep = leading product factors shared with the previous record of the chunk
+    size_t cur = 0; bool open = false; int nrec = 0; size_t base = 0; const HRecord* prev = nullptr;
+    auto close_chunk = [&]() { if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.nrec = nrec; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
     for (auto& r : N.recs) {
       size_t need = sizeof(FgRecHdr) + r.coef.size() * sizeof(double);
-      if (!open || cur + need > FG_CHUNK_BYTES) { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); nrec = 0; open = true; }
-      FgRecHdr h; std::memset(&h, 0, sizeof(h)); h.nf = (uint8_t)r.nf; h.k = (uint8_t)r.k; h.dst = (uint8_t)r.dst; h.ncomp = (uint8_t)r.ncomp;
-      std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx));
+      if (!open || cur + need > FG_CHUNK_BYTES) { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); nrec = 0; open = true; prev = nullptr; }
+      int keep = 0;
+      if (prev) while (keep < r.nf && keep < prev->nf && keep < 15 && r.fidx[keep] == prev->fidx[keep]) ++keep;
+      FgRecHdr h; std::memset(&h, 0, sizeof(h)); h.nf = (uint8_t)r.nf; h.k = (uint8_t)r.k; h.dst = (uint8_t)r.dst; h.flags = (uint8_t)(r.flags | (keep << 4));
+      std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs[0] = r.cabs[0]; h.cabs[1] = r.cabs[1];
       std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h);
       std::memcpy(&P.d_chunks[base + cur], r.coef.data(), r.coef.size() * sizeof(double)); cur += r.coef.size() * sizeof(double);
-      ++nrec;
+      ++nrec; prev = &r;
+      N.exec_flops += std::max(0, r.nf - std::max(keep, 1)); N.algo_flops += std::max(0, r.nf - std::max(keep, 1));
     }
     close_chunk();
     d.chunk_count = (int)(P.d_chunks.size() / FG_CHUNK_BYTES) - d.chunk_begin;

@@ -32,9 +32,9 @@ struct HGeom {
 };
 
 struct HRecord {
-  int nf, k, dst, ncomp;
+  int nf, k, dst, flags; float cabs[2];
   uint8_t fidx[FG_MAXF], vidx[FG_KMAX];
-  std::vector<double> coef;                     // ncomp * 2^k
+  std::vector<double> coef;                     // tables (see FgRecHdr), padded to an even count
 };
 
 struct HNum {

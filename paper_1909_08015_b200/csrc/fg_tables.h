@@ -50,16 +50,23 @@ struct FgTermDev {
   int32_t geom[FG_MAXMEM];    // geometries of the members (for prod U_S^2 and sum W_S)
 };
 
-// Record header inside a chunk (24 bytes, followed by ncomp * 2^k doubles):
-//   value = prod_{f<nf} V[fidx[f]] * sum_T coef[T] prod_{j in T} V[vidx[j]]   added to accumulator dst
-struct alignas(8) FgRecHdr {
-  uint8_t nf, k, dst, ncomp;
+// Record header inside a chunk (32 bytes, 16-byte aligned, followed by the coefficient tables as doubles):
+//   plain:        value = prod_{f<nf} V[fidx[f]] * sum_T coef[T] prod_{j in T} V[vidx[j]]        (2^k coefs per component)
+//   q-extension:  ... + prod * sum_{j<k} V[vidx[j] + ne] * sum_{T subset vars\j} coefq_j[T] prod_{i in T} V[vidx[i]]
+//                 (k further tables of 2^(k-1) coefs: the slot that carries gamma^nu with weight A^q_j)
+// added to accumulator dst.  keep = number of leading product factors shared with the previous record of the chunk.
+// cabs[c] = sum of |coef| of component c: with |A_j|, |A^q_j| <= 1 it bounds the sum of |terms| of the record.
+#define FG_REC_TWO 1
+#define FG_REC_QEXT 2
+struct alignas(16) FgRecHdr {
+  uint8_t nf, k, dst, flags;      // flags: bit0 two components, bit1 q-extension, bits 4..7 keep
   uint8_t fidx[FG_MAXF];
   uint8_t vidx[FG_KMAX];
   uint8_t pad[4];
+  float cabs[2];
 };
-// Chunk header (8 bytes): number of records in the chunk.
-struct FgChunkHdr { int32_t nrec; int32_t pad; };
+// Chunk header (16 bytes): number of records in the chunk.
+struct alignas(16) FgChunkHdr { int32_t nrec; int32_t pad[3]; };
 
 // Everything the kernels need, passed by value.
 struct FgPlanDev {

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfg.so")
 
 EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
-           "fg_plan_info", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
+           "fg_plan_info", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
            "fg_dfma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
 
@@ -68,6 +68,9 @@ def lib():
         L.fg_plan_opts_default.argtypes = [C.POINTER(fg_plan_opts)]
         L.fg_plan_create.argtypes = [vp, C.POINTER(fg_plan_opts), C.c_int32, C.POINTER(vp)]
         L.fg_plan_destroy.argtypes = [vp]
+        L.fg_plan_set_tol.argtypes = [vp, C.c_double, C.c_double]
+        L.fg_plan_profile.argtypes = [vp, C.c_int32]
+        L.fg_plan_timing.argtypes = [vp, vp, vp]
         L.fg_plan_info.argtypes = [vp, C.POINTER(fg_plan_stats)]
         L.fg_plan_structure.argtypes = [vp, vp, vp, C.c_int32]
         L.fg_plan_tables.argtypes = [vp, vp, vp]
@@ -155,6 +158,17 @@ class Plan:
     def info(self):
         s = fg_plan_stats(); _check(lib().fg_plan_info(self.h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in fg_plan_stats._fields_}
+
+    def set_tol(self, rel_tol, abs_tol):
+        _check(lib().fg_plan_set_tol(self.h, float(rel_tol), float(abs_tol)))
+
+    def profile(self, enable=True):
+        _check(lib().fg_plan_profile(self.h, int(bool(enable))))
+
+    def timing(self):
+        ms = np.zeros(3); n = np.zeros(1, dtype=np.int64)
+        _check(lib().fg_plan_timing(self.h, _p(ms), _p(n)))
+        return dict(ms_double=ms[0], ms_dd=ms[1], ms_reduce=ms[2], launches=int(n[0]))
 
     def structure(self):
         ns = self.stats["n_subgraphs"]
