@@ -115,14 +115,16 @@ FG_HD void draw_sample(const FgPlanDev& P, const double* __restrict__ Z1, const 
 // B = L D L^T (no square roots).  This step is always carried out in double-double, whatever the precision of the
 // numerator pass: it is a few per cent of the work at 5 loops and it removes the cancellations of the pivots,
 // of 1 - sum and of the beta dot products from the double-precision pass.
-// V receives beta (upper triangle, row-major), then A, then A^q, element idx at V[idx * vs]; amax = max(1,|A|,|A^q|).
+// V receives beta (upper triangle, row-major), then A, then A^q, element idx at V[idx * vs]; amax = max(1,|A|,|A^q|);
+// amp = conditioning of this step: product of the pivot ratios B_aa/d_a times the worst ratio sum|terms|/|value| of the
+// final sums of A, A^q and beta (relative error of the entries of V is about amp * 2^-104).
 // ------------------------------------------------------------------------------------------------
 template <class T> FG_HD T from_dd(dd a);
 template <> FG_HD double from_dd<double>(dd a) { return a.hi + a.lo; }
 template <> FG_HD dd from_dd<dd>(dd a) { return a; }
 
 template <class T>
-FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T& W, double& amax) {
+FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T& W, double& amax, double& amp) {
   const int l = E.l, ne = E.ne;
   dd B[FG_MAXL][FG_MAXL], C[FG_MAXL], Cq[FG_MAXL], invd[FG_MAXL];
   for (int a = 0; a < l; ++a) { C[a] = dd(0.0); Cq[a] = dd(0.0); for (int b = 0; b < l; ++b) B[a][b] = dd(0.0); }
@@ -136,11 +138,11 @@ FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T
     }
   }
   for (int a = 0; a < l; ++a) B[a][a] = dd_add_d(B[a][a], zl[E.line_ph[a]]);
-  dd u(1.0);
+  dd u(1.0); double growth = 1.0;
   for (int a = 0; a < l; ++a) {
-    dd d = B[a][a];
+    dd d = B[a][a]; const double baa = d.hi;
     for (int b = 0; b < a; ++b) d = d - B[a][b] * B[a][b] * B[b][b];     // B[b][b] holds d_b, B[a][b] holds L_ab
-    invd[a] = dd(1.0) / d; u = u * d;
+    invd[a] = dd(1.0) / d; u = u * d; growth *= fmax(1.0, baa / d.hi);
     for (int c = a + 1; c < l; ++c) {
       dd t = B[c][a];
       for (int b = 0; b < a; ++b) t = t - B[c][b] * B[a][b] * B[b][b];
@@ -153,54 +155,58 @@ FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T
   dd w(0.0); for (int a = 0; a < l; ++a) { w = w + C[a] * C[a] * invd[a]; C[a] = C[a] * invd[a]; Cq[a] = Cq[a] * invd[a]; }
   W = from_dd<T>(w);
   dd Y[FG_MAXNE][FG_MAXL];
-  const int nb = ne * (ne + 1) / 2; double am = 1.0;
+  const int nb = ne * (ne + 1) / 2; double am = 1.0, cond = 1.0;
   for (int q = 0; q < ne; ++q) {
     const unsigned m = E.eta[q];
     for (int a = 0; a < l; ++a) { dd y = ((m >> a) & 1u) ? dd(1.0) : dd(0.0); for (int b = 0; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
-    dd sa(0.0), sq(0.0);
-    for (int a = 0; a < l; ++a) { sa = sa + Y[q][a] * C[a]; sq = sq + Y[q][a] * Cq[a]; }
+    dd sa(0.0), sq(0.0); double ta = 1.0, tq = 0.5;
+    for (int a = 0; a < l; ++a) { const dd t1 = Y[q][a] * C[a], t2 = Y[q][a] * Cq[a]; sa = sa + t1; sq = sq + t2; ta += fabs(t1.hi); tq += fabs(t2.hi); }
     const dd A = dd(1.0) - sa, Aq = dd(0.5 * (double)E.xiq[q]) - sq;
     V[(nb + q) * vs] = from_dd<T>(A); V[(nb + ne + q) * vs] = from_dd<T>(Aq);
     am = fmax(am, fmax(fabs(A.hi), fabs(Aq.hi)));
+    if (A.hi != 0.0) cond = fmax(cond, ta / fabs(A.hi));
+    if (E.xiq[q] != 0 && Aq.hi != 0.0) cond = fmax(cond, tq / fabs(Aq.hi));
   }
   amax = am;
   int idx = 0;
   for (int i = 0; i < ne; ++i) {
     dd yd[FG_MAXL]; for (int a = 0; a < l; ++a) yd[a] = Y[i][a] * invd[a];
     for (int j = i; j < ne; ++j) {
-      dd b(0.0); for (int a = 0; a < l; ++a) b = b + yd[a] * Y[j][a];
+      dd b(0.0); double tb = 0.0; for (int a = 0; a < l; ++a) { const dd t1 = yd[a] * Y[j][a]; b = b + t1; tb += fabs(t1.hi); }
+      if (b.hi != 0.0) cond = fmax(cond, tb / fabs(b.hi));
       V[idx * vs] = from_dd<T>(b); ++idx;
     }
   }
+  amp = growth * cond;
 }
 
 // ------------------------------------------------------------------------------------------------
 // a6  multilinear polynomial in K variables with a dense 2^K coefficient table (uniform across the block)
 // ------------------------------------------------------------------------------------------------
-template <class T, int S, int K> struct Horner {
+template <class T, int S, int K, bool AC = false> struct Horner {   // AC: use |coef| (for the sum of |terms|)
   static FG_HD void run(const double* __restrict__ c, const T (*a)[S], T* out) {
     T lo[S], hi[S];
-    Horner<T, S, K - 1>::run(c, a, lo); Horner<T, S, K - 1>::run(c + (1 << (K - 1)), a, hi);
+    Horner<T, S, K - 1, AC>::run(c, a, lo); Horner<T, S, K - 1, AC>::run(c + (1 << (K - 1)), a, hi);
 #pragma unroll
     for (int s = 0; s < S; ++s) out[s] = t_fma(a[K - 1][s], hi[s], lo[s]);
   }
 };
-template <class T, int S> struct Horner<T, S, 0> {
+template <class T, int S, bool AC> struct Horner<T, S, 0, AC> {
   static FG_HD void run(const double* __restrict__ c, const T (*)[S], T* out) {
-    const double c0 = c[0];
+    const double c0 = AC ? fabs(c[0]) : c[0];
 #pragma unroll
     for (int s = 0; s < S; ++s) out[s] = T(c0);
   }
 };
-template <int S> struct Horner<double, S, 1> {   // leaf FMA takes both coefficients straight from the table
+template <int S, bool AC> struct Horner<double, S, 1, AC> {   // leaf FMA takes both coefficients straight from the table
   static FG_HD void run(const double* __restrict__ c, const double (*a)[S], double* out) {
-    const double c0 = c[0], c1 = c[1];
+    const double c0 = AC ? fabs(c[0]) : c[0], c1 = AC ? fabs(c[1]) : c[1];
 #pragma unroll
     for (int s = 0; s < S; ++s) out[s] = fma(a[0][s], c1, c0);
   }
 };
 // q-extension: q += sum_j aq[j] * (multilinear in the K-1 variables other than j)
-template <class T, int S, int K> struct QExt {
+template <class T, int S, int K, bool AC = false> struct QExt {
   static FG_HD void run(const double* __restrict__ cq, const T (*a)[S], const T (*aq)[S], T* q) {
 #pragma unroll
     for (int j = 0; j < K; ++j) {
@@ -210,13 +216,13 @@ template <class T, int S, int K> struct QExt {
 #pragma unroll
         for (int s = 0; s < S; ++s) b[i][s] = a[i < j ? i : i + 1][s];
       }
-      Horner<T, S, K - 1>::run(cq + j * (1 << (K - 1)), b, sub);
+      Horner<T, S, K - 1, AC>::run(cq + j * (1 << (K - 1)), b, sub);
 #pragma unroll
       for (int s = 0; s < S; ++s) q[s] = t_fma(aq[j][s], sub[s], q[s]);
     }
   }
 };
-template <class T, int S> struct QExt<T, S, 0> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
+template <class T, int S, bool AC> struct QExt<T, S, 0, AC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
 // Running state of one program: prefix products of the factor list, accumulators of the current destination.
 template <class T, int S> struct RecState { T p[FG_MAXF][S]; T acc[2][S]; double aab[2][S]; int cur; };
@@ -227,7 +233,8 @@ FG_HD int rec_ncoef(int k, int flags) {
 }
 
 // All records of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
-template <class T, int S, bool ABS, class Flush>
+// ABS: 0 no |.| tracking, 1 bound by cabs (needs |A|,|A^q| <= 1), 2 exact sum of |coef| prod |A| in double
+template <class T, int S, int ABS, class Flush>
 FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st, Flush&& flush) {
 #if defined(__CUDA_ARCH__)
   __builtin_assume(__isShared(chunk)); __builtin_assume(__isShared(Vt));   // LDS instead of generic loads
@@ -271,7 +278,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
         for (int s = 0; s < S; ++s) aq[j][s] = pq[s];
       }
     }
-    T q[2][S];
+    T q[2][S]; double qa[2][S];
     switch (k) {
 #define FG_CASE(K) case K: Horner<T, S, K>::run(coef, a, q[0]); \
                            if (flags & FG_REC_TWO) Horner<T, S, K>::run(coef + (1 << K), a, q[1]); \
@@ -280,13 +287,31 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
 #undef FG_CASE
       default: break;
     }
+    if (ABS == 2) {
+      double ab[FG_KMAX][S], abq[FG_KMAX][S];
+#pragma unroll
+      for (int j = 0; j < FG_KMAX; ++j) if (j < k) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) { ab[j][s] = t_abs_d(a[j][s]); abq[j][s] = (flags & FG_REC_QEXT) ? t_abs_d(aq[j][s]) : 0.0; }
+      }
+      switch (k) {
+#define FG_CASE(K) case K: Horner<double, S, K, true>::run(coef, ab, qa[0]); \
+                           if (flags & FG_REC_TWO) Horner<double, S, K, true>::run(coef + (1 << K), ab, qa[1]); \
+                           else if (flags & FG_REC_QEXT) QExt<double, S, K, true>::run(coef + (1 << K), ab, abq, qa[0]); break;
+        FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4) FG_CASE(5) FG_CASE(6)
+#undef FG_CASE
+        default: break;
+      }
+    }
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       st.acc[0][s] = t_fma(prod[s], q[0][s], st.acc[0][s]);
-      if (ABS) st.aab[0][s] = fma(t_abs_d(prod[s]), (double)h.cabs[0], st.aab[0][s]);
+      if (ABS == 1) st.aab[0][s] = fma(t_abs_d(prod[s]), (double)h.cabs[0], st.aab[0][s]);
+      if (ABS == 2) st.aab[0][s] = fma(t_abs_d(prod[s]), qa[0][s], st.aab[0][s]);
       if (flags & FG_REC_TWO) {
         st.acc[1][s] = t_fma(prod[s], q[1][s], st.acc[1][s]);
-        if (ABS) st.aab[1][s] = fma(t_abs_d(prod[s]), (double)h.cabs[1], st.aab[1][s]);
+        if (ABS == 1) st.aab[1][s] = fma(t_abs_d(prod[s]), (double)h.cabs[1], st.aab[1][s]);
+        if (ABS == 2) st.aab[1][s] = fma(t_abs_d(prod[s]), qa[1][s], st.aab[1][s]);
       }
     }
     off += (int)sizeof(FgRecHdr) + rec_ncoef(k, flags) * (int)sizeof(double);

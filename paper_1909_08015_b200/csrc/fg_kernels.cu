@@ -51,7 +51,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2]; };
 
 // a6: run the record stream of one program for the S samples of this thread
-template <class T, int S, bool ABS>
+template <class T, int S, int ABS>
 __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const T* Vt, int vs, int ne, T* Sc, int ss) {
   const int nslots = (1 << N.nse) * FG_NDEG * N.ncomp;
   for (int i = 0; i < nslots; ++i) {
@@ -84,8 +84,8 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
 }
 
 // a5-a7 for the S points of this thread
-template <class T, int S, bool ABS>
-__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* amp) {
+template <class T, int S, int ABS>
+__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* amx, double* amp) {
   const ScratchMap sm(P);
   double zl[S][FG_MAXLINES];
 #pragma unroll
@@ -94,16 +94,17 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
       const int l0 = P.var_line0[v], l1 = P.var_line1[v];
       if (l1 == 255) zl[s][l0] = z[s][v]; else { zl[s][l0] = 0.5 * z[s][v]; zl[s][l1] = 0.5 * z[s][v]; }
     }
-    amp[s] = 1.0;
+    amx[s] = 1.0; amp[s] = 1.0;
   }
   for (int g = 0; g < P.ngeom; ++g) {
     const FgGeomDev E = P.geoms[g];
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      T U, W; double am;
-      geom_eval<T>(E, zl[s], Vt + s, vs, U, W, am);
+      T U, W; double am, cp;
+      geom_eval<T>(E, zl[s], Vt + s, vs, U, W, am, cp);
       Sc[(2 * g) * ss + s] = U; Sc[(2 * g + 1) * ss + s] = W;
-      if (am > amp[s] || !(am == am)) amp[s] = am;
+      if (am > amx[s] || !(am == am)) amx[s] = am;
+      if (cp > amp[s] || !(cp == cp)) amp[s] = cp;
     }
     for (int ni = P.geom_num_begin[g]; ni < P.geom_num_begin[g + 1]; ++ni) {
       const FgNumDev N = P.nums[ni];
@@ -116,7 +117,7 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
   }
 #pragma unroll
   for (int s = 0; s < S; ++s) {
-    T Iv, Ia; assemble<T, ABS>(P, sm, Sc + s, ss, Iv, Ia);
+    T Iv, Ia; assemble<T, ABS != 0>(P, sm, Sc + s, ss, Iv, Ia);
     if (P.merge_var >= 0) { Iv = Iv * T(z[s][P.merge_var]); Ia = Ia * T(z[s][P.merge_var]); }
     I[s] = Iv; Iabs[s] = to_double(Ia);
   }
@@ -156,31 +157,32 @@ __global__ void __launch_bounds__(NT) fg_eval_kernel(const FgPlanDev P, const Ru
       }
       if (!valid[s] || bad[s]) for (int v = 0; v < M; ++v) z[s][v] = 1.0 / M;
     }
-    T I[S]; double Iabs[S], growth[S];
-    eval_points<T, S, !is_dd<T>::value>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth);
+    T I[S]; double Iabs[S], growth[S], amp[S];
+    eval_points<T, S, is_dd<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp);
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       if (!valid[s]) continue;
       const double Id = to_double(I[s]);
       double af = growth[s] * growth[s]; af = af * af * af;      // |A|, |A^q| <= 1 is assumed by cabs; amax^6 otherwise
-      const double err = is_dd<T>::value ? 0.0 : P.err_eps * af * Iabs[s];
+      // running error estimate: K * u * sum|terms| with u = 2^-53 (double pass) or 2^-104 (double-double pass)
+      // plus the conditioning of the (always double-double) geometry step, amp * 2^-104 / 32
+      const double err = ((is_dd<T>::value ? P.err_eps * 0x1p-51 : P.err_eps * af) + amp[s] * 0x1p-109) * Iabs[s];
       uint8_t fl = 0; double y = 0.0;
-      if (ex[s] > 1023 || ex[s] < -1021) ++nbig;
+      if (!A.idlist && (ex[s] > 1023 || ex[s] < -1021)) ++nbig;
       if (bad[s]) { ++nrej; fl = 2; }
       else {
         const double tol = fmax(P.rel_tol * fabs(Id), ldexp(P.abs_tol * mant[s], ex[s]));
-        const bool flagged = A.do_flag && !(err <= tol);
-        if (flagged) {
+        const bool over = !(err <= tol);
+        if (!is_dd<T>::value && A.do_flag && over) {
           fl = 1; ++nflag;
           if (A.flag_list) { const unsigned long long pos = atomicAdd(A.flag_count, 1ull); A.flag_list[pos] = (uint32_t)oid[s]; }
+        } else if (is_dd<T>::value && over) {
+          fl = 4; ++nrej;     // not resolved by the last rung: contributes 0 and is counted
         } else {
           const T yq = I[s] / T(mant[s]);
           y = ldexp(to_double(yq), -ex[s]);
           if (!isfinite(y)) { ++nrej; fl |= 2; y = 0.0; }
-          else {
-            const dd yd = is_dd<T>::value ? dd(ldexp(to_double(yq), -ex[s])) : dd(y);
-            sy = dd_add_d(sy, yd.hi); const dd y2 = two_prod(yd.hi, yd.hi); sy2 = sy2 + y2;
-          }
+          else { sy = dd_add_d(sy, y); sy2 = sy2 + two_prod(y, y); }
         }
       }
       if (A.outI) A.outI[oid[s]] = Id;
@@ -355,8 +357,11 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   p->smem_d = 2 * FG_CHUNK_BYTES + 128 + (size_t)vmax * NT_D * S_D * sizeof(double);
   p->smem_q = 2 * FG_CHUNK_BYTES + 128 + (size_t)vmax * NT_Q * S_Q * sizeof(dd);
   p->grid_d = p->sms; p->grid_q = p->sms;
-  auto setattr = [&](const void* f, size_t sm) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); };
-  e = setattr((const void*)fg_eval_kernel<double, S_D, NT_D>, p->smem_d); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>, p->smem_q);
+  // the attribute is per function, not per plan: always raise it to the device limit
+  int smem_max = 0; cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+  if ((size_t)smem_max < p->smem_d || (size_t)smem_max < p->smem_q) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
+  auto setattr = [&](const void* f) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max); };
+  e = setattr((const void*)fg_eval_kernel<double, S_D, NT_D>); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>);
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("shared memory: ") + cudaGetErrorString(e)); }
   size_t sc = (size_t)H.scratch_slots * std::max((size_t)NT_D * S_D * sizeof(double) * p->grid_d, (size_t)NT_Q * S_Q * sizeof(dd) * p->grid_q);
   auto dmalloc = [&](void** d, size_t bytes) { cudaError_t e2 = cudaMalloc(d, bytes); if (e2 == cudaSuccess) { p->allocs.push_back(*d); cudaMemset(*d, 0, bytes); } return e2; };
