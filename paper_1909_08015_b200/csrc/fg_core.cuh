@@ -224,59 +224,78 @@ template <class T, int S, int K, bool AC = false> struct QExt {
 };
 template <class T, int S, bool AC> struct QExt<T, S, 0, AC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
-// Running state of one program: prefix products of the factor list, accumulators of the current destination.
-template <class T, int S> struct RecState { T p[FG_MAXF][S]; T acc[2][S]; double aab[2][S]; int cur; };
+// Running state of one program: accumulators of the current destination.
+template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; int cur; };
 
-FG_HD int rec_ncoef(int k, int flags) {
-  const int n = (flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k;
-  return (n + 1) & ~1;
+FG_HD constexpr int rec_ncoef(int k, int flags) {
+  return (((flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k) + 1) & ~1;
 }
 
-// All records of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
-// ABS: 0 no |.| tracking, 1 bound by cabs (needs |A|,|A^q| <= 1), 2 exact sum of |coef| prod |A| in double
-template <class T, int S, int ABS, class Flush>
-FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st, Flush&& flush) {
-#if defined(__CUDA_ARCH__)
-  __builtin_assume(__isShared(chunk)); __builtin_assume(__isShared(Vt));   // LDS instead of generic loads
-#endif
-  const int nrec = ((const FgChunkHdr*)chunk)->nrec;
-  int off = (int)sizeof(FgChunkHdr);
-  for (int r = 0; r < nrec; ++r) {
-    const FgRecHdr h = *(const FgRecHdr*)(chunk + off);
-    const double* __restrict__ coef = (const double*)(chunk + off + sizeof(FgRecHdr));
-    const int nf = h.nf, k = h.k, flags = h.flags, keep = flags >> 4;
-    if ((int)h.dst != st.cur) {
-      if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
-      st.cur = h.dst;
+// One group of compact records, class known at compile time: the inner loop has no data-dependent control flow
+// except the (block-uniform) prefix depth `keep`.  ABS as in run_chunk.
+template <class T, int S, int ABS, int NF, int K, bool QX>
+FG_HD void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* acc, double* aab) {
+  constexpr int FL = QX ? FG_REC_QEXT : 0;
+  constexpr int STRIDE = (int)sizeof(FgRecC) + rec_ncoef(K, FL) * (int)sizeof(double);
+  T pf[NF > 0 ? NF : 1][S];
+  for (int r = 0; r < nrec; ++r, p += STRIDE) {
+    const FgRecC h = *(const FgRecC*)p;
+    const double* __restrict__ coef = (const double*)(p + sizeof(FgRecC));
+    const int keep = h.keep;
 #pragma unroll
-      for (int s = 0; s < S; ++s) { st.acc[0][s] = T(0.0); st.acc[1][s] = T(0.0); st.aab[0][s] = 0.0; st.aab[1][s] = 0.0; }
+    for (int f = 0; f < NF; ++f) if (f >= keep) {
+      const T* pv = Vt + (int)h.fidx[f] * vs;
+#pragma unroll
+      for (int s = 0; s < S; ++s) pf[f][s] = (f == 0) ? pv[s] : pf[f > 0 ? f - 1 : 0][s] * pv[s];
     }
-    T prod[S];
+    T a[K > 0 ? K : 1][S], aq[K > 0 ? K : 1][S];
 #pragma unroll
-    for (int s = 0; s < S; ++s) prod[s] = T(1.0);
-#pragma unroll
-    for (int f = 0; f < FG_MAXF; ++f) if (f < nf) {
-      if (f >= keep) {
-        const T* pv = Vt + (int)h.fidx[f] * vs;
-#pragma unroll
-        for (int s = 0; s < S; ++s) st.p[f][s] = (f == 0) ? pv[s] : st.p[f > 0 ? f - 1 : 0][s] * pv[s];
-      }
-      if (f == nf - 1) {
-#pragma unroll
-        for (int s = 0; s < S; ++s) prod[s] = st.p[f][s];
-      }
-    }
-    T a[FG_KMAX][S], aq[FG_KMAX][S];
-#pragma unroll
-    for (int j = 0; j < FG_KMAX; ++j) if (j < k) {
+    for (int j = 0; j < K; ++j) {
       const T* pv = Vt + (int)h.vidx[j] * vs;
 #pragma unroll
       for (int s = 0; s < S; ++s) a[j][s] = pv[s];
-      if (flags & FG_REC_QEXT) {
+      if (QX) {
         const T* pq = pv + ne * vs;
 #pragma unroll
         for (int s = 0; s < S; ++s) aq[j][s] = pq[s];
       }
+    }
+    T q[S];
+    Horner<T, S, K>::run(coef, a, q);
+    if (QX) QExt<T, S, K>::run(coef + (1 << K), a, aq, q);
+    const double cab = (double)h.cabs;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (NF > 0) { acc[s] = t_fma(pf[NF > 0 ? NF - 1 : 0][s], q[s], acc[s]); if (ABS) aab[s] = fma(t_abs_d(pf[NF > 0 ? NF - 1 : 0][s]), cab, aab[s]); }
+      else { acc[s] = acc[s] + q[s]; if (ABS) aab[s] += cab; }
+    }
+  }
+}
+
+// One group of any class, everything dynamic (wide records, two-component records, the double-double pass).
+template <class T, int S, int ABS>
+FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, int k, int flags, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st) {
+  const bool wide = (flags & FG_REC_WIDE) != 0;
+  const int stride = (wide ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double);
+  for (int r = 0; r < nrec; ++r, p += stride) {
+    const uint8_t* fidx = wide ? ((const FgRecW*)p)->fidx : ((const FgRecC*)p)->fidx;
+    const uint8_t* vidx = wide ? ((const FgRecW*)p)->vidx : ((const FgRecC*)p)->vidx;
+    const double cab = wide ? (double)((const FgRecW*)p)->cabs : (double)((const FgRecC*)p)->cabs;
+    const double* __restrict__ coef = (const double*)(p + (wide ? sizeof(FgRecW) : sizeof(FgRecC)));
+    T prod[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) prod[s] = T(1.0);
+    for (int f = 0; f < nf; ++f) {
+      const T* pv = Vt + (int)fidx[f] * vs;
+#pragma unroll
+      for (int s = 0; s < S; ++s) prod[s] = prod[s] * pv[s];
+    }
+    T a[FG_KMAX][S], aq[FG_KMAX][S];
+#pragma unroll
+    for (int j = 0; j < FG_KMAX; ++j) if (j < k) {
+      const T* pv = Vt + (int)vidx[j] * vs;
+#pragma unroll
+      for (int s = 0; s < S; ++s) { a[j][s] = pv[s]; aq[j][s] = (flags & FG_REC_QEXT) ? pv[ne * vs + s] : T(0.0); }
     }
     T q[2][S]; double qa[2][S];
     switch (k) {
@@ -292,7 +311,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
 #pragma unroll
       for (int j = 0; j < FG_KMAX; ++j) if (j < k) {
 #pragma unroll
-        for (int s = 0; s < S; ++s) { ab[j][s] = t_abs_d(a[j][s]); abq[j][s] = (flags & FG_REC_QEXT) ? t_abs_d(aq[j][s]) : 0.0; }
+        for (int s = 0; s < S; ++s) { ab[j][s] = t_abs_d(a[j][s]); abq[j][s] = t_abs_d(aq[j][s]); }
       }
       switch (k) {
 #define FG_CASE(K) case K: Horner<double, S, K, true>::run(coef, ab, qa[0]); \
@@ -306,15 +325,56 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       st.acc[0][s] = t_fma(prod[s], q[0][s], st.acc[0][s]);
-      if (ABS == 1) st.aab[0][s] = fma(t_abs_d(prod[s]), (double)h.cabs[0], st.aab[0][s]);
+      if (ABS == 1) st.aab[0][s] = fma(t_abs_d(prod[s]), cab, st.aab[0][s]);
       if (ABS == 2) st.aab[0][s] = fma(t_abs_d(prod[s]), qa[0][s], st.aab[0][s]);
       if (flags & FG_REC_TWO) {
         st.acc[1][s] = t_fma(prod[s], q[1][s], st.acc[1][s]);
-        if (ABS == 1) st.aab[1][s] = fma(t_abs_d(prod[s]), (double)h.cabs[1], st.aab[1][s]);
+        if (ABS == 1) st.aab[1][s] = fma(t_abs_d(prod[s]), cab, st.aab[1][s]);
         if (ABS == 2) st.aab[1][s] = fma(t_abs_d(prod[s]), qa[1][s], st.aab[1][s]);
       }
     }
-    off += (int)sizeof(FgRecHdr) + rec_ncoef(k, flags) * (int)sizeof(double);
+  }
+}
+
+// All groups of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
+// ABS: 0 no |.| tracking, 1 bound by cabs (needs |A|,|A^q| <= 1), 2 exact sum of |coef| prod |A| in double
+template <class T, int S, int ABS, class Flush>
+FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st, Flush&& flush) {
+#if defined(__CUDA_ARCH__)
+  __builtin_assume(__isShared(chunk)); __builtin_assume(__isShared(Vt));   // LDS instead of generic loads
+#endif
+  const int ngroups = ((const FgChunkHdr*)chunk)->ngroups;
+  const unsigned char* p = chunk + sizeof(FgChunkHdr);
+  for (int g = 0; g < ngroups; ++g) {
+    const FgGroupHdr gh = *(const FgGroupHdr*)p; p += sizeof(FgGroupHdr);
+    const int nrec = gh.nrec, nf = gh.nf, k = gh.k, flags = gh.flags;
+    if ((int)gh.dst != st.cur) {
+      if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
+      st.cur = gh.dst;
+#pragma unroll
+      for (int s = 0; s < S; ++s) { st.acc[0][s] = T(0.0); st.acc[1][s] = T(0.0); st.aab[0][s] = 0.0; st.aab[1][s] = 0.0; }
+    }
+    bool done = false;
+    if constexpr (!is_dd<T>::value && ABS != 2) {
+      if (!(flags & (FG_REC_WIDE | FG_REC_TWO))) {
+        done = true;
+        const bool qx = (flags & FG_REC_QEXT) != 0;
+        switch (nf * 8 + k) {
+#define FG_CLS(NF, K) case NF * 8 + K: if (qx) run_group_static<T, S, ABS, NF, K, true>(p, nrec, Vt, vs, ne, st.acc[0], st.aab[0]); \
+                                        else run_group_static<T, S, ABS, NF, K, false>(p, nrec, Vt, vs, ne, st.acc[0], st.aab[0]); break;
+          FG_CLS(0, 0) FG_CLS(0, 1) FG_CLS(0, 2) FG_CLS(0, 3) FG_CLS(0, 4) FG_CLS(0, 5) FG_CLS(0, 6)
+          FG_CLS(1, 0) FG_CLS(1, 1) FG_CLS(1, 2) FG_CLS(1, 3) FG_CLS(1, 4) FG_CLS(1, 5) FG_CLS(1, 6)
+          FG_CLS(2, 0) FG_CLS(2, 1) FG_CLS(2, 2) FG_CLS(2, 3) FG_CLS(2, 4) FG_CLS(2, 5) FG_CLS(2, 6)
+          FG_CLS(3, 0) FG_CLS(3, 1) FG_CLS(3, 2) FG_CLS(3, 3) FG_CLS(3, 4)
+          FG_CLS(4, 0) FG_CLS(4, 1) FG_CLS(4, 2)
+          FG_CLS(5, 0)
+#undef FG_CLS
+          default: done = false; break;
+        }
+      }
+    }
+    if (!done) run_group_dyn<T, S, ABS>(p, nrec, nf, k, flags, Vt, vs, ne, st);
+    p += nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));
   }
 }
 

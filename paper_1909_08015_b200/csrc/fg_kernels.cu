@@ -125,8 +125,9 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
 
 __device__ __forceinline__ dd shfl_dd(dd v, int off) { return dd(__shfl_down_sync(0xffffffffu, v.hi, off), __shfl_down_sync(0xffffffffu, v.lo, off)); }
 
-template <class T, int S, int NT>
-__global__ void __launch_bounds__(NT) fg_eval_kernel(const FgPlanDev P, const RunArgs A) {
+template <class T, int S, int MAXNT>
+__global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const RunArgs A) {
+  const int NT = blockDim.x;
   extern __shared__ __align__(128) unsigned char smem[];
   ChunkRing ring; ring.buf = smem; ring.bar = (uint64_t*)(smem + 2 * FG_CHUNK_BYTES); ring.phase[0] = ring.phase[1] = 0u;
   T* Vsm = (T*)(smem + 2 * FG_CHUNK_BYTES + 128);
@@ -259,8 +260,8 @@ static int fail(int code, const std::string& m) { g_err = m; return code; }
 
 struct fg_graph { Graph g; };
 
-static const int NT_D = 128, S_D = 2;     // double pass: threads per block, samples per thread
-static const int NT_Q = 128, S_Q = 1;     // double-double pass
+static const int NT_D = 384, S_D = 1;     // double pass: max threads per block (launch bound), samples per thread
+static const int NT_Q = 192, S_Q = 1;     // double-double pass
 static const uint64_t SLAB = 1ull << 24;  // samples per launch (bounds the re-evaluation queue)
 
 struct fg_plan {
@@ -268,7 +269,7 @@ struct fg_plan {
   std::vector<void*> allocs;
   void* scratch = nullptr; double* partials = nullptr; Accum* accum = nullptr; fg_result* result_dev = nullptr;
   uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr;
-  int grid_d = 0, grid_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
+  int grid_d = 0, grid_q = 0, nt_d = 0, nt_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
   int64_t table_bytes = 0;
   int profile = 0; cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; double ms[3] = {0, 0, 0}; long long launches = 0, flagged_last = 0;
   std::mutex mu;
@@ -354,16 +355,23 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
 #undef UP
   int vmax = 1; for (auto& E : H.geoms) vmax = std::max(vmax, E.ne * (E.ne + 1) / 2 + 2 * E.ne);
   p->vmax = vmax;
-  p->smem_d = 2 * FG_CHUNK_BYTES + 128 + (size_t)vmax * NT_D * S_D * sizeof(double);
-  p->smem_q = 2 * FG_CHUNK_BYTES + 128 + (size_t)vmax * NT_Q * S_Q * sizeof(dd);
-  p->grid_d = p->sms; p->grid_q = p->sms;
-  // the attribute is per function, not per plan: always raise it to the device limit
+  // threads per block: as many warps as the per-sample operand table V (vmax entries) leaves room for in shared memory
   int smem_max = 0; cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
-  if ((size_t)smem_max < p->smem_d || (size_t)smem_max < p->smem_q) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
+  const size_t ring_bytes = 2 * FG_CHUNK_BYTES + 128;
+  auto fit = [&](int maxnt, size_t per_thread) { long nt = ((long)smem_max - (long)ring_bytes) / (long)per_thread; nt = std::min<long>(maxnt, nt / 32 * 32); return (int)nt; };
+  p->nt_d = fit(NT_D, (size_t)vmax * S_D * sizeof(double)); p->nt_q = fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd));
+  if (p->nt_d < 32 || p->nt_q < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
+  p->smem_d = ring_bytes + (size_t)vmax * p->nt_d * S_D * sizeof(double);
+  p->smem_q = ring_bytes + (size_t)vmax * p->nt_q * S_Q * sizeof(dd);
+  // the attribute is per function, not per plan: always raise it to the device limit
   auto setattr = [&](const void* f) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max); };
   e = setattr((const void*)fg_eval_kernel<double, S_D, NT_D>); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>);
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("shared memory: ") + cudaGetErrorString(e)); }
-  size_t sc = (size_t)H.scratch_slots * std::max((size_t)NT_D * S_D * sizeof(double) * p->grid_d, (size_t)NT_Q * S_Q * sizeof(dd) * p->grid_q);
+  int bps_d = 1, bps_q = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_d, fg_eval_kernel<double, S_D, NT_D>, p->nt_d, p->smem_d);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_q, fg_eval_kernel<dd, S_Q, NT_Q>, p->nt_q, p->smem_q);
+  p->grid_d = p->sms * std::max(1, std::min(bps_d, 4)); p->grid_q = p->sms * std::max(1, std::min(bps_q, 2));
+  size_t sc = (size_t)H.scratch_slots * std::max((size_t)p->nt_d * S_D * sizeof(double) * p->grid_d, (size_t)p->nt_q * S_Q * sizeof(dd) * p->grid_q);
   auto dmalloc = [&](void** d, size_t bytes) { cudaError_t e2 = cudaMalloc(d, bytes); if (e2 == cudaSuccess) { p->allocs.push_back(*d); cudaMemset(*d, 0, bytes); } return e2; };
   e = dmalloc(&p->scratch, sc);
   if (e == cudaSuccess) e = dmalloc((void**)&p->partials, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double));
@@ -437,11 +445,11 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
   if (mode != 2) {
     CU(cudaMemsetAsync(p->flag_count, 0, sizeof(unsigned long long), st));
     A.flag_list = p->flag_list; A.flag_count = p->flag_count; A.do_flag = (mode == 0); A.partials = p->partials;
-    uint64_t nbatch = (n + (uint64_t)NT_D * S_D - 1) / ((uint64_t)NT_D * S_D);
+    uint64_t nbatch = (n + (uint64_t)p->nt_d * S_D - 1) / ((uint64_t)p->nt_d * S_D);
     int grid = (int)std::min<uint64_t>((uint64_t)p->grid_d, std::max<uint64_t>(nbatch, 1));
     CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
     if (p->profile) CU(cudaEventRecord(p->ev[0], st));
-    fg_eval_kernel<double, S_D, NT_D><<<grid, NT_D, p->smem_d, st>>>(p->D, A);
+    fg_eval_kernel<double, S_D, NT_D><<<grid, p->nt_d, p->smem_d, st>>>(p->D, A);
     CU(cudaGetLastError()); ++p->launches;
     if (p->profile) CU(cudaEventRecord(p->ev[1], st));
     nparts = p->grid_d;
@@ -450,7 +458,7 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
     RunArgs B = A; B.do_flag = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
     if (mode == 0) { B.idlist = p->flag_list; B.idcount = p->flag_count; }
     if (p->profile && mode == 2) { CU(cudaEventRecord(p->ev[0], st)); CU(cudaEventRecord(p->ev[1], st)); }
-    fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, NT_Q, p->smem_q, st>>>(p->D, B);
+    fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, p->nt_q, p->smem_q, st>>>(p->D, B);
     CU(cudaGetLastError()); ++p->launches;
     nparts = p->grid_d + p->grid_q;
   }

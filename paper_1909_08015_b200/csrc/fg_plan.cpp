@@ -355,7 +355,11 @@ static void build_records(const HGeom& E, int type, HNum& N, bool& limit_hit) {
   }
   if (over) limit_hit = true;
   for (auto& v : per) for (auto& r : v) N.recs.push_back(std::move(r));
-  std::stable_sort(N.recs.begin(), N.recs.end(), [](const HRecord& a, const HRecord& b) { return a.dst < b.dst; });
+  std::stable_sort(N.recs.begin(), N.recs.end(), [](const HRecord& a, const HRecord& b) {
+    if (a.dst != b.dst) return a.dst < b.dst;
+    if (a.nf != b.nf) return a.nf < b.nf;
+    if (a.k != b.k) return a.k > b.k;
+    return (a.flags & 3) < (b.flags & 3); });
   for (auto& r : N.recs) {
     long nc = (long)r.coef.size(), nz = 0; for (double v : r.coef) if (v != 0.0) ++nz;
     int nco = (r.flags & FG_REC_TWO) ? 2 : 1;
@@ -543,19 +547,31 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     d.geom = N.geom; d.op = N.op; d.ncomp = N.ncomp; d.nse = N.nse;
     d.node_begin = N.nodes.empty() ? 0 : N.nodes.front(); d.node_count = (int)N.nodes.size();
     d.chunk_begin = (int)(P.d_chunks.size() / FG_CHUNK_BYTES);
-    // pack records into chunks; keep = leading product factors shared with the previous record of the chunk
-    size_t cur = 0; bool open = false; int nrec = 0; size_t base = 0; const HRecord* prev = nullptr;
-    auto close_chunk = [&]() { if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.nrec = nrec; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
+    // pack records into chunks of class-uniform groups; keep = leading product factors shared with the previous record
+    size_t cur = 0, base = 0, ghdr = 0; bool open = false, gopen = false; int ngroups = 0, gn = 0; const HRecord* prev = nullptr;
+    auto cls = [](const HRecord& r) { int fl = r.flags & (FG_REC_TWO | FG_REC_QEXT); if (r.nf > FG_NFC) fl |= FG_REC_WIDE; return (r.dst << 16) | (r.nf << 12) | (r.k << 8) | fl; };
+    auto close_group = [&]() { if (gopen) { FgGroupHdr g; std::memcpy(&g, &P.d_chunks[ghdr], sizeof(g)); g.nrec = (uint16_t)gn; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); gopen = false; } };
+    auto close_chunk = [&]() { close_group(); if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.ngroups = ngroups; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
     for (auto& r : N.recs) {
-      size_t need = sizeof(FgRecHdr) + r.coef.size() * sizeof(double);
-      if (!open || cur + need > FG_CHUNK_BYTES) { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); nrec = 0; open = true; prev = nullptr; }
+      const bool wide = r.nf > FG_NFC;
+      size_t need = (wide ? sizeof(FgRecW) : sizeof(FgRecC)) + r.coef.size() * sizeof(double);
+      bool newgroup = !gopen || !prev || cls(*prev) != cls(r) || gn >= 65535;
+      if (!open || cur + need + (newgroup ? sizeof(FgGroupHdr) : 0) > FG_CHUNK_BYTES) {
+        close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); ngroups = 0; open = true; newgroup = true;
+      }
+      if (newgroup) {
+        close_group();
+        FgGroupHdr g; std::memset(&g, 0, sizeof(g)); g.nf = (uint8_t)r.nf; g.k = (uint8_t)r.k; g.dst = (uint8_t)r.dst;
+        g.flags = (uint8_t)((r.flags & (FG_REC_TWO | FG_REC_QEXT)) | (wide ? FG_REC_WIDE : 0));
+        ghdr = base + cur; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); cur += sizeof(g); gopen = true; gn = 0; ++ngroups; prev = nullptr;
+      }
       int keep = 0;
-      if (prev) while (keep < r.nf && keep < prev->nf && keep < 15 && r.fidx[keep] == prev->fidx[keep]) ++keep;
-      FgRecHdr h; std::memset(&h, 0, sizeof(h)); h.nf = (uint8_t)r.nf; h.k = (uint8_t)r.k; h.dst = (uint8_t)r.dst; h.flags = (uint8_t)(r.flags | (keep << 4));
-      std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs[0] = r.cabs[0]; h.cabs[1] = r.cabs[1];
-      std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h);
+      if (prev) while (keep < r.nf && keep < prev->nf && r.fidx[keep] == prev->fidx[keep]) ++keep;
+      const float cab = std::max(r.cabs[0], r.cabs[1]);
+      if (wide) { FgRecW h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
+      else { FgRecC h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
       std::memcpy(&P.d_chunks[base + cur], r.coef.data(), r.coef.size() * sizeof(double)); cur += r.coef.size() * sizeof(double);
-      ++nrec; prev = &r;
+      ++gn; prev = &r;
       N.exec_flops += std::max(0, r.nf - std::max(keep, 1)); N.algo_flops += std::max(0, r.nf - std::max(keep, 1));
     }
     close_chunk();

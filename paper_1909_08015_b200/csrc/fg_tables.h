@@ -50,23 +50,33 @@ struct FgTermDev {
   int32_t geom[FG_MAXMEM];    // geometries of the members (for prod U_S^2 and sum W_S)
 };
 
-// Record header inside a chunk (32 bytes, 16-byte aligned, followed by the coefficient tables as doubles):
+// Numerator stream.  A chunk (FG_CHUNK_BYTES, 16-byte aligned) holds groups; a group
+// holds records of ONE class (nf, k, flags) that add to ONE accumulator dst, so the kernel runs a fully static inner loop
+// per class.  One record:
 //   plain:        value = prod_{f<nf} V[fidx[f]] * sum_T coef[T] prod_{j in T} V[vidx[j]]        (2^k coefs per component)
 //   q-extension:  ... + prod * sum_{j<k} V[vidx[j] + ne] * sum_{T subset vars\j} coefq_j[T] prod_{i in T} V[vidx[i]]
 //                 (k further tables of 2^(k-1) coefs: the slot that carries gamma^nu with weight A^q_j)
-// added to accumulator dst.  keep = number of leading product factors shared with the previous record of the chunk.
-// cabs[c] = sum of |coef| of component c: with |A_j|, |A^q_j| <= 1 it bounds the sum of |terms| of the record.
-#define FG_REC_TWO 1
-#define FG_REC_QEXT 2
-struct alignas(16) FgRecHdr {
-  uint8_t nf, k, dst, flags;      // flags: bit0 two components, bit1 q-extension, bits 4..7 keep
+// keep = number of leading product factors shared with the previous record of the group (prefix products are kept).
+// cabs = sum of |coef| (max over components): with |A_j|, |A^q_j| <= 1 it bounds the sum of |terms| of the record.
+#define FG_REC_TWO 1       // two components (u, v) of a self-energy element
+#define FG_REC_QEXT 2      // q-extension tables follow
+#define FG_REC_WIDE 4      // records use the wide header (nf > FG_NFC): generic slow path
+#define FG_NFC 5           // product factors of a compact record (= Wick pairs, <= n)
+struct alignas(16) FgRecC {   // compact record header, 16 bytes, followed by the coefficient tables (even count of doubles)
+  uint8_t keep;
+  uint8_t fidx[FG_NFC];
+  uint8_t vidx[FG_KMAX];
+  float cabs;
+};
+struct alignas(16) FgRecW {   // wide record header, 32 bytes
+  uint8_t keep, pad0[3];
   uint8_t fidx[FG_MAXF];
   uint8_t vidx[FG_KMAX];
-  uint8_t pad[4];
-  float cabs[2];
+  uint8_t pad1[8];
+  float cabs;
 };
-// Chunk header (16 bytes): number of records in the chunk.
-struct alignas(16) FgChunkHdr { int32_t nrec; int32_t pad[3]; };
+struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t pad[10]; };
+struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
 
 // Everything the kernels need, passed by value.
 struct FgPlanDev {
