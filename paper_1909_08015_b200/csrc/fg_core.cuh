@@ -183,30 +183,37 @@ FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T
 // ------------------------------------------------------------------------------------------------
 // a6  multilinear polynomial in K variables with a dense 2^K coefficient table (uniform across the block)
 // ------------------------------------------------------------------------------------------------
-template <class T, int S, int K, bool AC = false> struct Horner {   // AC: use |coef| (for the sum of |terms|)
+template <class T, int S, int K, bool AC = false, bool RC = false> struct Horner {   // AC: use |coef|; RC: coefs already in registers
   static FG_HD void run(const double* __restrict__ c, const T (*a)[S], T* out) {
     T lo[S], hi[S];
-    Horner<T, S, K - 1, AC>::run(c, a, lo); Horner<T, S, K - 1, AC>::run(c + (1 << (K - 1)), a, hi);
+    Horner<T, S, K - 1, AC, RC>::run(c, a, lo); Horner<T, S, K - 1, AC, RC>::run(c + (1 << (K - 1)), a, hi);
 #pragma unroll
     for (int s = 0; s < S; ++s) out[s] = t_fma(a[K - 1][s], hi[s], lo[s]);
   }
 };
-template <class T, int S, bool AC> struct Horner<T, S, 0, AC> {
+template <class T, int S, bool AC, bool RC> struct Horner<T, S, 0, AC, RC> {
   static FG_HD void run(const double* __restrict__ c, const T (*)[S], T* out) {
     const double c0 = AC ? fabs(c[0]) : c[0];
 #pragma unroll
     for (int s = 0; s < S; ++s) out[s] = T(c0);
   }
 };
-template <int S, bool AC> struct Horner<double, S, 1, AC> {   // leaf FMA takes both coefficients straight from the table
+#if defined(__CUDACC__)
+FG_HD void ld_coef2(const double* __restrict__ c, double& c0, double& c1) { const double2 v = *reinterpret_cast<const double2*>(c); c0 = v.x; c1 = v.y; }   // one 128-bit (broadcast) load
+#else
+FG_HD void ld_coef2(const double* __restrict__ c, double& c0, double& c1) { c0 = c[0]; c1 = c[1]; }
+#endif
+template <int S, bool AC, bool RC> struct Horner<double, S, 1, AC, RC> {   // leaf FMA takes both coefficients straight from the table (16-byte aligned)
   static FG_HD void run(const double* __restrict__ c, const double (*a)[S], double* out) {
-    const double c0 = AC ? fabs(c[0]) : c[0], c1 = AC ? fabs(c[1]) : c[1];
+    double c0, c1;
+    if (RC) { c0 = c[0]; c1 = c[1]; } else ld_coef2(c, c0, c1);
+    if (AC) { c0 = fabs(c0); c1 = fabs(c1); }
 #pragma unroll
     for (int s = 0; s < S; ++s) out[s] = fma(a[0][s], c1, c0);
   }
 };
 // q-extension: q += sum_j aq[j] * (multilinear in the K-1 variables other than j)
-template <class T, int S, int K, bool AC = false> struct QExt {
+template <class T, int S, int K, bool AC = false, bool RC = false> struct QExt {
   static FG_HD void run(const double* __restrict__ cq, const T (*a)[S], const T (*aq)[S], T* q) {
 #pragma unroll
     for (int j = 0; j < K; ++j) {
@@ -216,13 +223,13 @@ template <class T, int S, int K, bool AC = false> struct QExt {
 #pragma unroll
         for (int s = 0; s < S; ++s) b[i][s] = a[i < j ? i : i + 1][s];
       }
-      Horner<T, S, K - 1, AC>::run(cq + j * (1 << (K - 1)), b, sub);
+      Horner<T, S, K - 1, AC, RC>::run(cq + j * (1 << (K - 1)), b, sub);
 #pragma unroll
       for (int s = 0; s < S; ++s) q[s] = t_fma(aq[j][s], sub[s], q[s]);
     }
   }
 };
-template <class T, int S, bool AC> struct QExt<T, S, 0, AC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
+template <class T, int S, bool AC, bool RC> struct QExt<T, S, 0, AC, RC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
 // Running state of one program: accumulators of the current destination.
 template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; int cur; };
@@ -232,15 +239,36 @@ FG_HD constexpr int rec_ncoef(int k, int flags) {
 }
 
 // One group of compact records, class known at compile time: the inner loop has no data-dependent control flow
-// except the (block-uniform) prefix depth `keep`.  ABS as in run_chunk.
+// except the (block-uniform) prefix depth `keep`.  Kept out of line on the device so that every class gets its own
+// register allocation and instruction schedule (the accumulators travel through memory once per group).
+// The coefficients of a record are read into registers first (128-bit broadcast loads, all in flight together),
+// then consumed by the FMA tree: the shared-memory latency is paid once per record, not once per FMA.
+#if defined(__CUDACC__)
+#define FG_NOINLINE __device__ __noinline__
+#else
+#define FG_NOINLINE inline
+#endif
 template <class T, int S, int ABS, int NF, int K, bool QX>
-FG_HD void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* acc, double* aab) {
+FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* __restrict__ accp, double* __restrict__ aabp) {
+#if defined(__CUDA_ARCH__)
+  __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vt));
+#endif
   constexpr int FL = QX ? FG_REC_QEXT : 0;
-  constexpr int STRIDE = (int)sizeof(FgRecC) + rec_ncoef(K, FL) * (int)sizeof(double);
-  T pf[NF > 0 ? NF : 1][S];
+  constexpr int NC = rec_ncoef(K, FL);
+  constexpr int STRIDE = (int)sizeof(FgRecC) + NC * (int)sizeof(double);
+  constexpr bool PRELOAD = NC <= 48;      // tables small enough to sit in registers
+  T pf[NF > 0 ? NF : 1][S], acc[S]; double aab[S];
+#pragma unroll
+  for (int s = 0; s < S; ++s) { acc[s] = accp[s]; aab[s] = aabp[s]; }
   for (int r = 0; r < nrec; ++r, p += STRIDE) {
     const FgRecC h = *(const FgRecC*)p;
     const double* __restrict__ coef = (const double*)(p + sizeof(FgRecC));
+    double cr[PRELOAD ? NC : 2];
+    if (PRELOAD) {
+#pragma unroll
+      for (int i = 0; i < NC; i += 2) ld_coef2(coef + i, cr[i], cr[i + 1]);
+    }
+    const double* __restrict__ cc = PRELOAD ? cr : coef;
     const int keep = h.keep;
 #pragma unroll
     for (int f = 0; f < NF; ++f) if (f >= keep) {
@@ -261,8 +289,8 @@ FG_HD void run_group_static(const unsigned char* __restrict__ p, int nrec, const
       }
     }
     T q[S];
-    Horner<T, S, K>::run(coef, a, q);
-    if (QX) QExt<T, S, K>::run(coef + (1 << K), a, aq, q);
+    Horner<T, S, K, false, PRELOAD>::run(cc, a, q);
+    if (QX) QExt<T, S, K, false, PRELOAD>::run(cc + (1 << K), a, aq, q);
     const double cab = (double)h.cabs;
 #pragma unroll
     for (int s = 0; s < S; ++s) {
@@ -270,6 +298,8 @@ FG_HD void run_group_static(const unsigned char* __restrict__ p, int nrec, const
       else { acc[s] = acc[s] + q[s]; if (ABS) aab[s] += cab; }
     }
   }
+#pragma unroll
+  for (int s = 0; s < S; ++s) { accp[s] = acc[s]; aabp[s] = aab[s]; }
 }
 
 // One group of any class, everything dynamic (wide records, two-component records, the double-double pass).
