@@ -238,6 +238,16 @@ FG_HD constexpr int rec_ncoef(int k, int flags) {
   return (((flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k) + 1) & ~1;
 }
 
+#if defined(__CUDACC__)
+template <int I, int N> struct PreLoad {
+  static __device__ __forceinline__ void run(unsigned caddr, double* cr) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(cr[I]), "=d"(cr[I + 1]) : "r"(caddr), "n"(I * 8));
+    PreLoad<I + 2, N>::run(caddr, cr);
+  }
+};
+template <int N> struct PreLoad<N, N> { static __device__ __forceinline__ void run(unsigned, double*) {} };
+#endif
+
 // One group of compact records, class known at compile time: the inner loop has no data-dependent control flow
 // except the (block-uniform) prefix depth `keep`.  Kept out of line on the device so that every class gets its own
 // register allocation and instruction schedule (the accumulators travel through memory once per group).
@@ -265,8 +275,14 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
     const double* __restrict__ coef = (const double*)(p + sizeof(FgRecC));
     double cr[PRELOAD ? NC : 2];
     if (PRELOAD) {
-#pragma unroll
-      for (int i = 0; i < NC; i += 2) ld_coef2(coef + i, cr[i], cr[i + 1]);
+#if defined(__CUDA_ARCH__)
+      // volatile PTX keeps these loads together at the head of the record (the compiler otherwise sinks each load
+      // next to its FMA and the warp pays the shared-memory latency once per FMA pair)
+      const unsigned caddr = (unsigned)__cvta_generic_to_shared(coef);
+      PreLoad<0, NC>::run(caddr, cr);
+#else
+      for (int i = 0; i < NC; ++i) cr[i] = coef[i];
+#endif
     }
     const double* __restrict__ cc = PRELOAD ? cr : coef;
     const int keep = h.keep;
@@ -288,6 +304,9 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
         for (int s = 0; s < S; ++s) aq[j][s] = pq[s];
       }
     }
+#if defined(__CUDA_ARCH__)
+    __syncwarp();   // scheduling fence: every load of the record is issued before the first FMA waits on one
+#endif
     T q[S];
     Horner<T, S, K, false, PRELOAD>::run(cc, a, q);
     if (QX) QExt<T, S, K, false, PRELOAD>::run(cc + (1 << K), a, aq, q);
@@ -332,7 +351,7 @@ FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, 
 #define FG_CASE(K) case K: Horner<T, S, K>::run(coef, a, q[0]); \
                            if (flags & FG_REC_TWO) Horner<T, S, K>::run(coef + (1 << K), a, q[1]); \
                            else if (flags & FG_REC_QEXT) QExt<T, S, K>::run(coef + (1 << K), a, aq, q[0]); break;
-      FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4) FG_CASE(5) FG_CASE(6)
+      FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4)
 #undef FG_CASE
       default: break;
     }
@@ -347,7 +366,7 @@ FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, 
 #define FG_CASE(K) case K: Horner<double, S, K, true>::run(coef, ab, qa[0]); \
                            if (flags & FG_REC_TWO) Horner<double, S, K, true>::run(coef + (1 << K), ab, qa[1]); \
                            else if (flags & FG_REC_QEXT) QExt<double, S, K, true>::run(coef + (1 << K), ab, abq, qa[0]); break;
-        FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4) FG_CASE(5) FG_CASE(6)
+        FG_CASE(0) FG_CASE(1) FG_CASE(2) FG_CASE(3) FG_CASE(4)
 #undef FG_CASE
         default: break;
       }
@@ -365,6 +384,131 @@ FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, 
     }
   }
 }
+
+// ---- tensor-core groups (FG_REC_MMA): monomial order shared by the planner, the scalar interpreter and the DMMA path ----
+FG_HD constexpr int mma_steps(int k, bool qx) { return (1 << (k - 2)) + (qx ? (1 << (k - 2)) + (k - 2) * ((1 << k) >> 3) : 0); }
+
+// all monomials of one point: mono[4*step + x] (see FgRecM in fg_tables.h)
+template <class T>
+FG_HD void mma_monomials(int k, bool qx, const T* a, const T* aq, T* mono) {
+  const int nm = 1 << (k - 2);
+  T mlo[4] = {T(1.0), a[0], a[1], a[0] * a[1]};
+  for (int t = 0; t < nm; ++t) {
+    T h = T(1.0); for (int i = 0; i + 2 < k; ++i) if ((t >> i) & 1) h = h * a[2 + i];
+    for (int x = 0; x < 4; ++x) mono[4 * t + x] = mlo[x] * h;
+    if (qx) {
+      mono[4 * (nm + t) + 0] = aq[0] * h; mono[4 * (nm + t) + 1] = aq[0] * a[1] * h;
+      mono[4 * (nm + t) + 2] = aq[1] * h; mono[4 * (nm + t) + 3] = aq[1] * a[0] * h;
+    }
+  }
+  if (qx) {
+    const int nh = (1 << k) >> 3; int step = 2 * nm;
+    for (int j = 2; j < k; ++j) for (int t2 = 0; t2 < nh; ++t2, ++step) {
+      T h = aq[j]; int bit = 0;
+      for (int i = 2; i < k; ++i) if (i != j) { if ((t2 >> bit) & 1) h = h * a[i]; ++bit; }
+      for (int x = 0; x < 4; ++x) mono[4 * step + x] = mlo[x] * h;
+    }
+  }
+}
+
+// scalar interpreter of a tensor-core group (double-double pass, host harness): one point per thread
+template <class T, int S, int ABS>
+FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, int nf, int k, int flags, const uint8_t* vidx, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st) {
+  const bool qx = (flags & FG_REC_QEXT) != 0; const int steps = mma_steps(k, qx);
+  T mono[S][48]; double monoa[S][48];
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    T a[FG_KMAX], aq[FG_KMAX];
+    for (int j = 0; j < k; ++j) { a[j] = Vt[(int)vidx[j] * vs + s]; aq[j] = qx ? Vt[((int)vidx[j] + ne) * vs + s] : T(0.0); }
+    mma_monomials<T>(k, qx, a, aq, mono[s]);
+    if (ABS == 2) for (int J = 0; J < 4 * steps; ++J) monoa[s][J] = t_abs_d(mono[s][J]);
+  }
+  const int tile_bytes = 8 * (int)sizeof(FgRecM) + steps * 32 * (int)sizeof(double);
+  for (int t = 0; t < ntiles; ++t, p += tile_bytes) {
+    const FgRecM* recs = (const FgRecM*)p; const double* __restrict__ fr = (const double*)(p + 8 * sizeof(FgRecM));
+    for (int n = 0; n < 8; ++n) {
+      const double cab = (double)recs[n].cabs;
+#pragma unroll
+      for (int s = 0; s < S; ++s) {
+        T q = T(0.0); double qa = 0.0;
+        for (int J = 0; J < 4 * steps; ++J) { const double c = fr[(J >> 2) * 32 + n * 4 + (J & 3)]; q = q + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
+        T bp = T(1.0); for (int f = 0; f < nf; ++f) bp = bp * Vt[(int)recs[n].fidx[f] * vs + s];
+        st.acc[0][s] = st.acc[0][s] + bp * q;
+        if (ABS == 1) st.aab[0][s] = fma(t_abs_d(bp), cab, st.aab[0][s]);
+        if (ABS == 2) st.aab[0][s] = fma(t_abs_d(bp), qa, st.aab[0][s]);
+      }
+    }
+  }
+}
+
+#if defined(__CUDACC__)
+// Tensor-core path of a group (double pass, one sample per thread, whole warp converged).  DMMA m8n8k4:
+//   A (8 samples x 4 monomials): lane (r = lane/4, c = lane%4) holds monomial 4*step + c of sample 8*b + r;
+//   B (4 monomials x 8 records): lane holds coef[4*step + c] of record r -> one conflict-free LDS.64 per step;
+//   D (8 x 8): lane holds records 2c, 2c+1 of sample 8*b + r.
+// Each lane then weights its two record values with their products of beta's and keeps per-lane partial sums for the four
+// row blocks b; out[0..3] = value partials, out[4..7] = |.| partials (reduced over the quad by the caller).
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+template <int NF, int K, bool QX>
+__device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict__ p, int ntiles, const double* __restrict__ Vw, int vs, int ne, unsigned vidx4, double* __restrict__ out) {
+  __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
+  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
+  const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
+  const int v0 = (int)(vidx4 & 255u) * vs, v1 = (int)((vidx4 >> 8) & 255u) * vs, v2 = (int)((vidx4 >> 16) & 255u) * vs, v3 = (int)(vidx4 >> 24) * vs, vq = ne * vs;
+  double acc[4] = {0.0, 0.0, 0.0, 0.0}, aab[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int t = 0; t < ntiles; ++t, p += TILE) {
+    const uint4 h0 = *(const uint4*)(p + (2 * c) * 16), h1 = *(const uint4*)(p + (2 * c + 1) * 16);
+    double B[STEPS];
+#pragma unroll
+    for (int st = 0; st < STEPS; ++st) B[st] = ((const double*)(p + 8 * sizeof(FgRecM)))[st * 32 + lane];
+    const double cab0 = (double)__uint_as_float(h0.w), cab1 = (double)__uint_as_float(h1.w);
+    int f0[NF > 0 ? NF : 1], f1[NF > 0 ? NF : 1];
+#pragma unroll
+    for (int i = 0; i < NF; ++i) {
+      f0[i] = (int)((i < 4 ? (h0.x >> (8 * i)) : h0.y) & 255u) * vs;
+      f1[i] = (int)((i < 4 ? (h1.x >> (8 * i)) : h1.y) & 255u) * vs;
+    }
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const double* __restrict__ Vs = Vw + 8 * b + r;
+      const double a0 = Vs[v0], a1 = Vs[v1];
+      const double a2 = K > 2 ? Vs[v2] : 1.0, a3 = K > 3 ? Vs[v3] : 1.0;
+      const double a01 = a0 * a1;
+      const double mlo = c == 0 ? 1.0 : c == 1 ? a0 : c == 2 ? a1 : a01;
+      double hi[NM]; hi[0] = 1.0;
+      if (K > 2) hi[1] = a2;
+      if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
+      double d0 = 0.0, d1 = 0.0;
+      dmma884(d0, d1, mlo, B[0]);
+#pragma unroll
+      for (int tt = 1; tt < NM; ++tt) dmma884(d0, d1, mlo * hi[tt], B[tt]);
+      if (QX) {
+        const double q0 = Vs[v0 + vq], q1 = Vs[v1 + vq];
+        const double mq = c == 0 ? q0 : c == 1 ? q0 * a1 : c == 2 ? q1 : q1 * a0;
+        dmma884(d0, d1, mq, B[NM]);
+#pragma unroll
+        for (int tt = 1; tt < NM; ++tt) dmma884(d0, d1, mq * hi[tt], B[NM + tt]);
+        if (K == 3) { const double q2 = Vs[v2 + vq]; dmma884(d0, d1, mlo * q2, B[2 * NM]); }
+        if (K == 4) {
+          const double q2 = Vs[v2 + vq], q3 = Vs[v3 + vq];
+          const double m2 = mlo * q2, m3 = mlo * q3;
+          dmma884(d0, d1, m2, B[2 * NM]); dmma884(d0, d1, m2 * a3, B[2 * NM + 1]);
+          dmma884(d0, d1, m3, B[2 * NM + 2]); dmma884(d0, d1, m3 * a2, B[2 * NM + 3]);
+        }
+      }
+      double bp0 = 1.0, bp1 = 1.0;
+#pragma unroll
+      for (int i = 0; i < NF; ++i) { bp0 = (i == 0) ? Vs[f0[i]] : bp0 * Vs[f0[i]]; bp1 = (i == 0) ? Vs[f1[i]] : bp1 * Vs[f1[i]]; }
+      acc[b] = fma(bp0, d0, acc[b]); acc[b] = fma(bp1, d1, acc[b]);
+      aab[b] = fma(fabs(bp0), cab0, aab[b]); aab[b] = fma(fabs(bp1), cab1, aab[b]);
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < 4; ++b) { out[b] = acc[b]; out[4 + b] = aab[b]; }
+}
+#endif
 
 // All groups of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
 // ABS: 0 no |.| tracking, 1 bound by cabs (needs |A|,|A^q| <= 1), 2 exact sum of |coef| prod |A| in double
@@ -386,22 +530,56 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
     }
     bool done = false;
     if constexpr (!is_dd<T>::value && ABS != 2) {
-      if (!(flags & (FG_REC_WIDE | FG_REC_TWO))) {
+      if (!(flags & (FG_REC_WIDE | FG_REC_TWO | FG_REC_MMA))) {
         done = true;
         const bool qx = (flags & FG_REC_QEXT) != 0;
         switch (nf * 8 + k) {
 #define FG_CLS(NF, K) case NF * 8 + K: if (qx) run_group_static<T, S, ABS, NF, K, true>(p, nrec, Vt, vs, ne, st.acc[0], st.aab[0]); \
                                         else run_group_static<T, S, ABS, NF, K, false>(p, nrec, Vt, vs, ne, st.acc[0], st.aab[0]); break;
-          FG_CLS(0, 0) FG_CLS(0, 1) FG_CLS(0, 2) FG_CLS(0, 3) FG_CLS(0, 4) FG_CLS(0, 5) FG_CLS(0, 6)
-          FG_CLS(1, 0) FG_CLS(1, 1) FG_CLS(1, 2) FG_CLS(1, 3) FG_CLS(1, 4) FG_CLS(1, 5) FG_CLS(1, 6)
-          FG_CLS(2, 0) FG_CLS(2, 1) FG_CLS(2, 2) FG_CLS(2, 3) FG_CLS(2, 4) FG_CLS(2, 5) FG_CLS(2, 6)
+          FG_CLS(0, 0) FG_CLS(0, 1) FG_CLS(0, 2) FG_CLS(0, 3) FG_CLS(0, 4)
+          FG_CLS(1, 0) FG_CLS(1, 1) FG_CLS(1, 2) FG_CLS(1, 3) FG_CLS(1, 4)
+          FG_CLS(2, 0) FG_CLS(2, 1) FG_CLS(2, 2) FG_CLS(2, 3) FG_CLS(2, 4)
           FG_CLS(3, 0) FG_CLS(3, 1) FG_CLS(3, 2) FG_CLS(3, 3) FG_CLS(3, 4)
-          FG_CLS(4, 0) FG_CLS(4, 1) FG_CLS(4, 2)
-          FG_CLS(5, 0)
+          FG_CLS(4, 0) FG_CLS(4, 1) FG_CLS(4, 2) FG_CLS(4, 3) FG_CLS(4, 4)
+          FG_CLS(5, 0) FG_CLS(5, 1) FG_CLS(5, 2) FG_CLS(5, 3) FG_CLS(5, 4)
 #undef FG_CLS
           default: done = false; break;
         }
       }
+    }
+    if (flags & FG_REC_MMA) {
+#if defined(__CUDA_ARCH__)
+      if constexpr (!is_dd<T>::value && ABS == 1 && S == 1) {
+        double part[8]; done = true;
+        const double* Vw = (const double*)Vt - (threadIdx.x & 31);
+        const unsigned v4 = (unsigned)gh.vidx[0] | ((unsigned)gh.vidx[1] << 8) | ((unsigned)gh.vidx[2] << 16) | ((unsigned)gh.vidx[3] << 24);
+        const bool qx = (flags & FG_REC_QEXT) != 0;
+        switch (nf * 8 + k) {
+#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p, nrec, Vw, vs, ne, v4, part); else run_group_mma_fast<NF, K, false>(p, nrec, Vw, vs, ne, v4, part); break;
+          FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
+          FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
+#undef FG_MM
+          default: done = false; break;
+        }
+        if (done) {
+          // quad-reduce the partials, then hand every thread the sums of its own sample (lane L <- lane 4*(L%8), row block L/8)
+          const int lane = threadIdx.x & 31, src = (lane & 7) << 2, myb = lane >> 3;
+          double mv = 0.0, ma = 0.0;
+#pragma unroll
+          for (int b = 0; b < 4; ++b) {
+            double v = part[b], w = part[4 + b];
+            v += __shfl_xor_sync(0xffffffffu, v, 1); w += __shfl_xor_sync(0xffffffffu, w, 1);
+            v += __shfl_xor_sync(0xffffffffu, v, 2); w += __shfl_xor_sync(0xffffffffu, w, 2);
+            v = __shfl_sync(0xffffffffu, v, src); w = __shfl_sync(0xffffffffu, w, src);
+            if (b == myb) { mv = v; ma = w; }
+          }
+          st.acc[0][0] = st.acc[0][0] + T(mv); st.aab[0][0] += ma;
+        }
+      }
+#endif
+      if (!done) run_group_mma_dyn<T, S, ABS>(p, nrec, nf, k, flags, gh.vidx, Vt, vs, ne, st);
+      p += nrec * (8 * (int)sizeof(FgRecM) + mma_steps(k, (flags & FG_REC_QEXT) != 0) * 32 * (int)sizeof(double));
+      continue;
     }
     if (!done) run_group_dyn<T, S, ABS>(p, nrec, nf, k, flags, Vt, vs, ne, st);
     p += nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));

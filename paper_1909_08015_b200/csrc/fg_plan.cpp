@@ -359,13 +359,12 @@ static void build_records(const HGeom& E, int type, HNum& N, bool& limit_hit) {
     if (a.dst != b.dst) return a.dst < b.dst;
     if (a.nf != b.nf) return a.nf < b.nf;
     if (a.k != b.k) return a.k > b.k;
-    return (a.flags & 3) < (b.flags & 3); });
+    if ((a.flags & 3) != (b.flags & 3)) return (a.flags & 3) < (b.flags & 3);
+    return std::memcmp(a.vidx, b.vidx, sizeof(a.vidx)) < 0; });
   for (auto& r : N.recs) {
     long nc = (long)r.coef.size(), nz = 0; for (double v : r.coef) if (v != 0.0) ++nz;
     int nco = (r.flags & FG_REC_TWO) ? 2 : 1;
     N.n_coefs += nc; N.n_nonzero += nz;
-    N.exec_flops += nco * (2.0 * ((1 << r.k) - 1) + 4.0);
-    if (r.flags & FG_REC_QEXT) N.exec_flops += r.k * (2.0 * ((1 << r.k) / 2 - 1) + 2.0);
     N.algo_flops += 2.0 * nz;
   }
 }
@@ -547,32 +546,74 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     d.geom = N.geom; d.op = N.op; d.ncomp = N.ncomp; d.nse = N.nse;
     d.node_begin = N.nodes.empty() ? 0 : N.nodes.front(); d.node_count = (int)N.nodes.size();
     d.chunk_begin = (int)(P.d_chunks.size() / FG_CHUNK_BYTES);
-    // pack records into chunks of class-uniform groups; keep = leading product factors shared with the previous record
+    // pack records into chunks of class-uniform groups; keep = leading product factors shared with the previous record.
+    // Runs of records with the same class and the same free variables become tensor-core (DMMA) tile groups.
     size_t cur = 0, base = 0, ghdr = 0; bool open = false, gopen = false; int ngroups = 0, gn = 0; const HRecord* prev = nullptr;
     auto cls = [](const HRecord& r) { int fl = r.flags & (FG_REC_TWO | FG_REC_QEXT); if (r.nf > FG_NFC) fl |= FG_REC_WIDE; return (r.dst << 16) | (r.nf << 12) | (r.k << 8) | fl; };
     auto close_group = [&]() { if (gopen) { FgGroupHdr g; std::memcpy(&g, &P.d_chunks[ghdr], sizeof(g)); g.nrec = (uint16_t)gn; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); gopen = false; } };
     auto close_chunk = [&]() { close_group(); if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.ngroups = ngroups; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
-    for (auto& r : N.recs) {
-      const bool wide = r.nf > FG_NFC;
-      size_t need = (wide ? sizeof(FgRecW) : sizeof(FgRecC)) + r.coef.size() * sizeof(double);
-      bool newgroup = !gopen || !prev || cls(*prev) != cls(r) || gn >= 65535;
-      if (!open || cur + need + (newgroup ? sizeof(FgGroupHdr) : 0) > FG_CHUNK_BYTES) {
-        close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); ngroups = 0; open = true; newgroup = true;
-      }
-      if (newgroup) {
+    auto new_chunk = [&]() { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); ngroups = 0; open = true; };
+    auto open_group = [&](const HRecord& r, int extra_flags) {
+      close_group();
+      FgGroupHdr g; std::memset(&g, 0, sizeof(g)); g.nf = (uint8_t)r.nf; g.k = (uint8_t)r.k; g.dst = (uint8_t)r.dst;
+      g.flags = (uint8_t)((r.flags & (FG_REC_TWO | FG_REC_QEXT)) | (r.nf > FG_NFC ? FG_REC_WIDE : 0) | extra_flags);
+      std::memcpy(g.vidx, r.vidx, sizeof(g.vidx));
+      ghdr = base + cur; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); cur += sizeof(g); gopen = true; gn = 0; ++ngroups; prev = nullptr;
+    };
+    auto mma_steps = [](int k, bool qx) { int nm = 1 << (k - 2); return nm + (qx ? nm + (k - 2) * ((1 << k) >> 3) : 0); };
+    auto mma_coef = [](const HRecord& r, int step, int x) -> double {
+      const int k = r.k, nm = 1 << (k - 2); const double* mainT = r.coef.data(); const double* qT = mainT + (1 << k); const int qs = (1 << k) >> 1;
+      if (step < nm) return mainT[x | (step << 2)];
+      if (step < 2 * nm) { int t = step - nm, j = x >> 1; return qT[j * qs + ((x & 1) | (t << 1))]; }
+      int s2 = step - 2 * nm, nh = (1 << k) >> 3, j = 2 + s2 / nh, t2 = s2 % nh; return qT[j * qs + (x | (t2 << 2))];
+    };
+    size_t nr = N.recs.size();
+    for (size_t i = 0; i < nr;) {
+      size_t j = i + 1;
+      while (j < nr && cls(N.recs[j]) == cls(N.recs[i]) && std::memcmp(N.recs[j].vidx, N.recs[i].vidx, sizeof(N.recs[i].vidx)) == 0) ++j;
+      const HRecord& r0 = N.recs[i];
+      const bool qx = (r0.flags & FG_REC_QEXT) != 0;
+      const bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= 2 && (j - i) >= FG_MMA_MINREC;
+      if (mma) {
+        const int steps = mma_steps(r0.k, qx); const size_t tile_bytes = 8 * sizeof(FgRecM) + (size_t)steps * 32 * sizeof(double);
+        for (size_t t0 = i; t0 < j; t0 += 8) {
+          bool need_group = !gopen || prev != nullptr;      // prev != nullptr: a regular group is open
+          if (!open || cur + tile_bytes + (need_group ? sizeof(FgGroupHdr) : 0) > FG_CHUNK_BYTES) { new_chunk(); need_group = true; }
+          if (need_group) open_group(r0, FG_REC_MMA);
+          for (int n = 0; n < 8; ++n) {
+            FgRecM h; std::memset(&h, 0, sizeof(h));
+            if (t0 + n < j) { const HRecord& r = N.recs[t0 + n]; std::memcpy(h.fidx, r.fidx, FG_NFC); h.cabs = std::max(r.cabs[0], r.cabs[1]); }
+            std::memcpy(&P.d_chunks[base + cur + n * sizeof(FgRecM)], &h, sizeof(h));
+          }
+          double* fr = (double*)&P.d_chunks[base + cur + 8 * sizeof(FgRecM)];
+          for (int st = 0; st < steps; ++st) for (int n = 0; n < 8; ++n) for (int x = 0; x < 4; ++x)
+            fr[st * 32 + n * 4 + x] = (t0 + n < j) ? mma_coef(N.recs[t0 + n], st, x) : 0.0;
+          cur += tile_bytes; ++gn;
+          N.exec_flops += 8.0 * (8.0 * steps + 2.0 * std::max(0, r0.nf - 1) + 4.0);
+        }
+        for (size_t t = i; t < j; ++t) N.algo_flops += std::max(0, N.recs[t].nf - 1);
         close_group();
-        FgGroupHdr g; std::memset(&g, 0, sizeof(g)); g.nf = (uint8_t)r.nf; g.k = (uint8_t)r.k; g.dst = (uint8_t)r.dst;
-        g.flags = (uint8_t)((r.flags & (FG_REC_TWO | FG_REC_QEXT)) | (wide ? FG_REC_WIDE : 0));
-        ghdr = base + cur; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); cur += sizeof(g); gopen = true; gn = 0; ++ngroups; prev = nullptr;
+        i = j; continue;
       }
-      int keep = 0;
-      if (prev) while (keep < r.nf && keep < prev->nf && r.fidx[keep] == prev->fidx[keep]) ++keep;
-      const float cab = std::max(r.cabs[0], r.cabs[1]);
-      if (wide) { FgRecW h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
-      else { FgRecC h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
-      std::memcpy(&P.d_chunks[base + cur], r.coef.data(), r.coef.size() * sizeof(double)); cur += r.coef.size() * sizeof(double);
-      ++gn; prev = &r;
-      N.exec_flops += std::max(0, r.nf - std::max(keep, 1)); N.algo_flops += std::max(0, r.nf - std::max(keep, 1));
+      for (size_t t = i; t < j; ++t) {
+        const HRecord& r = N.recs[t];
+        const bool wide = r.nf > FG_NFC;
+        size_t need = (wide ? sizeof(FgRecW) : sizeof(FgRecC)) + r.coef.size() * sizeof(double);
+        bool newgroup = !gopen || !prev || cls(*prev) != cls(r) || gn >= 65535;
+        if (!open || cur + need + (newgroup ? sizeof(FgGroupHdr) : 0) > FG_CHUNK_BYTES) { new_chunk(); newgroup = true; }
+        if (newgroup) open_group(r, 0);
+        int keep = 0;
+        if (prev) while (keep < r.nf && keep < prev->nf && r.fidx[keep] == prev->fidx[keep]) ++keep;
+        const float cab = std::max(r.cabs[0], r.cabs[1]);
+        if (wide) { FgRecW h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
+        else { FgRecC h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
+        std::memcpy(&P.d_chunks[base + cur], r.coef.data(), r.coef.size() * sizeof(double)); cur += r.coef.size() * sizeof(double);
+        ++gn; prev = &r;
+        const int nco = (r.flags & FG_REC_TWO) ? 2 : 1;
+        N.exec_flops += std::max(0, r.nf - std::max(keep, 1)) + nco * (2.0 * ((1 << r.k) - 1) + 4.0) + ((r.flags & FG_REC_QEXT) ? r.k * (2.0 * ((1 << r.k) / 2 - 1) + 2.0) : 0.0);
+        N.algo_flops += std::max(0, r.nf - std::max(keep, 1));
+      }
+      i = j;
     }
     close_chunk();
     d.chunk_count = (int)(P.d_chunks.size() / FG_CHUNK_BYTES) - d.chunk_begin;

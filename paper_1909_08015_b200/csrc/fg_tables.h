@@ -8,7 +8,7 @@
 #define FG_MAXLINES 15     // 3n
 #define FG_MAXM 15         // Feynman variables (3n, or 3n-1 after the merge of PAPER.md:222)
 #define FG_NDEG 6          // polynomial in t: degrees 0..5
-#define FG_KMAX 6          // free variables of one numerator record (dense 2^k table)
+#define FG_KMAX 4          // free variables of one numerator record (dense 2^k table); further ones are enumerated
 #define FG_MAXF 10         // product factors of one record
 #define FG_CHUNK_BYTES 8192   // numerator stream is cut into chunks of this size (records never straddle)
 #define FG_MAXSE 4         // self-energy children of one element
@@ -61,21 +61,35 @@ struct FgTermDev {
 #define FG_REC_TWO 1       // two components (u, v) of a self-energy element
 #define FG_REC_QEXT 2      // q-extension tables follow
 #define FG_REC_WIDE 4      // records use the wide header (nf > FG_NFC): generic slow path
+#define FG_REC_MMA 8       // tensor-core group: records that share their free variables, stored as 8-record tiles
 #define FG_NFC 5           // product factors of a compact record (= Wick pairs, <= n)
+#define FG_MMA_MINREC 5    // a run of records with equal free variables becomes a tensor-core group from this length on
 struct alignas(16) FgRecC {   // compact record header, 16 bytes, followed by the coefficient tables (even count of doubles)
   uint8_t keep;
   uint8_t fidx[FG_NFC];
   uint8_t vidx[FG_KMAX];
+  uint8_t pad[2];
   float cabs;
 };
 struct alignas(16) FgRecW {   // wide record header, 32 bytes
   uint8_t keep, pad0[3];
   uint8_t fidx[FG_MAXF];
   uint8_t vidx[FG_KMAX];
-  uint8_t pad1[8];
+  uint8_t pad1[10];
   float cabs;
 };
-struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t pad[10]; };
+static_assert(sizeof(FgRecC) == 16 && sizeof(FgRecW) == 32, "record header sizes");
+// Tensor-core group (FG_REC_MMA): for a fixed set of free variables the record values are a dense contraction
+//   Q[sample][record] = sum_J mono_J(a, a^q)[sample] * coef[J][record]
+// evaluated with DMMA m8n8k4 (8 samples x 4 monomials x 8 records).  Monomial J = 4*step + x:
+//   main  steps t < 2^(k-2):        mlo[x] * mhi[t],  mlo = {1, a0, a1, a0 a1}, mhi[t] = prod_{bit i of t} a_{2+i}
+//   low-q steps (q-extension):      {aq0, aq0 a1, aq1, aq1 a0}[x] * mhi[t]
+//   high-q steps, j = 2..k-1:       aq_j * mlo[x] * (product over the subset t' of the other high variables)
+// A tile = 8 x FgRecM (product factors, cabs) + steps x 32 doubles in B-fragment order (lane = 4*record + x).
+// The group header carries the free variables (vidx) and nrec = number of tiles.
+struct alignas(16) FgRecM { uint8_t fidx[FG_NFC]; uint8_t pad[7]; float cabs; };
+struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint8_t pad[6]; };
+static_assert(sizeof(FgRecM) == 16 && sizeof(FgGroupHdr) == 16, "group header sizes");
 struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
 
 // Everything the kernels need, passed by value.
