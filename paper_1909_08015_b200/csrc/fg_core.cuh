@@ -232,7 +232,7 @@ template <class T, int S, int K, bool AC = false, bool RC = false> struct QExt {
 template <class T, int S, bool AC, bool RC> struct QExt<T, S, 0, AC, RC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
 // Running state of one program: accumulators of the current destination.
-template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; int cur; };
+template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part; };   // part: per-lane DMMA partial sums
 
 FG_HD constexpr int rec_ncoef(int k, int flags) {
   return (((flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k) + 1) & ~1;
@@ -457,7 +457,9 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
   constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int v0 = (int)(vidx4 & 255u) * vs, v1 = (int)((vidx4 >> 8) & 255u) * vs, v2 = (int)((vidx4 >> 16) & 255u) * vs, v3 = (int)(vidx4 >> 24) * vs, vq = ne * vs;
-  double acc[4] = {0.0, 0.0, 0.0, 0.0}, aab[4] = {0.0, 0.0, 0.0, 0.0};
+  double acc[4], aab[4];
+#pragma unroll
+  for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; }
   for (int t = 0; t < ntiles; ++t, p += TILE) {
     const uint4 h0 = *(const uint4*)(p + (2 * c) * 16), h1 = *(const uint4*)(p + (2 * c + 1) * 16);
     double B[STEPS];
@@ -476,7 +478,7 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
       const double a0 = Vs[v0], a1 = Vs[v1];
       const double a2 = K > 2 ? Vs[v2] : 1.0, a3 = K > 3 ? Vs[v3] : 1.0;
       const double a01 = a0 * a1;
-      const double mlo = c == 0 ? 1.0 : c == 1 ? a0 : c == 2 ? a1 : a01;
+      const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
       double hi[NM]; hi[0] = 1.0;
       if (K > 2) hi[1] = a2;
       if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
@@ -486,7 +488,7 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
       for (int tt = 1; tt < NM; ++tt) dmma884(d0, d1, mlo * hi[tt], B[tt]);
       if (QX) {
         const double q0 = Vs[v0 + vq], q1 = Vs[v1 + vq];
-        const double mq = c == 0 ? q0 : c == 1 ? q0 * a1 : c == 2 ? q1 : q1 * a0;
+        const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
         dmma884(d0, d1, mq, B[NM]);
 #pragma unroll
         for (int tt = 1; tt < NM; ++tt) dmma884(d0, d1, mq * hi[tt], B[NM + tt]);
@@ -510,6 +512,29 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
 }
 #endif
 
+// Fold the per-lane DMMA partial sums into the accumulators of the owning threads: quad-reduce, then lane L takes the
+// sums of its own sample from lane 4*(L%8), row block L/8.  Called when the destination changes.
+template <class T, int S>
+FG_HD void fold_mma_partials(RecState<T, S>& st) {
+#if defined(__CUDA_ARCH__)
+  if constexpr (!is_dd<T>::value && S == 1) {
+    if (st.has_part) {
+      const int lane = threadIdx.x & 31, src = (lane & 7) << 2, myb = lane >> 3;
+      double mv = 0.0, ma = 0.0;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        double v = st.part[b], w = st.part[4 + b];
+        v += __shfl_xor_sync(0xffffffffu, v, 1); w += __shfl_xor_sync(0xffffffffu, w, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2); w += __shfl_xor_sync(0xffffffffu, w, 2);
+        v = __shfl_sync(0xffffffffu, v, src); w = __shfl_sync(0xffffffffu, w, src);
+        if (b == myb) { mv = v; ma = w; }
+      }
+      st.acc[0][0] = st.acc[0][0] + T(mv); st.aab[0][0] += ma; st.has_part = 0;
+    }
+  }
+#endif
+}
+
 // All groups of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
 // ABS: 0 no |.| tracking, 1 bound by cabs (needs |A|,|A^q| <= 1), 2 exact sum of |coef| prod |A| in double
 template <class T, int S, int ABS, class Flush>
@@ -523,6 +548,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
     const FgGroupHdr gh = *(const FgGroupHdr*)p; p += sizeof(FgGroupHdr);
     const int nrec = gh.nrec, nf = gh.nf, k = gh.k, flags = gh.flags;
     if ((int)gh.dst != st.cur) {
+      fold_mma_partials(st);
       if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
       st.cur = gh.dst;
 #pragma unroll
@@ -550,30 +576,17 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
     if (flags & FG_REC_MMA) {
 #if defined(__CUDA_ARCH__)
       if constexpr (!is_dd<T>::value && ABS == 1 && S == 1) {
-        double part[8]; done = true;
+        done = true;
+        if (!st.has_part) { st.has_part = 1; for (int b = 0; b < 8; ++b) st.part[b] = 0.0; }
         const double* Vw = (const double*)Vt - (threadIdx.x & 31);
         const unsigned v4 = (unsigned)gh.vidx[0] | ((unsigned)gh.vidx[1] << 8) | ((unsigned)gh.vidx[2] << 16) | ((unsigned)gh.vidx[3] << 24);
         const bool qx = (flags & FG_REC_QEXT) != 0;
         switch (nf * 8 + k) {
-#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p, nrec, Vw, vs, ne, v4, part); else run_group_mma_fast<NF, K, false>(p, nrec, Vw, vs, ne, v4, part); break;
+#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p, nrec, Vw, vs, ne, v4, st.part); else run_group_mma_fast<NF, K, false>(p, nrec, Vw, vs, ne, v4, st.part); break;
           FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
           FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
 #undef FG_MM
           default: done = false; break;
-        }
-        if (done) {
-          // quad-reduce the partials, then hand every thread the sums of its own sample (lane L <- lane 4*(L%8), row block L/8)
-          const int lane = threadIdx.x & 31, src = (lane & 7) << 2, myb = lane >> 3;
-          double mv = 0.0, ma = 0.0;
-#pragma unroll
-          for (int b = 0; b < 4; ++b) {
-            double v = part[b], w = part[4 + b];
-            v += __shfl_xor_sync(0xffffffffu, v, 1); w += __shfl_xor_sync(0xffffffffu, w, 1);
-            v += __shfl_xor_sync(0xffffffffu, v, 2); w += __shfl_xor_sync(0xffffffffu, w, 2);
-            v = __shfl_sync(0xffffffffu, v, src); w = __shfl_sync(0xffffffffu, w, src);
-            if (b == myb) { mv = v; ma = w; }
-          }
-          st.acc[0][0] = st.acc[0][0] + T(mv); st.aab[0][0] += ma;
         }
       }
 #endif

@@ -65,7 +65,7 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     mbar_expect_tx(&ring.bar[0], FG_CHUNK_BYTES); bulk_g2s(ring.buf, g0, FG_CHUNK_BYTES, &ring.bar[0]);
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], FG_CHUNK_BYTES); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[1]); }
   }
-  RecState<T, S> st; st.cur = -1;
+  RecState<T, S> st; st.cur = -1; st.has_part = 0;
   const int nc = N.ncomp, rawv = sm.rawv, rawa = sm.rawa;
   auto flush = [&](int dst, const T (*acc)[S], const double (*aab)[S]) {
     for (int c = 0; c < nc; ++c) {
@@ -80,6 +80,7 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     __syncthreads();   // every thread is done with buffer b
     if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], FG_CHUNK_BYTES); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[b]); }
   }
+  fold_mma_partials(st);
   if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
 }
 
