@@ -457,9 +457,9 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
   constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int v0 = (int)(vidx4 & 255u) * vs, v1 = (int)((vidx4 >> 8) & 255u) * vs, v2 = (int)((vidx4 >> 16) & 255u) * vs, v3 = (int)(vidx4 >> 24) * vs, vq = ne * vs;
-  double acc[4], aab[4];
+  double acc[4], aab[4], pf[4][NF > 0 ? NF : 1];
 #pragma unroll
-  for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; }
+  for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[b][i] = 1.0; }
   for (int t = 0; t < ntiles; ++t, p += TILE) {
     const uint4 h0 = *(const uint4*)(p + (2 * c) * 16), h1 = *(const uint4*)(p + (2 * c + 1) * 16);
     double B[STEPS];
@@ -467,6 +467,7 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
     for (int st = 0; st < STEPS; ++st) B[st] = ((const double*)(p + 8 * sizeof(FgRecM)))[st * 32 + lane];
     const double cab0 = (double)__uint_as_float(h0.w), cab1 = (double)__uint_as_float(h1.w);
     int f0[NF > 0 ? NF : 1], f1[NF > 0 ? NF : 1];
+    const int keep0 = (int)((h0.y >> 8) & 255u), keep1 = (int)((h1.y >> 8) & 255u);
 #pragma unroll
     for (int i = 0; i < NF; ++i) {
       f0[i] = (int)((i < 4 ? (h0.x >> (8 * i)) : h0.y) & 255u) * vs;
@@ -500,9 +501,16 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
           dmma884(d0, d1, m3, B[2 * NM + 2]); dmma884(d0, d1, m3 * a2, B[2 * NM + 3]);
         }
       }
+      // products of beta's of this lane's two records; the prefix stack of the row block survives from record to record
       double bp0 = 1.0, bp1 = 1.0;
+      if (NF > 0) {
 #pragma unroll
-      for (int i = 0; i < NF; ++i) { bp0 = (i == 0) ? Vs[f0[i]] : bp0 * Vs[f0[i]]; bp1 = (i == 0) ? Vs[f1[i]] : bp1 * Vs[f1[i]]; }
+        for (int i = 0; i < NF; ++i) if (i >= keep0) pf[b][i] = (i == 0) ? Vs[f0[i]] : pf[b][i > 0 ? i - 1 : 0] * Vs[f0[i]];
+        bp0 = pf[b][NF > 0 ? NF - 1 : 0];
+#pragma unroll
+        for (int i = 0; i < NF; ++i) if (i >= keep1) pf[b][i] = (i == 0) ? Vs[f1[i]] : pf[b][i > 0 ? i - 1 : 0] * Vs[f1[i]];
+        bp1 = pf[b][NF > 0 ? NF - 1 : 0];
+      }
       acc[b] = fma(bp0, d0, acc[b]); acc[b] = fma(bp1, d1, acc[b]);
       aab[b] = fma(fabs(bp0), cab0, aab[b]); aab[b] = fma(fabs(bp1), cab1, aab[b]);
     }

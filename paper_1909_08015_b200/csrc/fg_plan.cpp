@@ -576,20 +576,30 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       const bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= 2 && (j - i) >= FG_MMA_MINREC;
       if (mma) {
         const int steps = mma_steps(r0.k, qx); const size_t tile_bytes = 8 * sizeof(FgRecM) + (size_t)steps * 32 * sizeof(double);
-        for (size_t t0 = i; t0 < j; t0 += 8) {
+        const int R = (int)(j - i), ntiles = (R + 7) / 8;
+        // record shown to lane c (of every quad) in tile t, slot e: depth-first index c*2*ntiles + 2t + e
+        auto rec_at = [&](int t, int n) -> const HRecord* { int d = (n >> 1) * 2 * ntiles + 2 * t + (n & 1); return d < R ? &N.recs[i + d] : nullptr; };
+        for (int t = 0; t < ntiles; ++t) {
           bool need_group = !gopen || prev != nullptr;      // prev != nullptr: a regular group is open
           if (!open || cur + tile_bytes + (need_group ? sizeof(FgGroupHdr) : 0) > FG_CHUNK_BYTES) { new_chunk(); need_group = true; }
           if (need_group) open_group(r0, FG_REC_MMA);
           for (int n = 0; n < 8; ++n) {
-            FgRecM h; std::memset(&h, 0, sizeof(h));
-            if (t0 + n < j) { const HRecord& r = N.recs[t0 + n]; std::memcpy(h.fidx, r.fidx, FG_NFC); h.cabs = std::max(r.cabs[0], r.cabs[1]); }
+            FgRecM h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)r0.nf;
+            if (const HRecord* r = rec_at(t, n)) {
+              std::memcpy(h.fidx, r->fidx, FG_NFC); h.cabs = std::max(r->cabs[0], r->cabs[1]);
+              const HRecord* pr = (n & 1) ? rec_at(t, n - 1) : (t > 0 && gn > 0 ? rec_at(t - 1, n + 1) : nullptr);   // gn == 0: first tile of a (re)opened group
+              int keep = 0; if (pr) while (keep < r->nf && r->fidx[keep] == pr->fidx[keep]) ++keep;
+              h.keep = (uint8_t)keep;
+              N.exec_flops += std::max(0, r->nf - std::max(keep, 1));
+            }
             std::memcpy(&P.d_chunks[base + cur + n * sizeof(FgRecM)], &h, sizeof(h));
           }
           double* fr = (double*)&P.d_chunks[base + cur + 8 * sizeof(FgRecM)];
-          for (int st = 0; st < steps; ++st) for (int n = 0; n < 8; ++n) for (int x = 0; x < 4; ++x)
-            fr[st * 32 + n * 4 + x] = (t0 + n < j) ? mma_coef(N.recs[t0 + n], st, x) : 0.0;
+          for (int st = 0; st < steps; ++st) for (int n = 0; n < 8; ++n) for (int x = 0; x < 4; ++x) {
+            const HRecord* r = rec_at(t, n); fr[st * 32 + n * 4 + x] = r ? mma_coef(*r, st, x) : 0.0;
+          }
           cur += tile_bytes; ++gn;
-          N.exec_flops += 8.0 * (8.0 * steps + 2.0 * std::max(0, r0.nf - 1) + 4.0);
+          N.exec_flops += 8.0 * (8.0 * steps + 4.0);
         }
         for (size_t t = i; t < j; ++t) N.algo_flops += std::max(0, N.recs[t].nf - 1);
         close_group();

@@ -86,8 +86,11 @@ static_assert(sizeof(FgRecC) == 16 && sizeof(FgRecW) == 32, "record header sizes
 //   low-q steps (q-extension):      {aq0, aq0 a1, aq1, aq1 a0}[x] * mhi[t]
 //   high-q steps, j = 2..k-1:       aq_j * mlo[x] * (product over the subset t' of the other high variables)
 // A tile = 8 x FgRecM (product factors, cabs) + steps x 32 doubles in B-fragment order (lane = 4*record + x).
+// Lane c of a quad weights records 2c, 2c+1 of every tile; the planner deals the records of a run out so that these form
+// one contiguous stretch of the depth-first matching order, and keep = leading product factors shared with the lane's
+// previous record (prefix products stay in registers).
 // The group header carries the free variables (vidx) and nrec = number of tiles.
-struct alignas(16) FgRecM { uint8_t fidx[FG_NFC]; uint8_t pad[7]; float cabs; };
+struct alignas(16) FgRecM { uint8_t fidx[FG_NFC]; uint8_t keep; uint8_t pad[6]; float cabs; };
 struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint8_t pad[6]; };
 static_assert(sizeof(FgRecM) == 16 && sizeof(FgGroupHdr) == 16, "group header sizes");
 struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
