@@ -452,14 +452,20 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 template <int NF, int K, bool QX>
-__device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict__ p, int ntiles, const double* __restrict__ Vw, int vs, int ne, unsigned vidx4, double* __restrict__ out) {
+__device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int vs, int ne, double* __restrict__ out) {
   __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
   constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
-  const int v0 = (int)(vidx4 & 255u) * vs, v1 = (int)((vidx4 >> 8) & 255u) * vs, v2 = (int)((vidx4 >> 16) & 255u) * vs, v3 = (int)(vidx4 >> 24) * vs, vq = ne * vs;
+  const int vq = ne * vs;
   double acc[4], aab[4], pf[4][NF > 0 ? NF : 1];
 #pragma unroll
-  for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[b][i] = 1.0; }
+  for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; }
+  for (int g = 0; g < nseq; ++g) {       // consecutive groups of this class (same destination), each with its own free variables
+  const uint4 gw = *(const uint4*)p; p += sizeof(FgGroupHdr);
+  const int ntiles = (int)(gw.x & 0xffffu);
+  const int v0 = (int)((gw.y >> 16) & 255u) * vs, v1 = (int)(gw.y >> 24) * vs, v2 = (int)(gw.z & 255u) * vs, v3 = (int)((gw.z >> 8) & 255u) * vs;
+#pragma unroll
+  for (int b = 0; b < 4; ++b) for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[b][i] = 1.0;
   for (int t = 0; t < ntiles; ++t, p += TILE) {
     const uint4 h0 = *(const uint4*)(p + (2 * c) * 16), h1 = *(const uint4*)(p + (2 * c + 1) * 16);
     double B[STEPS];
@@ -514,6 +520,7 @@ __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict_
       acc[b] = fma(bp0, d0, acc[b]); acc[b] = fma(bp1, d1, acc[b]);
       aab[b] = fma(fabs(bp0), cab0, aab[b]); aab[b] = fma(fabs(bp1), cab1, aab[b]);
     }
+  }
   }
 #pragma unroll
   for (int b = 0; b < 4; ++b) { out[b] = acc[b]; out[4 + b] = aab[b]; }
@@ -587,15 +594,23 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
         done = true;
         if (!st.has_part) { st.has_part = 1; for (int b = 0; b < 8; ++b) st.part[b] = 0.0; }
         const double* Vw = (const double*)Vt - (threadIdx.x & 31);
-        const unsigned v4 = (unsigned)gh.vidx[0] | ((unsigned)gh.vidx[1] << 8) | ((unsigned)gh.vidx[2] << 16) | ((unsigned)gh.vidx[3] << 24);
         const bool qx = (flags & FG_REC_QEXT) != 0;
+        const int tile_bytes = 8 * (int)sizeof(FgRecM) + mma_steps(k, qx) * 32 * (int)sizeof(double);
+        // consecutive tensor-core groups of the same class and destination are run by one call
+        const unsigned char* p0 = p - sizeof(FgGroupHdr); const unsigned char* pe = p + nrec * tile_bytes; int nseq = 1;
+        while (g + nseq < ngroups) {
+          const FgGroupHdr nx = *(const FgGroupHdr*)pe;
+          if (nx.nf != gh.nf || nx.k != gh.k || nx.flags != gh.flags || nx.dst != gh.dst) break;
+          pe += sizeof(FgGroupHdr) + (int)nx.nrec * tile_bytes; ++nseq;
+        }
         switch (nf * 8 + k) {
-#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p, nrec, Vw, vs, ne, v4, st.part); else run_group_mma_fast<NF, K, false>(p, nrec, Vw, vs, ne, v4, st.part); break;
+#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p0, nseq, Vw, vs, ne, st.part); else run_group_mma_fast<NF, K, false>(p0, nseq, Vw, vs, ne, st.part); break;
           FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
           FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
 #undef FG_MM
           default: done = false; break;
         }
+        if (done) { p = pe; g += nseq - 1; continue; }
       }
 #endif
       if (!done) run_group_mma_dyn<T, S, ABS>(p, nrec, nf, k, flags, gh.vidx, Vt, vs, ne, st);

@@ -61,9 +61,10 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
   const int nch = N.chunk_count;
   if (nch == 0) return;
   const unsigned char* g0 = P.chunks + (size_t)N.chunk_begin * FG_CHUNK_BYTES;
+  const uint32_t* used = P.chunk_used + N.chunk_begin;
   if (threadIdx.x == 0) {
-    mbar_expect_tx(&ring.bar[0], FG_CHUNK_BYTES); bulk_g2s(ring.buf, g0, FG_CHUNK_BYTES, &ring.bar[0]);
-    if (nch > 1) { mbar_expect_tx(&ring.bar[1], FG_CHUNK_BYTES); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[1]); }
+    mbar_expect_tx(&ring.bar[0], used[0]); bulk_g2s(ring.buf, g0, used[0], &ring.bar[0]);
+    if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
   }
   RecState<T, S> st; st.cur = -1; st.has_part = 0;
   const int nc = N.ncomp, rawv = sm.rawv, rawa = sm.rawa;
@@ -78,7 +79,7 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     mbar_wait(&ring.bar[b], ring.phase[b]); ring.phase[b] ^= 1u;
     run_chunk<T, S, ABS>(ring.buf + b * FG_CHUNK_BYTES, Vt, vs, ne, st, flush);
     __syncthreads();   // every thread is done with buffer b
-    if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], FG_CHUNK_BYTES); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, FG_CHUNK_BYTES, &ring.bar[b]); }
+    if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], used[ch + 2]); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, used[ch + 2], &ring.bar[b]); }
   }
   fold_mma_partials(st);
   if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
@@ -352,7 +353,7 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   D.quarter_pow = std::pow(-0.25, H.g.n); D.fact[0] = 1; for (int k = 1; k < FG_NDEG; ++k) D.fact[k] = D.fact[k - 1] * k;
 #define UP(vec, field) do { int rc_ = upload(p, vec, &D.field); if (rc_ != FG_OK) { fg_plan_destroy(p); return rc_; } } while (0)
   UP(H.d_geoms, geoms); UP(H.d_nums, nums); UP(H.d_nodes, nodes); UP(H.d_terms, terms); UP(H.d_geom_num_begin, geom_num_begin);
-  UP(H.d_chunks, chunks); UP(H.Z1, Z1); UP(H.Z3, Z3);
+  UP(H.d_chunks, chunks); UP(H.d_chunk_used, chunk_used); UP(H.Z1, Z1); UP(H.Z3, Z3);
 #undef UP
   int vmax = 1; for (auto& E : H.geoms) vmax = std::max(vmax, E.ne * (E.ne + 1) / 2 + 2 * E.ne);
   p->vmax = vmax;

@@ -551,7 +551,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     size_t cur = 0, base = 0, ghdr = 0; bool open = false, gopen = false; int ngroups = 0, gn = 0; const HRecord* prev = nullptr;
     auto cls = [](const HRecord& r) { int fl = r.flags & (FG_REC_TWO | FG_REC_QEXT); if (r.nf > FG_NFC) fl |= FG_REC_WIDE; return (r.dst << 16) | (r.nf << 12) | (r.k << 8) | fl; };
     auto close_group = [&]() { if (gopen) { FgGroupHdr g; std::memcpy(&g, &P.d_chunks[ghdr], sizeof(g)); g.nrec = (uint16_t)gn; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); gopen = false; } };
-    auto close_chunk = [&]() { close_group(); if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.ngroups = ngroups; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; } };
+    auto close_chunk = [&]() { close_group(); if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.ngroups = ngroups; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; P.d_chunk_used.push_back((uint32_t)((cur + 15) & ~(size_t)15)); } };
     auto new_chunk = [&]() { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); ngroups = 0; open = true; };
     auto open_group = [&](const HRecord& r, int extra_flags) {
       close_group();

@@ -71,7 +71,7 @@ struct HostPlan {
   std::vector<double> deg, Z1, Z3; double lnZfull[4];
   // flattened
   std::vector<FgGeomDev> d_geoms; std::vector<FgNumDev> d_nums; std::vector<FgNodeDev> d_nodes;
-  std::vector<FgTermDev> d_terms; std::vector<int32_t> d_geom_num_begin; std::vector<unsigned char> d_chunks;
+  std::vector<FgTermDev> d_terms; std::vector<int32_t> d_geom_num_begin; std::vector<unsigned char> d_chunks; std::vector<uint32_t> d_chunk_used;
   int raw_slots = 0, scratch_slots = 0;
   long n_records = 0, n_coefs = 0, n_nonzero = 0;
   double algo_flops = 0, exec_flops = 0, plan_seconds = 0;

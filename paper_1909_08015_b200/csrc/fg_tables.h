@@ -10,7 +10,7 @@
 #define FG_NDEG 6          // polynomial in t: degrees 0..5
 #define FG_KMAX 4          // free variables of one numerator record (dense 2^k table); further ones are enumerated
 #define FG_MAXF 10         // product factors of one record
-#define FG_CHUNK_BYTES 8192   // numerator stream is cut into chunks of this size (records never straddle)
+#define FG_CHUNK_BYTES 16384  // numerator stream is cut into chunks of this size (records and tiles never straddle)
 #define FG_MAXSE 4         // self-energy children of one element
 #define FG_MAXVC 5         // vertexlike children of one element
 #define FG_MAXMEM 8        // members of one forest
@@ -107,6 +107,7 @@ struct FgPlanDev {
   const FgTermDev* terms;
   const int32_t* geom_num_begin;      // nums are sorted by geometry: nums of geom g are [begin[g], begin[g+1])
   const unsigned char* chunks;        // nchunk * FG_CHUNK_BYTES
+  const uint32_t* chunk_used;         // bytes in use of every chunk (multiple of 16): what the TMA copy moves
   // density
   const double* Z1;                   // 2^M
   const double* Z3;                   // 2^M
