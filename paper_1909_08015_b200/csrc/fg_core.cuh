@@ -451,76 +451,105 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
+// NT2 (1 or 2) consecutive tiles share the monomials (A fragments) of a row block: the loads of a, a^q and the monomial
+// products are paid once per 8 or 16 records.
+template <int NF, int K, bool QX, int NT2>
+__device__ __forceinline__ void mma_tiles(const unsigned char* __restrict__ p, const double* __restrict__ Vw, int vs, int lane, int r, int c,
+                                          int v0, int v1, int v2, int v3, int vq, double* acc, double* aab, double (*pf)[NF > 0 ? NF : 1]) {
+  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
+  double B[NT2][STEPS], cab[NT2][2]; int ff[NT2][2][NF > 0 ? NF : 1], keep[NT2][2];
+#pragma unroll
+  for (int u = 0; u < NT2; ++u) {
+    const unsigned char* pt = p + u * TILE;
+#pragma unroll
+    for (int st = 0; st < STEPS; ++st) B[u][st] = ((const double*)(pt + 8 * sizeof(FgRecM)))[st * 32 + lane];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const uint4 h = *(const uint4*)(pt + (2 * c + e) * 16);
+      cab[u][e] = (double)__uint_as_float(h.w); keep[u][e] = (int)((h.y >> 8) & 255u);
+#pragma unroll
+      for (int i = 0; i < NF; ++i) ff[u][e][i] = (int)((i < 4 ? (h.x >> (8 * i)) : h.y) & 255u) * vs;
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < 4; ++b) {
+    const double* __restrict__ Vs = Vw + 8 * b + r;
+    const double a0 = Vs[v0], a1 = Vs[v1];
+    const double a2 = K > 2 ? Vs[v2] : 1.0, a3 = K > 3 ? Vs[v3] : 1.0;
+    const double a01 = a0 * a1;
+    const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
+    double hi[NM]; hi[0] = 1.0;
+    if (K > 2) hi[1] = a2;
+    if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
+    double d[NT2][2];
+#pragma unroll
+    for (int u = 0; u < NT2; ++u) { d[u][0] = 0.0; d[u][1] = 0.0; dmma884(d[u][0], d[u][1], mlo, B[u][0]); }
+#pragma unroll
+    for (int tt = 1; tt < NM; ++tt) {
+      const double m = mlo * hi[tt];
+#pragma unroll
+      for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], m, B[u][tt]);
+    }
+    if (QX) {
+      const double q0 = Vs[v0 + vq], q1 = Vs[v1 + vq];
+      const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
+#pragma unroll
+      for (int tt = 0; tt < NM; ++tt) {
+        const double m = tt ? mq * hi[tt] : mq;
+#pragma unroll
+        for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], m, B[u][NM + tt]);
+      }
+      if (K == 3) {
+        const double m = mlo * Vs[v2 + vq];
+#pragma unroll
+        for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], m, B[u][2 * NM]);
+      }
+      if (K == 4) {
+        const double m2 = mlo * Vs[v2 + vq], m3 = mlo * Vs[v3 + vq];
+        const double mm[4] = {m2, m2 * a3, m3, m3 * a2};
+#pragma unroll
+        for (int tt = 0; tt < 4; ++tt) {
+#pragma unroll
+          for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], mm[tt], B[u][2 * NM + tt]);
+        }
+      }
+    }
+    // products of beta's of this lane's records (tile by tile, slot by slot: the lane's depth-first stretch); the prefix
+    // stack of the row block survives from record to record
+#pragma unroll
+    for (int u = 0; u < NT2; ++u) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        double bp = 1.0;
+        if (NF > 0) {
+#pragma unroll
+          for (int i = 0; i < NF; ++i) if (i >= keep[u][e]) pf[b][i] = (i == 0) ? Vs[ff[u][e][i]] : pf[b][i > 0 ? i - 1 : 0] * Vs[ff[u][e][i]];
+          bp = pf[b][NF > 0 ? NF - 1 : 0];
+        }
+        acc[b] = fma(bp, d[u][e], acc[b]); aab[b] = fma(fabs(bp), cab[u][e], aab[b]);
+      }
+    }
+  }
+}
+
 template <int NF, int K, bool QX>
 __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int vs, int ne, double* __restrict__ out) {
   __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
-  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
+  constexpr int STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int vq = ne * vs;
   double acc[4], aab[4], pf[4][NF > 0 ? NF : 1];
 #pragma unroll
   for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; }
   for (int g = 0; g < nseq; ++g) {       // consecutive groups of this class (same destination), each with its own free variables
-  const uint4 gw = *(const uint4*)p; p += sizeof(FgGroupHdr);
-  const int ntiles = (int)(gw.x & 0xffffu);
-  const int v0 = (int)((gw.y >> 16) & 255u) * vs, v1 = (int)(gw.y >> 24) * vs, v2 = (int)(gw.z & 255u) * vs, v3 = (int)((gw.z >> 8) & 255u) * vs;
+    const uint4 gw = *(const uint4*)p; p += sizeof(FgGroupHdr);
+    const int ntiles = (int)(gw.x & 0xffffu);
+    const int v0 = (int)((gw.y >> 16) & 255u) * vs, v1 = (int)(gw.y >> 24) * vs, v2 = (int)(gw.z & 255u) * vs, v3 = (int)((gw.z >> 8) & 255u) * vs;
 #pragma unroll
-  for (int b = 0; b < 4; ++b) for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[b][i] = 1.0;
-  for (int t = 0; t < ntiles; ++t, p += TILE) {
-    const uint4 h0 = *(const uint4*)(p + (2 * c) * 16), h1 = *(const uint4*)(p + (2 * c + 1) * 16);
-    double B[STEPS];
-#pragma unroll
-    for (int st = 0; st < STEPS; ++st) B[st] = ((const double*)(p + 8 * sizeof(FgRecM)))[st * 32 + lane];
-    const double cab0 = (double)__uint_as_float(h0.w), cab1 = (double)__uint_as_float(h1.w);
-    int f0[NF > 0 ? NF : 1], f1[NF > 0 ? NF : 1];
-    const int keep0 = (int)((h0.y >> 8) & 255u), keep1 = (int)((h1.y >> 8) & 255u);
-#pragma unroll
-    for (int i = 0; i < NF; ++i) {
-      f0[i] = (int)((i < 4 ? (h0.x >> (8 * i)) : h0.y) & 255u) * vs;
-      f1[i] = (int)((i < 4 ? (h1.x >> (8 * i)) : h1.y) & 255u) * vs;
-    }
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      const double* __restrict__ Vs = Vw + 8 * b + r;
-      const double a0 = Vs[v0], a1 = Vs[v1];
-      const double a2 = K > 2 ? Vs[v2] : 1.0, a3 = K > 3 ? Vs[v3] : 1.0;
-      const double a01 = a0 * a1;
-      const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
-      double hi[NM]; hi[0] = 1.0;
-      if (K > 2) hi[1] = a2;
-      if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
-      double d0 = 0.0, d1 = 0.0;
-      dmma884(d0, d1, mlo, B[0]);
-#pragma unroll
-      for (int tt = 1; tt < NM; ++tt) dmma884(d0, d1, mlo * hi[tt], B[tt]);
-      if (QX) {
-        const double q0 = Vs[v0 + vq], q1 = Vs[v1 + vq];
-        const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
-        dmma884(d0, d1, mq, B[NM]);
-#pragma unroll
-        for (int tt = 1; tt < NM; ++tt) dmma884(d0, d1, mq * hi[tt], B[NM + tt]);
-        if (K == 3) { const double q2 = Vs[v2 + vq]; dmma884(d0, d1, mlo * q2, B[2 * NM]); }
-        if (K == 4) {
-          const double q2 = Vs[v2 + vq], q3 = Vs[v3 + vq];
-          const double m2 = mlo * q2, m3 = mlo * q3;
-          dmma884(d0, d1, m2, B[2 * NM]); dmma884(d0, d1, m2 * a3, B[2 * NM + 1]);
-          dmma884(d0, d1, m3, B[2 * NM + 2]); dmma884(d0, d1, m3 * a2, B[2 * NM + 3]);
-        }
-      }
-      // products of beta's of this lane's two records; the prefix stack of the row block survives from record to record
-      double bp0 = 1.0, bp1 = 1.0;
-      if (NF > 0) {
-#pragma unroll
-        for (int i = 0; i < NF; ++i) if (i >= keep0) pf[b][i] = (i == 0) ? Vs[f0[i]] : pf[b][i > 0 ? i - 1 : 0] * Vs[f0[i]];
-        bp0 = pf[b][NF > 0 ? NF - 1 : 0];
-#pragma unroll
-        for (int i = 0; i < NF; ++i) if (i >= keep1) pf[b][i] = (i == 0) ? Vs[f1[i]] : pf[b][i > 0 ? i - 1 : 0] * Vs[f1[i]];
-        bp1 = pf[b][NF > 0 ? NF - 1 : 0];
-      }
-      acc[b] = fma(bp0, d0, acc[b]); acc[b] = fma(bp1, d1, acc[b]);
-      aab[b] = fma(fabs(bp0), cab0, aab[b]); aab[b] = fma(fabs(bp1), cab1, aab[b]);
-    }
-  }
+    for (int b = 0; b < 4; ++b) for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[b][i] = 1.0;
+    int t = 0;
+    for (; t + 2 <= ntiles; t += 2, p += 2 * TILE) mma_tiles<NF, K, QX, 2>(p, Vw, vs, lane, r, c, v0, v1, v2, v3, vq, acc, aab, pf);
+    if (t < ntiles) { mma_tiles<NF, K, QX, 1>(p, Vw, vs, lane, r, c, v0, v1, v2, v3, vq, acc, aab, pf); p += TILE; }
   }
 #pragma unroll
   for (int b = 0; b < 4; ++b) { out[b] = acc[b]; out[4 + b] = aab[b]; }
