@@ -31,10 +31,10 @@ UNIT = "samples/s"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--graphs", type=int, default=2, help="how many graphs of the 32-graph config-5 batch to time")
-    ap.add_argument("--samples", type=int, default=1 << 20, help="samples per graph per step")
+    ap.add_argument("--samples", type=int, default=1 << 24, help="samples per graph per step (one slab of the integrator)")
     ap.add_argument("--impl", default="fg", choices=["fg", "reference"])
     ap.add_argument("--rel-tol", type=float, default=0.0)
     ap.add_argument("--target-samples", type=float, default=1e10, help="run length the acceptance tolerance is set for")
@@ -202,6 +202,12 @@ def main_fg(args):
     algo = sum(p.stats["flops_per_sample"] for p in plans) * S * args.steps
     execf = sum(p.stats["exec_flops_per_sample"] for p in plans) * S * args.steps
     ach = algo / (ms_d * 1e-3) / 1e12
+    traffic = None      # DRAM bytes per launch, scaled per sample from the committed ncu capture (profiles/r01_traffic.json)
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))
+        traffic = (tj["dram_bytes_read"] + tj["dram_bytes_write"]) / tj["samples"] * S
+    except Exception:
+        pass
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
@@ -211,8 +217,8 @@ def main_fg(args):
                        "graphs": info, "flagged_fraction": flagged / max(1.0, total / world), "rejected": rejected,
                        "kernel_ms": {"double_pass": ms_d, "dd_pass": ms_q, "share_double": ms_d / max(ms_d + ms_q, 1e-9)},
                        "exec_tflops_double_pass": execf / (ms_d * 1e-3) / 1e12},
-            "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": None,
-                         "kernel": "fg_eval_kernel<double,2,128>", "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": traffic,
+                         "kernel": "fg_eval_kernel<double,1,256>", "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
                          "frac_executed": execf / (ms_d * 1e-3) / 1e12 / peak_tf},
             "e2e": {"value": total / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 80 * len(plans)},
             "gpu_launches": launches, "clocks": clk}
