@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
   const int tid = threadIdx.x;
   if (tid == 0) { mbar_init(&ring.bar[0], 1); mbar_init(&ring.bar[1], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
   __syncthreads();
-  const int vs = NT * S, ss = NT * S;
+  const int vs = NT * S + FG_VPAD, ss = NT * S;   // padded row stride of V: rows of different parity fall into different banks
   T* Vt = Vsm + tid * S;
   T* Sc = (T*)A.scratch + (size_t)blockIdx.x * (size_t)P.scratch_slots * ss + tid * S;
   const uint64_t nwork = A.idlist ? (uint64_t)*A.idcount : A.n;
@@ -360,11 +360,11 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   // threads per block: as many warps as the per-sample operand table V (vmax entries) leaves room for in shared memory
   int smem_max = 0; cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
   const size_t ring_bytes = 2 * FG_CHUNK_BYTES + 128;
-  auto fit = [&](int maxnt, size_t per_thread) { long nt = ((long)smem_max - (long)ring_bytes) / (long)per_thread; nt = std::min<long>(maxnt, nt / 32 * 32); return (int)nt; };
+  auto fit = [&](int maxnt, size_t per_thread) { long nt = ((long)smem_max - (long)ring_bytes) / (long)per_thread - FG_VPAD; nt = std::min<long>(maxnt, nt / 32 * 32); return (int)nt; };
   p->nt_d = fit(NT_D, (size_t)vmax * S_D * sizeof(double)); p->nt_q = fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd));
   if (p->nt_d < 32 || p->nt_q < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
-  p->smem_d = ring_bytes + (size_t)vmax * p->nt_d * S_D * sizeof(double);
-  p->smem_q = ring_bytes + (size_t)vmax * p->nt_q * S_Q * sizeof(dd);
+  p->smem_d = ring_bytes + (size_t)vmax * (p->nt_d * S_D + FG_VPAD) * sizeof(double);
+  p->smem_q = ring_bytes + (size_t)vmax * (p->nt_q * S_Q + FG_VPAD) * sizeof(dd);
   // the attribute is per function, not per plan: always raise it to the device limit
   auto setattr = [&](const void* f) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max); };
   e = setattr((const void*)fg_eval_kernel<double, S_D, NT_D>); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>);

@@ -11,6 +11,7 @@
 #define FG_KMAX 4          // free variables of one numerator record (dense 2^k table); further ones are enumerated
 #define FG_MAXF 10         // product factors of one record
 #define FG_CHUNK_BYTES 32768  // numerator stream is cut into chunks of this size (records and tiles never straddle)
+#define FG_VPAD 8          // padding (elements) of the row stride of the per-sample operand table V in shared memory
 #define FG_MAXSE 4         // self-energy children of one element
 #define FG_MAXVC 5         // vertexlike children of one element
 #define FG_MAXMEM 8        // members of one forest
