@@ -93,6 +93,12 @@ typedef struct {
 } fg_plan_stats;
 int fg_plan_info(const fg_plan*, fg_plan_stats* out);
 
+/* Host-only planning (no device, no kernels): runs the whole planner and returns its statistics (table_bytes = 0),
+ * the structure dump described below (subs: up to subs_cap rows of 4 ints; returns the ints written to `terms`) and
+ * the Deg / Z_1 tables (2^M doubles each).  Any output pointer may be NULL.  For CPU tests of the host logic. */
+int fg_host_plan(const fg_graph*, const fg_plan_opts*, fg_plan_stats* stats, int32_t* subs, int32_t subs_cap,
+                 int32_t* terms, int32_t terms_cap, double* deg, double* Z1);
+
 /* Structure dump for tests (expression (11)).
  *  subs: n_subgraphs rows (a, b, type 0 = self-energy / 1 = vertexlike, in_chain)
  *  terms: flat ints: sign, index of G', n_members, then (sub index, op) pairs, op 0=A 1=U 2=L 3=L-U.

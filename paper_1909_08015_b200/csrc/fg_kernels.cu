@@ -417,6 +417,41 @@ int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
   return FG_OK;
 }
 
+static void fill_stats(const HostPlan& H, fg_plan_stats* s) {
+  std::memset(s, 0, sizeof(*s));
+  s->n_loops = H.g.n; s->M = H.M; s->n_subgraphs = (int)H.subs.size(); s->n_forests = (int)H.forests.size(); s->n_terms = (int)H.terms.size();
+  s->n_geoms = (int)H.geoms.size(); s->n_nums = (int)H.nums.size(); s->n_nodes = (int)H.nodes.size();
+  s->n_records = H.n_records; s->n_coefs = H.n_coefs; s->n_coefs_nonzero = H.n_nonzero;
+  s->stream_bytes = (int64_t)H.d_chunks.size();
+  s->flops_per_sample = H.algo_flops; s->exec_flops_per_sample = H.exec_flops; s->plan_seconds = H.plan_seconds;
+}
+static int dump_structure(const HostPlan& H, int32_t* subs, int32_t* terms, int32_t cap) {
+  if (subs) for (size_t k = 0; k < H.subs.size(); ++k) { subs[4 * k] = H.subs[k].a; subs[4 * k + 1] = H.subs[k].b; subs[4 * k + 2] = H.subs[k].type; subs[4 * k + 3] = H.subs[k].chain; }
+  int w = 0;
+  if (terms) for (auto& t : H.terms) {
+    if (w + 3 + 2 * (int)t.members.size() > cap) return fail(FG_E_LIMIT, "terms buffer too small");
+    terms[w++] = t.sign; terms[w++] = t.gprime; terms[w++] = (int)t.members.size();
+    for (size_t k = 0; k < t.members.size(); ++k) { terms[w++] = t.members[k]; terms[w++] = t.ops[k]; }
+  }
+  return w;
+}
+
+int fg_host_plan(const fg_graph* g, const fg_plan_opts* opts, fg_plan_stats* stats, int32_t* subs, int32_t subs_cap, int32_t* terms, int32_t terms_cap, double* deg, double* Z1) {
+  if (!g) return fail(FG_E_ARG, "graph is NULL");
+  fg_plan_opts o; if (opts) o = *opts; else fg_plan_opts_default(&o);
+  PlanOpts po; for (int k = 0; k < 4; ++k) po.C[k] = o.C[k]; po.D = o.D; po.merge = o.merge_ext_lines ? 1 : 0;
+  int M = 3 * g->g.n - (po.merge ? 1 : 0);
+  if (o.deg_table) po.deg_override.assign(o.deg_table, o.deg_table + ((size_t)1 << M));
+  HostPlan H; std::string msg;
+  int rc = build_plan(g->g, po, H, msg);
+  if (rc != FG_OK) return fail(rc, msg);
+  if (stats) fill_stats(H, stats);
+  if (subs && (int)H.subs.size() > subs_cap) return fail(FG_E_LIMIT, "subs buffer too small");
+  if (deg) std::memcpy(deg, H.deg.data(), H.deg.size() * sizeof(double));
+  if (Z1) std::memcpy(Z1, H.Z1.data(), H.Z1.size() * sizeof(double));
+  return dump_structure(H, subs, terms, terms_cap);
+}
+
 int fg_plan_structure(const fg_plan* p, int32_t* subs, int32_t* terms, int32_t cap) {
   if (!p) return fail(FG_E_ARG, "NULL plan");
   const HostPlan& H = p->H;

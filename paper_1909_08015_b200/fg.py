@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfg.so")
 
 EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
-           "fg_plan_info", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
+           "fg_plan_info", "fg_host_plan", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
            "fg_dfma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
 
@@ -68,6 +68,7 @@ def lib():
         L.fg_plan_opts_default.argtypes = [C.POINTER(fg_plan_opts)]
         L.fg_plan_create.argtypes = [vp, C.POINTER(fg_plan_opts), C.c_int32, C.POINTER(vp)]
         L.fg_plan_destroy.argtypes = [vp]
+        L.fg_host_plan.argtypes = [vp, C.POINTER(fg_plan_opts), C.POINTER(fg_plan_stats), vp, C.c_int32, vp, C.c_int32, vp, vp]
         L.fg_plan_set_tol.argtypes = [vp, C.c_double, C.c_double]
         L.fg_plan_profile.argtypes = [vp, C.c_int32]
         L.fg_plan_timing.argtypes = [vp, vp, vp]
@@ -220,6 +221,33 @@ class Plan:
         I = np.zeros(n); y = np.zeros(n); fl = np.zeros(n, dtype=np.uint8)
         _check(lib().fg_sample_eval_dump(self.h, int(first), int(n), int(seed), _stream(stream), _p(I), _p(y), _p(fl)))
         return dict(I=I, y=y, flags=fl)
+
+
+_OPS = {0: "A", 1: "U", 2: "L", 3: "L-U"}
+
+
+def host_plan(graph, merge_ext_lines=False, deg_table=None, tables=False):
+    """fg_host_plan: the planner alone (host, no device): (stats, subgraphs, terms[, Deg, Z_1])."""
+    o = fg_plan_opts(); lib().fg_plan_opts_default(C.byref(o)); o.merge_ext_lines = int(bool(merge_ext_lines))
+    keep = None
+    if deg_table is not None:
+        keep = np.ascontiguousarray(deg_table, dtype=np.float64); o.deg_table = keep.ctypes.data
+    st = fg_plan_stats(); subs = np.zeros((64, 4), dtype=np.int32); buf = np.zeros(1 << 16, dtype=np.int32)
+    deg = z1 = None
+    if tables:
+        deg = np.zeros(1 << 15); z1 = np.zeros(1 << 15)
+    w = _check(lib().fg_host_plan(graph.h, C.byref(o), C.byref(st), _p(subs), 64, _p(buf), len(buf), _p(deg), _p(z1)))
+    stats = {k: getattr(st, k) for k, _ in fg_plan_stats._fields_}
+    terms, i = [], 0
+    while i < w:
+        sign, gp, nm = int(buf[i]), int(buf[i + 1]), int(buf[i + 2]); i += 3
+        terms.append(dict(sign=sign, gprime=gp, members=[(int(buf[i + 2 * k]), _OPS[int(buf[i + 2 * k + 1])]) for k in range(nm)]))
+        i += 2 * nm
+    ss = [dict(a=int(r[0]), b=int(r[1]), type="V" if r[2] else "SE", in_chain=bool(r[3])) for r in subs[:stats["n_subgraphs"]]]
+    if tables:
+        n = 1 << stats["M"]
+        return stats, ss, terms, deg[:n], z1[:n]
+    return stats, ss, terms
 
 
 def result_merge(a, b):
