@@ -232,7 +232,9 @@ template <class T, int S, int K, bool AC = false, bool RC = false> struct QExt {
 template <class T, int S, bool AC, bool RC> struct QExt<T, S, 0, AC, RC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
 // Running state of one program: accumulators of the current destination.
-template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part; };   // part: per-lane DMMA partial sums
+// part: per-lane DMMA partial sums.  split: the 32 lanes of a warp evaluate the SAME point and share its records out
+// (record i goes to lane i % 32); their partial sums are added when a destination is finished (short double-double queues).
+template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part, split, rr; };
 
 FG_HD constexpr int rec_ncoef(int k, int flags) {
   return (((flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k) + 1) & ~1;
@@ -321,12 +323,38 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
   for (int s = 0; s < S; ++s) { accp[s] = acc[s]; aabp[s] = aab[s]; }
 }
 
+FG_HD int fg_lane() {
+#if defined(__CUDA_ARCH__)
+  return (int)(threadIdx.x & 31);
+#else
+  return 0;
+#endif
+}
+#if defined(__CUDACC__)
+__device__ __forceinline__ double warp_sum(double v) { for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o); return v; }
+__device__ __forceinline__ dd warp_sum(dd v) { for (int o = 16; o > 0; o >>= 1) v = v + dd(__shfl_xor_sync(0xffffffffu, v.hi, o), __shfl_xor_sync(0xffffffffu, v.lo, o)); return v; }
+#endif
+// split mode: add the partial sums of the 32 lanes (every lane ends up with the same totals)
+template <class T, int S>
+FG_HD void fold_split(RecState<T, S>& st) {
+#if defined(__CUDA_ARCH__)
+  if (st.split) {
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+#pragma unroll
+      for (int s = 0; s < S; ++s) { st.acc[c][s] = warp_sum(st.acc[c][s]); st.aab[c][s] = warp_sum(st.aab[c][s]); }
+    }
+  }
+#endif
+}
+
 // One group of any class, everything dynamic (wide records, two-component records, the double-double pass).
 template <class T, int S, int ABS>
 FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, int k, int flags, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st) {
   const bool wide = (flags & FG_REC_WIDE) != 0;
   const int stride = (wide ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double);
   for (int r = 0; r < nrec; ++r, p += stride) {
+    if (st.split && ((st.rr++) & 31) != fg_lane()) continue;
     const uint8_t* fidx = wide ? ((const FgRecW*)p)->fidx : ((const FgRecC*)p)->fidx;
     const uint8_t* vidx = wide ? ((const FgRecW*)p)->vidx : ((const FgRecC*)p)->vidx;
     const double cab = wide ? (double)((const FgRecW*)p)->cabs : (double)((const FgRecC*)p)->cabs;
@@ -427,6 +455,7 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
   for (int t = 0; t < ntiles; ++t, p += tile_bytes) {
     const FgRecM* recs = (const FgRecM*)p; const double* __restrict__ fr = (const double*)(p + 8 * sizeof(FgRecM));
     for (int n = 0; n < 8; ++n) {
+      if (st.split && ((st.rr++) & 31) != fg_lane()) continue;
       const double cab = (double)recs[n].cabs;
 #pragma unroll
       for (int s = 0; s < S; ++s) {
@@ -593,7 +622,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
     const int nrec = gh.nrec, nf = gh.nf, k = gh.k, flags = gh.flags;
     if ((int)gh.dst != st.cur) {
       fold_mma_partials(st);
-      if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
+      if (st.cur >= 0) { fold_split(st); flush(st.cur, st.acc, st.aab); }
       st.cur = gh.dst;
 #pragma unroll
       for (int s = 0; s < S; ++s) { st.acc[0][s] = T(0.0); st.acc[1][s] = T(0.0); st.aab[0][s] = 0.0; st.aab[1][s] = 0.0; }

@@ -52,7 +52,7 @@ struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2]; };
 
 // a6: run the record stream of one program for the S samples of this thread
 template <class T, int S, int ABS>
-__device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const T* Vt, int vs, int ne, T* Sc, int ss) {
+__device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const T* Vt, int vs, int ne, T* Sc, int ss, int split) {
   const int nslots = (1 << N.nse) * FG_NDEG * N.ncomp;
   for (int i = 0; i < nslots; ++i) {
 #pragma unroll
@@ -66,7 +66,7 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     mbar_expect_tx(&ring.bar[0], used[0]); bulk_g2s(ring.buf, g0, used[0], &ring.bar[0]);
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
   }
-  RecState<T, S> st; st.cur = -1; st.has_part = 0;
+  RecState<T, S> st; st.cur = -1; st.has_part = 0; st.split = split; st.rr = 0;
   const int nc = N.ncomp, rawv = sm.rawv, rawa = sm.rawa;
   auto flush = [&](int dst, const T (*acc)[S], const double (*aab)[S]) {
     for (int c = 0; c < nc; ++c) {
@@ -82,12 +82,12 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], used[ch + 2]); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, used[ch + 2], &ring.bar[b]); }
   }
   fold_mma_partials(st);
-  if (st.cur >= 0) flush(st.cur, st.acc, st.aab);
+  if (st.cur >= 0) { fold_split(st); flush(st.cur, st.acc, st.aab); }
 }
 
 // a5-a7 for the S points of this thread
 template <class T, int S, int ABS>
-__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* amx, double* amp) {
+__device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* amx, double* amp, int split) {
   const ScratchMap sm(P);
   double zl[S][FG_MAXLINES];
 #pragma unroll
@@ -110,7 +110,7 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
     }
     for (int ni = P.geom_num_begin[g]; ni < P.geom_num_begin[g + 1]; ++ni) {
       const FgNumDev N = P.nums[ni];
-      run_program<T, S, ABS>(P, N, sm, ring, Vt, vs, (int)E.ne, Sc, ss);
+      run_program<T, S, ABS>(P, N, sm, ring, Vt, vs, (int)E.ne, Sc, ss, split);
       for (int k = 0; k < N.node_count; ++k) {
 #pragma unroll
         for (int s = 0; s < S; ++s) { finish_node<T, false>(P, sm, N.node_begin + k, Sc + s, ss); if (ABS) finish_node<T, true>(P, sm, N.node_begin + k, Sc + s, ss); }
@@ -140,14 +140,16 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
   T* Vt = Vsm + tid * S;
   T* Sc = (T*)A.scratch + (size_t)blockIdx.x * (size_t)P.scratch_slots * ss + tid * S;
   const uint64_t nwork = A.idlist ? (uint64_t)*A.idcount : A.n;
-  const uint64_t per_batch = (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
+  // short double-double queues: one point per WARP, its records shared out over the lanes (32x shorter latency)
+  const int split = (is_dd<T>::value && S == 1 && nwork * 32 <= (uint64_t)gridDim.x * NT) ? 1 : 0;
+  const uint64_t per_batch = split ? (uint64_t)(NT / 32) : (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
   dd sy(0.0), sy2(0.0); unsigned long long nflag = 0, nrej = 0, nbig = 0;
   const int M = P.M;
   for (uint64_t batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
     double z[S][FG_MAXM], mant[S]; int ex[S]; bool valid[S], bad[S]; uint64_t oid[S];
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      const uint64_t ord = batch * per_batch + (uint64_t)s * NT + tid;
+      const uint64_t ord = split ? batch * per_batch + (uint64_t)(tid >> 5) : batch * per_batch + (uint64_t)s * NT + tid;
       valid[s] = ord < nwork; bad[s] = false; mant[s] = 0.5; ex[s] = 1; oid[s] = 0;
       if (valid[s]) {
         oid[s] = A.idlist ? (uint64_t)A.idlist[ord] : ord;
@@ -161,10 +163,10 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
       if (!valid[s] || bad[s]) for (int v = 0; v < M; ++v) z[s][v] = 1.0 / M;
     }
     T I[S]; double Iabs[S], growth[S], amp[S];
-    eval_points<T, S, is_dd<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp);
+    eval_points<T, S, is_dd<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp, split);
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      if (!valid[s]) continue;
+      if (!valid[s] || (split && (tid & 31) != 0)) continue;
       const double Id = to_double(I[s]);
       double af = growth[s] * growth[s]; af = af * af * af;      // |A|, |A^q| <= 1 is assumed by cabs; amax^6 otherwise
       // running error estimate: K * u * sum|terms| with u = 2^-53 (double pass) or 2^-104 (double-double pass)

@@ -192,6 +192,31 @@ def test_structure_matches_expression_11(fg):
     assert np.allclose(z["z"].sum(axis=1), 1.0, atol=1e-14) and not z["bad"].any()
 
 
+def test_config3_all_fifty_three_loop_graphs(fg):       # BASELINE.json config 3: every graph, double-double fallback on
+    worst = 0.0; unresolved = 0; total = 0
+    for x, ph in inputs.all_graphs(3):
+        plan = fg.plan_for(x, ph, rel_tol=1e-12); orc = O.Oracle(x, ph, printed=False)
+        z = plan.sample_dump(0, 600, 3, words=False)["z"]
+        Iq = orc.eval(z)[1]; e0 = plan.eval_points(z, mode=0)
+        ok = np.isfinite(Iq) & (Iq != 0) & ((e0["flags"] & 6) == 0)
+        worst = max(worst, float(np.max(np.abs(e0["I"][ok] - Iq[ok]) / np.abs(Iq[ok]))))
+        unresolved += int((~ok).sum()); total += len(z)
+    assert worst <= 1e-12 and unresolved < 0.03 * total
+
+
+def test_config4_ladder_prefix_per_sample(fg):          # BASELINE.json config 4: per-sample agreement on a prefix
+    plan, orc = pair(fg, *G4)
+    n = 32768
+    d = plan.sample_eval_dump(0, n, 1); s = plan.sample_dump(0, n, 1, words=False); so = orc.sample(1, 0, n)
+    assert np.array_equal(s["order"], so["order"]) and np.array_equal(s["comp"], so["comp"])
+    Iq = orc.eval(s["z"])[1]
+    ok = np.isfinite(Iq) & (Iq != 0) & ((d["flags"] & 6) == 0)
+    assert ok.mean() > 0.9
+    assert np.all(np.abs(d["I"][ok] - Iq[ok]) <= 1e-12 * np.abs(Iq[ok]))
+    gq = so["pdf_mant"] * np.exp2(so["pdf_exp"].astype(np.float64))
+    assert np.all(np.abs(d["y"][ok] - Iq[ok] / gq[ok]) <= 2e-12 * np.abs(Iq[ok] / gq[ok]))
+
+
 @pytest.mark.skipif((os.cpu_count() or 1) < 16 and not os.environ.get("FG_TEST_5LOOP"), reason="oracle tables of a 5-loop graph take ~5 min on 8 cores")
 def test_five_loop_sampled_outputs(fg):            # config 5 in the launch configuration bench.py times
     cfg = inputs.config(5); x, ph = cfg["graphs"][0]
