@@ -353,8 +353,11 @@ template <class T, int S, int ABS>
 FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, int k, int flags, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st) {
   const bool wide = (flags & FG_REC_WIDE) != 0;
   const int stride = (wide ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double);
-  for (int r = 0; r < nrec; ++r, p += stride) {
-    if (st.split && ((st.rr++) & 31) != fg_lane()) continue;
+  // split mode: record i of the running count goes to lane i % 32; every lane walks its own records (all lanes busy)
+  int r0 = 0, rstep = 1;
+  if (st.split) { r0 = (fg_lane() - st.rr) & 31; rstep = 32; st.rr += nrec; }
+  p += (size_t)r0 * stride;
+  for (int r = r0; r < nrec; r += rstep, p += (size_t)rstep * stride) {
     const uint8_t* fidx = wide ? ((const FgRecW*)p)->fidx : ((const FgRecC*)p)->fidx;
     const uint8_t* vidx = wide ? ((const FgRecW*)p)->vidx : ((const FgRecC*)p)->vidx;
     const double cab = wide ? (double)((const FgRecW*)p)->cabs : (double)((const FgRecC*)p)->cabs;
@@ -452,20 +455,21 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
     if (ABS == 2) for (int J = 0; J < 4 * steps; ++J) monoa[s][J] = t_abs_d(mono[s][J]);
   }
   const int tile_bytes = 8 * (int)sizeof(FgRecM) + steps * 32 * (int)sizeof(double);
-  for (int t = 0; t < ntiles; ++t, p += tile_bytes) {
-    const FgRecM* recs = (const FgRecM*)p; const double* __restrict__ fr = (const double*)(p + 8 * sizeof(FgRecM));
-    for (int n = 0; n < 8; ++n) {
-      if (st.split && ((st.rr++) & 31) != fg_lane()) continue;
-      const double cab = (double)recs[n].cabs;
+  int q0 = 0, qstep = 1;
+  if (st.split) { q0 = (fg_lane() - st.rr) & 31; qstep = 32; st.rr += ntiles * 8; }
+  for (int q = q0; q < ntiles * 8; q += qstep) {
+    const int t = q >> 3, n = q & 7;
+    const unsigned char* pt = p + (size_t)t * tile_bytes;
+    const FgRecM* recs = (const FgRecM*)pt; const double* __restrict__ fr = (const double*)(pt + 8 * sizeof(FgRecM));
+    const double cab = (double)recs[n].cabs;
 #pragma unroll
-      for (int s = 0; s < S; ++s) {
-        T q = T(0.0); double qa = 0.0;
-        for (int J = 0; J < 4 * steps; ++J) { const double c = fr[(J >> 2) * 32 + n * 4 + (J & 3)]; q = q + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
-        T bp = T(1.0); for (int f = 0; f < nf; ++f) bp = bp * Vt[(int)recs[n].fidx[f] * vs + s];
-        st.acc[0][s] = st.acc[0][s] + bp * q;
-        if (ABS == 1) st.aab[0][s] = fma(t_abs_d(bp), cab, st.aab[0][s]);
-        if (ABS == 2) st.aab[0][s] = fma(t_abs_d(bp), qa, st.aab[0][s]);
-      }
+    for (int s = 0; s < S; ++s) {
+      T qv = T(0.0); double qa = 0.0;
+      for (int J = 0; J < 4 * steps; ++J) { const double c = fr[(J >> 2) * 32 + n * 4 + (J & 3)]; qv = qv + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
+      T bp = T(1.0); for (int f = 0; f < nf; ++f) bp = bp * Vt[(int)recs[n].fidx[f] * vs + s];
+      st.acc[0][s] = st.acc[0][s] + bp * qv;
+      if (ABS == 1) st.aab[0][s] = fma(t_abs_d(bp), cab, st.aab[0][s]);
+      if (ABS == 2) st.aab[0][s] = fma(t_abs_d(bp), qa, st.aab[0][s]);
     }
   }
 }
