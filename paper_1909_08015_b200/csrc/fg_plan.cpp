@@ -15,6 +15,8 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <numeric>
@@ -303,71 +305,61 @@ static void build_records(const HGeom& E, int type, HNum& N, bool& limit_hit) {
     bool wantq = (N.op == FG_OP_A && type == 1);
     bool pseudo = false; for (int s : m.unmatched) if (E.slots[s].se >= 0) pseudo = true;
     int k = (int)m.unmatched.size();
-    if (wantq && !pseudo && k >= 1 && k <= FG_KMAX) {
-      // one record for the whole matching: main table + one table per slot that may carry gamma^nu A^q
-      std::vector<double> main_t; matching_table(E, type, N.op, 0, m, -1, false, m.unmatched, main_t);
-      HRecord r; r.nf = npairs; r.k = k; r.dst = sig0 * FG_NDEG + npairs; r.flags = 0;
-      std::memset(r.fidx, 0, sizeof(r.fidx)); std::memset(r.vidx, 0, sizeof(r.vidx));
-      for (int t = 0; t < r.nf; ++t) r.fidx[t] = (uint8_t)f0[t];
-      for (int t = 0; t < k; ++t) r.vidx[t] = (uint8_t)(nb + E.slots[m.unmatched[t]].e);
-      r.coef = main_t; bool nz = false, nzq = false; for (double v : main_t) if (v != 0.0) nz = true;
-      std::vector<double> qall;
-      for (int j = 0; j < k; ++j) {
-        std::vector<int> gaps; for (int s : m.unmatched) if (s != m.unmatched[j]) gaps.push_back(s);
-        std::vector<double> qt; matching_table(E, type, N.op, 0, m, m.unmatched[j], true, gaps, qt);
-        for (double v : qt) if (v != 0.0) nzq = true;
-        qall.insert(qall.end(), qt.begin(), qt.end());
-      }
-      if (nzq) { r.flags |= FG_REC_QEXT; r.coef.insert(r.coef.end(), qall.begin(), qall.end()); }
-      if (nz || nzq) { finish_record(r); per[mi].push_back(std::move(r)); }
-      continue;
-    }
-    if (wantq && !pseudo && k > FG_KMAX && npairs + (k - FG_KMAX) <= FG_MAXF - 1) {
-      // more free slots than a dense table holds: the first FG_KMAX unmatched slots stay free variables, the others are
-      // enumerated (a slot in the set carries A_j p-hat and becomes a product factor).  The slot that carries gamma^nu A^q
-      // is either one of the free variables (q-extension tables of the same record) or an enumerated slot (own records).
+    if (wantq) {
+      // Operator A: besides the gamma^0 A_j terms exactly one unmatched slot may carry gamma^nu A^q_j.
+      // Free variables of the records = the first FG_KMAX unmatched OWN lines; every other unmatched slot (further own
+      // lines, pseudo-slots of self-energy children) is enumerated: in the set -> product factor A_j (and the v
+      // component of the child), not in the set -> factor 1 (u component).  The gamma^nu slot is either a free variable
+      // (q-extension tables of the same record) or an enumerated slot (own records with the factor A^q).
       const std::vector<int>& um = m.unmatched;
-      const int ke = k - FG_KMAX;
+      std::vector<int> mat, en;
+      for (int sl : um) { if (E.slots[sl].se < 0 && (int)mat.size() < FG_KMAX) mat.push_back(sl); else en.push_back(sl); }
+      const int km = (int)mat.size(), ke = (int)en.size();
+      if (npairs + ke + 1 > FG_MAXF) { over = true; continue; }
       auto tab_index = [](const std::vector<int>& gaps, const std::vector<int>& set) { size_t T = 0; for (int sl : set) { size_t pos = std::find(gaps.begin(), gaps.end(), sl) - gaps.begin(); T |= (size_t)1 << pos; } return T; };
       std::vector<double> main_t; matching_table(E, type, N.op, 0, m, -1, false, um, main_t);
       std::vector<std::vector<double>> qt(k); std::vector<std::vector<int>> qgaps(k);
       for (int j = 0; j < k; ++j) { for (int sl : um) if (sl != um[j]) qgaps[j].push_back(sl); matching_table(E, type, N.op, 0, m, um[j], true, qgaps[j], qt[j]); }
-      auto fill_common = [&](HRecord& r, const std::vector<int>& extra) {
+      auto pos_in_um = [&](int sl) { return (int)(std::find(um.begin(), um.end(), sl) - um.begin()); };
+      auto fill_common = [&](HRecord& r, const std::vector<int>& extra, int sig) {
         std::memset(r.fidx, 0, sizeof(r.fidx)); std::memset(r.vidx, 0, sizeof(r.vidx));
         std::vector<int> f = f0; for (int v : extra) f.push_back(v);
         r.nf = (int)f.size(); for (int t = 0; t < r.nf; ++t) r.fidx[t] = (uint8_t)f[t];
-        r.k = FG_KMAX; for (int t = 0; t < FG_KMAX; ++t) r.vidx[t] = (uint8_t)(nb + E.slots[um[t]].e);
-        r.dst = sig0 * FG_NDEG + npairs;
+        r.k = km; for (int t = 0; t < km; ++t) r.vidx[t] = (uint8_t)(nb + E.slots[mat[t]].e);
+        r.dst = sig * FG_NDEG + npairs;
       };
       for (unsigned eb = 0; eb < (1u << ke); ++eb) {
-        std::vector<int> te, extra; for (int t = 0; t < ke; ++t) if ((eb >> t) & 1) { te.push_back(um[FG_KMAX + t]); extra.push_back(nb + E.slots[um[FG_KMAX + t]].e); }
-        HRecord r; r.flags = 0; fill_common(r, extra);
-        r.coef.assign((size_t)1 << FG_KMAX, 0.0); bool nz = false, nzq = false;
-        for (size_t sub = 0; sub < ((size_t)1 << FG_KMAX); ++sub) {
-          std::vector<int> set = te; for (int t = 0; t < FG_KMAX; ++t) if ((sub >> t) & 1) set.push_back(um[t]);
+        std::vector<int> te, extra; int sig = sig0;
+        for (int t = 0; t < ke; ++t) if ((eb >> t) & 1) { const Slot& sl = E.slots[en[t]]; te.push_back(en[t]); extra.push_back(nb + sl.e); if (sl.se >= 0) sig |= 1 << sl.se; }
+        HRecord r; r.flags = 0; fill_common(r, extra, sig);
+        r.coef.assign((size_t)1 << km, 0.0); bool nz = false, nzq = false;
+        for (size_t sub = 0; sub < ((size_t)1 << km); ++sub) {
+          std::vector<int> set = te; for (int t = 0; t < km; ++t) if ((sub >> t) & 1) set.push_back(mat[t]);
           double v = main_t[tab_index(um, set)]; r.coef[sub] = v; if (v != 0.0) nz = true;
         }
         std::vector<double> qall;
-        for (int j = 0; j < FG_KMAX; ++j) {
-          std::vector<int> rest; for (int t = 0; t < FG_KMAX; ++t) if (t != j) rest.push_back(um[t]);
-          for (size_t sub = 0; sub < ((size_t)1 << (FG_KMAX - 1)); ++sub) {
-            std::vector<int> set = te; for (int t = 0; t < FG_KMAX - 1; ++t) if ((sub >> t) & 1) set.push_back(rest[t]);
-            double v = qt[j][tab_index(qgaps[j], set)]; qall.push_back(v); if (v != 0.0) nzq = true;
+        for (int j = 0; j < km; ++j) {
+          const int ju = pos_in_um(mat[j]);
+          std::vector<int> rest; for (int t = 0; t < km; ++t) if (t != j) rest.push_back(mat[t]);
+          for (size_t sub = 0; sub < ((size_t)1 << (km - 1)); ++sub) {
+            std::vector<int> set = te; for (int t = 0; t < km - 1; ++t) if ((sub >> t) & 1) set.push_back(rest[t]);
+            double v = qt[ju][tab_index(qgaps[ju], set)]; qall.push_back(v); if (v != 0.0) nzq = true;
           }
         }
         if (nzq) { r.flags |= FG_REC_QEXT; r.coef.insert(r.coef.end(), qall.begin(), qall.end()); }
         if (nz || nzq) { finish_record(r); per[mi].push_back(std::move(r)); }
       }
-      for (int jq = FG_KMAX; jq < k; ++jq) {       // gamma^nu on an enumerated slot
-        std::vector<int> others; for (int t = FG_KMAX; t < k; ++t) if (t != jq) others.push_back(um[t]);
+      for (int jq = 0; jq < ke; ++jq) {       // gamma^nu on an enumerated slot
+        const Slot& qs = E.slots[en[jq]]; const int ju = pos_in_um(en[jq]);
+        std::vector<int> others; for (int t = 0; t < ke; ++t) if (t != jq) others.push_back(en[t]);
         for (unsigned eb = 0; eb < (1u << others.size()); ++eb) {
-          std::vector<int> te, extra = {nb + ne + E.slots[um[jq]].e};
-          for (size_t t = 0; t < others.size(); ++t) if ((eb >> t) & 1) { te.push_back(others[t]); extra.push_back(nb + E.slots[others[t]].e); }
-          HRecord r; r.flags = 0; fill_common(r, extra);
-          r.coef.assign((size_t)1 << FG_KMAX, 0.0); bool nz = false;
-          for (size_t sub = 0; sub < ((size_t)1 << FG_KMAX); ++sub) {
-            std::vector<int> set = te; for (int t = 0; t < FG_KMAX; ++t) if ((sub >> t) & 1) set.push_back(um[t]);
-            double v = qt[jq][tab_index(qgaps[jq], set)]; r.coef[sub] = v; if (v != 0.0) nz = true;
+          std::vector<int> te, extra = {nb + ne + qs.e}; int sig = sig0 | (qs.se >= 0 ? 1 << qs.se : 0);
+          for (size_t t = 0; t < others.size(); ++t) if ((eb >> t) & 1) { const Slot& sl = E.slots[others[t]]; te.push_back(others[t]); extra.push_back(nb + sl.e); if (sl.se >= 0) sig |= 1 << sl.se; }
+          HRecord r; r.flags = 0; fill_common(r, extra, sig);
+          r.coef.assign((size_t)1 << km, 0.0); bool nz = false;
+          for (size_t sub = 0; sub < ((size_t)1 << km); ++sub) {
+            std::vector<int> set = te; for (int t = 0; t < km; ++t) if ((sub >> t) & 1) set.push_back(mat[t]);
+            double v = qt[ju][tab_index(qgaps[ju], set)]; r.coef[sub] = v; if (v != 0.0) nz = true;
           }
           if (nz) { finish_record(r); per[mi].push_back(std::move(r)); }
         }
