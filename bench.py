@@ -202,6 +202,10 @@ def main_fg(args):
     algo = sum(p.stats["flops_per_sample"] for p in plans) * S * args.steps
     execf = sum(p.stats["exec_flops_per_sample"] for p in plans) * S * args.steps
     ach = algo / (ms_d * 1e-3) / 1e12
+    for gi, x in enumerate(tim):       # per-graph throughput of the double-precision pass and its algorithmic FP64 rate
+        info[gi]["samples_per_s"] = S * args.steps / (x["ms_double"] * 1e-3)
+        info[gi]["algo_tflops"] = info[gi]["flops_per_sample"] * info[gi]["samples_per_s"] / 1e12
+        info[gi]["dd_ms_per_step"] = x["ms_dd"] / args.steps
     traffic = None      # DRAM bytes per launch, scaled per sample from the committed ncu capture (profiles/r01_traffic.json)
     try:
         tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))

@@ -157,6 +157,17 @@ def test_ranges_shard_and_merge_exactly(fg):       # sharding by sa
     assert again.sum_y[0] == whole.sum_y[0] and again.sum_y2[0] == whole.sum_y2[0]
 
 
+def test_more_than_one_slab(fg):                   # the integrator works in slabs of 2^24 samples
+    plan, _ = pair(fg, *G1)
+    n = (1 << 24) + 12345
+    whole = plan.integrate_range(7, n, 3, raw=True)
+    a = plan.integrate_range(7, 1 << 24, 3, raw=True); b = plan.integrate_range(7 + (1 << 24), 12345, 3, raw=True)
+    m = fg.result_merge(a, b)
+    assert whole.n_samples == n == m.n_samples and whole.n_flagged == m.n_flagged and whole.n_rejected == m.n_rejected
+    assert abs(whole.sum_y[0] - m.sum_y[0]) <= 1e-14 * abs(m.sum_y[0]) and abs(whole.sum_y2[0] - m.sum_y2[0]) <= 1e-14 * m.sum_y2[0]
+    assert abs(whole.mean - 0.5) < 5 * math.sqrt(whole.variance)
+
+
 @pytest.mark.parametrize("n", [1, 2, 255, 256, 257, 4097])
 def test_ragged_sizes(fg, n):
     plan, orc = pair(fg, *G2[0])
