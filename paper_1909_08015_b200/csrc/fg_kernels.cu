@@ -141,7 +141,8 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
   T* Sc = (T*)A.scratch + (size_t)blockIdx.x * (size_t)P.scratch_slots * ss + tid * S;
   const uint64_t nwork = A.idlist ? (uint64_t)*A.idcount : A.n;
   // short double-double queues: one point per WARP, its records shared out over the lanes (32x shorter latency)
-  const int split = (is_dd<T>::value && S == 1 && nwork * 32 <= (uint64_t)gridDim.x * NT) ? 1 : 0;
+  // (a split round is ~7x shorter than a round with one point per thread, so up to 6 split rounds still win)
+  const int split = (is_dd<T>::value && S == 1 && nwork * 32 <= 6ull * gridDim.x * NT) ? 1 : 0;
   const uint64_t per_batch = split ? (uint64_t)(NT / 32) : (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
   dd sy(0.0), sy2(0.0); unsigned long long nflag = 0, nrej = 0, nbig = 0;
   const int M = P.M;
