@@ -145,6 +145,19 @@ def test_one_loop_value_and_two_loop_sum(fg):
     assert abs(tot - target) < 4 * math.sqrt(var) and math.sqrt(var) < 0.01
 
 
+def test_config2_full_size_two_loop_sum(fg):           # BASELINE.json config 2: 1e8 samples per graph
+    """Sum of the six 2-loop graphs without lepton loops = A1^(4) - (119/36 - pi^2/3) (PAPER.md:28 and north_star)."""
+    tot = var = 0.0; rej = 0
+    for x, ph in G2:
+        plan = fg.plan_for(x, ph, rel_tol=1e-9)
+        r = plan.integrate(10 ** 8, 1)
+        tot += r["mean"]; var += r["variance"]; rej += r["n_rejected"]
+    target = -0.328478965579 - (119.0 / 36.0 - math.pi ** 2 / 3.0)
+    assert math.sqrt(var) < 2.5e-3
+    assert abs(tot - target) < 4 * math.sqrt(var), (tot, target, math.sqrt(var))
+    assert rej < 6e8 * 1e-3
+
+
 def test_ranges_shard_and_merge_exactly(fg):       # SURVEY 8(e): sharding by sample-id range
     plan, _ = pair(fg, *G2[2])
     whole = plan.integrate_range(100, 70001, 4, raw=True)
