@@ -657,14 +657,9 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
         if (!st.has_part) { st.has_part = 1; for (int b = 0; b < 8; ++b) st.part[b] = 0.0; }
         const double* Vw = (const double*)Vt - (threadIdx.x & 31);
         const bool qx = (flags & FG_REC_QEXT) != 0;
-        const int tile_bytes = 8 * (int)sizeof(FgRecM) + mma_steps(k, qx) * 32 * (int)sizeof(double);
-        // consecutive tensor-core groups of the same class and destination are run by one call
-        const unsigned char* p0 = p - sizeof(FgGroupHdr); const unsigned char* pe = p + nrec * tile_bytes; int nseq = 1;
-        while (g + nseq < ngroups) {
-          const FgGroupHdr nx = *(const FgGroupHdr*)pe;
-          if (nx.nf != gh.nf || nx.k != gh.k || nx.flags != gh.flags || nx.dst != gh.dst) break;
-          pe += sizeof(FgGroupHdr) + (int)nx.nrec * tile_bytes; ++nseq;
-        }
+        // consecutive tensor-core groups of the same class and destination are run by one call (run length and size
+        // come from the planner)
+        const unsigned char* p0 = p - sizeof(FgGroupHdr); const int nseq = gh.nseq; const unsigned char* pe = p0 + gh.seq_bytes;
         switch (nf * 8 + k) {
 #define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p0, nseq, Vw, vs, ne, st.part); else run_group_mma_fast<NF, K, false>(p0, nseq, Vw, vs, ne, st.part); break;
           FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)

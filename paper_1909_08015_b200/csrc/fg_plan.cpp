@@ -593,9 +593,32 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     // pack records into chunks of class-uniform groups; keep = leading product factors shared with the previous record.
     // Runs of records with the same class and the same free variables become tensor-core (DMMA) tile groups.
     size_t cur = 0, base = 0, ghdr = 0; bool open = false, gopen = false; int ngroups = 0, gn = 0; const HRecord* prev = nullptr;
+    auto mma_steps = [](int k, bool qx) { int nm = 1 << (k - 2); return nm + (qx ? nm + (k - 2) * ((1 << k) >> 3) : 0); };
+    auto rec_ncoef_host = [](int k, int flags) { int n = (flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k; return (n + 1) & ~1; };
     auto cls = [](const HRecord& r) { int fl = r.flags & (FG_REC_TWO | FG_REC_QEXT); if (r.nf > FG_NFC) fl |= FG_REC_WIDE; return (r.dst << 16) | (r.nf << 12) | (r.k << 8) | fl; };
     auto close_group = [&]() { if (gopen) { FgGroupHdr g; std::memcpy(&g, &P.d_chunks[ghdr], sizeof(g)); g.nrec = (uint16_t)gn; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); gopen = false; } };
-    auto close_chunk = [&]() { close_group(); if (open) { FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.ngroups = ngroups; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false; P.d_chunk_used.push_back((uint32_t)((cur + 15) & ~(size_t)15)); } };
+    auto close_chunk = [&]() {
+      close_group();
+      if (!open) return;
+      FgChunkHdr h; std::memset(&h, 0, sizeof(h)); h.ngroups = ngroups; std::memcpy(&P.d_chunks[base], &h, sizeof(h)); open = false;
+      P.d_chunk_used.push_back((uint32_t)((cur + 15) & ~(size_t)15));
+      // sequences of tensor-core groups of one class: length and byte size, stored in the first header of each run
+      std::vector<size_t> offs, sizes; size_t o = base + sizeof(FgChunkHdr);
+      for (int gi = 0; gi < ngroups; ++gi) {
+        FgGroupHdr g; std::memcpy(&g, &P.d_chunks[o], sizeof(g));
+        const bool qx = (g.flags & FG_REC_QEXT) != 0;
+        size_t body = (g.flags & FG_REC_MMA) ? (size_t)g.nrec * (8 * sizeof(FgRecM) + (size_t)mma_steps(g.k, qx) * 32 * sizeof(double))
+                                             : (size_t)g.nrec * (((g.flags & FG_REC_WIDE) ? sizeof(FgRecW) : sizeof(FgRecC)) + (size_t)rec_ncoef_host(g.k, g.flags) * sizeof(double));
+        offs.push_back(o); sizes.push_back(sizeof(FgGroupHdr) + body); o += sizeof(FgGroupHdr) + body;
+      }
+      for (int gi = 0; gi < ngroups; ++gi) {
+        FgGroupHdr g; std::memcpy(&g, &P.d_chunks[offs[gi]], sizeof(g));
+        if (!(g.flags & FG_REC_MMA)) continue;
+        int n = 1; size_t bytes = sizes[gi];
+        for (int gj = gi + 1; gj < ngroups; ++gj) { FgGroupHdr g2; std::memcpy(&g2, &P.d_chunks[offs[gj]], sizeof(g2)); if (g2.nf != g.nf || g2.k != g.k || g2.flags != g.flags || g2.dst != g.dst) break; ++n; bytes += sizes[gj]; }
+        g.nseq = (uint16_t)n; g.seq_bytes = (uint32_t)bytes; std::memcpy(&P.d_chunks[offs[gi]], &g, sizeof(g));
+      }
+    };
     auto new_chunk = [&]() { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); ngroups = 0; open = true; };
     auto open_group = [&](const HRecord& r, int extra_flags) {
       close_group();
@@ -604,7 +627,6 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       std::memcpy(g.vidx, r.vidx, sizeof(g.vidx));
       ghdr = base + cur; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); cur += sizeof(g); gopen = true; gn = 0; ++ngroups; prev = nullptr;
     };
-    auto mma_steps = [](int k, bool qx) { int nm = 1 << (k - 2); return nm + (qx ? nm + (k - 2) * ((1 << k) >> 3) : 0); };
     auto mma_coef = [](const HRecord& r, int step, int x) -> double {
       const int k = r.k, nm = 1 << (k - 2); const double* mainT = r.coef.data(); const double* qT = mainT + (1 << k); const int qs = (1 << k) >> 1;
       if (step < nm) return mainT[x | (step << 2)];

@@ -92,7 +92,9 @@ static_assert(sizeof(FgRecC) == 16 && sizeof(FgRecW) == 32, "record header sizes
 // previous record (prefix products stay in registers).
 // The group header carries the free variables (vidx) and nrec = number of tiles.
 struct alignas(16) FgRecM { uint8_t fidx[FG_NFC]; uint8_t keep; uint8_t pad[6]; float cabs; };
-struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint8_t pad[6]; };
+// nseq / seq_bytes (tensor-core groups): number and total size of the consecutive groups of the same class and
+// destination that start here inside this chunk (one kernel call runs them all).
+struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint16_t nseq; uint32_t seq_bytes; };
 static_assert(sizeof(FgRecM) == 16 && sizeof(FgGroupHdr) == 16, "group header sizes");
 struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
 
