@@ -154,13 +154,17 @@ FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T
   for (int a = 0; a < l; ++a) for (int b = 0; b < a; ++b) { C[a] = C[a] - B[a][b] * C[b]; Cq[a] = Cq[a] - B[a][b] * Cq[b]; }   // L^-1 C, L^-1 C^q
   dd w(0.0); for (int a = 0; a < l; ++a) { w = w + C[a] * C[a] * invd[a]; C[a] = C[a] * invd[a]; Cq[a] = Cq[a] * invd[a]; }
   W = from_dd<T>(w);
-  dd Y[FG_MAXNE][FG_MAXL];
+  dd Y[FG_MAXNE][FG_MAXL]; int first[FG_MAXNE];
   const int nb = ne * (ne + 1) / 2; double am = 1.0, cond = 1.0;
   for (int q = 0; q < ne; ++q) {
     const unsigned m = E.eta[q];
-    for (int a = 0; a < l; ++a) { dd y = ((m >> a) & 1u) ? dd(1.0) : dd(0.0); for (int b = 0; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
+    // y = L^-1 eta_q vanishes below the first loop of the line: structural zeros (block-uniform) are skipped everywhere
+    int fq = 0; while (fq < l && !((m >> fq) & 1u)) ++fq;
+    first[q] = fq;
+    for (int a = 0; a < fq; ++a) Y[q][a] = dd(0.0);
+    for (int a = fq; a < l; ++a) { dd y = ((m >> a) & 1u) ? dd(1.0) : dd(0.0); for (int b = fq; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
     dd sa(0.0), sq(0.0); double ta = 1.0, tq = 0.5;
-    for (int a = 0; a < l; ++a) { const dd t1 = Y[q][a] * C[a], t2 = Y[q][a] * Cq[a]; sa = sa + t1; sq = sq + t2; ta += fabs(t1.hi); tq += fabs(t2.hi); }
+    for (int a = fq; a < l; ++a) { const dd t1 = Y[q][a] * C[a], t2 = Y[q][a] * Cq[a]; sa = sa + t1; sq = sq + t2; ta += fabs(t1.hi); tq += fabs(t2.hi); }
     const dd A = dd(1.0) - sa, Aq = dd(0.5 * (double)E.xiq[q]) - sq;
     V[(nb + q) * vs] = from_dd<T>(A); V[(nb + ne + q) * vs] = from_dd<T>(Aq);
     am = fmax(am, fmax(fabs(A.hi), fabs(Aq.hi)));
@@ -170,9 +174,10 @@ FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T
   amax = am;
   int idx = 0;
   for (int i = 0; i < ne; ++i) {
-    dd yd[FG_MAXL]; for (int a = 0; a < l; ++a) yd[a] = Y[i][a] * invd[a];
+    dd yd[FG_MAXL]; for (int a = first[i]; a < l; ++a) yd[a] = Y[i][a] * invd[a];
     for (int j = i; j < ne; ++j) {
-      dd b(0.0); double tb = 0.0; for (int a = 0; a < l; ++a) { const dd t1 = yd[a] * Y[j][a]; b = b + t1; tb += fabs(t1.hi); }
+      const int f2 = first[i] > first[j] ? first[i] : first[j];
+      dd b(0.0); double tb = 0.0; for (int a = f2; a < l; ++a) { const dd t1 = yd[a] * Y[j][a]; b = b + t1; tb += fabs(t1.hi); }
       if (b.hi != 0.0) cond = fmax(cond, tb / fabs(b.hi));
       V[idx * vs] = from_dd<T>(b); ++idx;
     }
