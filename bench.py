@@ -206,9 +206,9 @@ def main_fg(args):
         info[gi]["samples_per_s"] = S * args.steps / (x["ms_double"] * 1e-3)
         info[gi]["algo_tflops"] = info[gi]["flops_per_sample"] * info[gi]["samples_per_s"] / 1e12
         info[gi]["dd_ms_per_step"] = x["ms_dd"] / args.steps
-    traffic = None      # DRAM bytes per launch, scaled per sample from the committed ncu capture (profiles/r01_traffic.json)
+    traffic = None      # DRAM bytes per launch, scaled per sample from the committed ncu capture (profiles/r01_traffic.txt)
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.txt")))
         traffic = (tj["dram_bytes_read"] + tj["dram_bytes_write"]) / tj["samples"] * S
     except Exception:
         pass
