@@ -114,7 +114,8 @@ typedef struct {
   double sum_y2[2];
   uint64_t n_samples;
   uint64_t n_flagged;     /* samples re-evaluated in double-double */
-  uint64_t n_rejected;    /* samples that contributed 0 (non-finite or degenerate point) */
+  uint64_t n_rejected;    /* samples that contributed 0: degenerate point, non-finite value, or not resolved by the
+                             double-double rung */
   uint64_t n_pdf_big_exp; /* samples whose pdf left the double range, kept as x*2^j */
 } fg_result;
 
@@ -135,9 +136,11 @@ int fg_result_merge(const fg_result* a, const fg_result* b, fg_result* out);
  * ordering j_1..j_M (n*M), z (n*M), pdf mantissa in [0.5,1) and exponent (n each), bad flag (n). */
 int fg_sample_dump(const fg_plan*, uint64_t first, uint64_t n, uint64_t seed, void* stream, uint32_t* philox_words,
                    int32_t* comp, uint8_t* orderings, double* z, double* pdf_mant, int32_t* pdf_exp, uint8_t* bad);
-/* fg_eval_points: integrand at n given points (n*M doubles, on the simplex).  I = final value (double-double
- * where flagged), I_double = plain double pass, err = its running error estimate, flags bit0 = flagged,
- * bit1 = non-finite.  mode 0: as the integrator does; 1: double only; 2: double-double for every point. */
+/* fg_eval_points: integrand at n given points (n*M doubles, on the simplex; n <= 2^24).  I = final value (double-double
+ * where flagged), I_double = plain double pass, err = its running error estimate.  flags: bit0 = re-evaluated in
+ * double-double, bit1 = non-finite value or degenerate point, bit2 = not resolved by the last rung (estimated error of
+ * the double-double value still above the tolerance: the integrator lets such a sample contribute 0).
+ * mode 0: as the integrator does; 1: double only; 2: double-double for every point. */
 int fg_eval_points(const fg_plan*, const double* z, uint64_t n, int32_t mode, void* stream, double* I,
                    double* I_double, double* err, uint8_t* flags);
 /* fg_sample_eval_dump: what the integrator computes per sample, for samples first..first+n-1:
