@@ -33,10 +33,10 @@ FG_HD dd two_sum(double a, double b) { double s = f_add(a, b), bb = f_add(s, -a)
 FG_HD dd quick_two_sum(double a, double b) { double s = f_add(a, b); return dd(s, f_add(b, -f_add(s, -a))); }
 FG_HD dd two_prod(double a, double b) { double p = f_mul(a, b); return dd(p, f_fma(a, b, -p)); }
 
-FG_HD dd operator+(dd a, dd b) {
-  dd s = two_sum(a.hi, b.hi), t = two_sum(a.lo, b.lo);
-  s.lo = f_add(s.lo, t.hi); s = quick_two_sum(s.hi, s.lo);
-  s.lo = f_add(s.lo, t.lo); return quick_two_sum(s.hi, s.lo);
+FG_HD dd operator+(dd a, dd b) {      // "sloppy" sum: error <= 2^-104 (|a| + |b|); cancellation is accounted for by the |.| sums
+  dd s = two_sum(a.hi, b.hi);
+  s.lo = f_add(s.lo, f_add(a.lo, b.lo));
+  return quick_two_sum(s.hi, s.lo);
 }
 FG_HD dd operator-(dd a) { return dd(-a.hi, -a.lo); }
 FG_HD dd operator-(dd a, dd b) { return a + (-b); }
