@@ -144,6 +144,7 @@ def main_fg(args):
         plans.append(p); info.append(dict(graph=gi, x=x, photons=ph, abs_tol=0.25 * sig_target, **{k: p.stats[k] for k in ("n_terms", "n_records", "n_coefs", "flops_per_sample", "exec_flops_per_sample", "plan_seconds")}))
     peak_tf, _ = fg.dfma_peak(local, 200000, stream)
     peak_tf = max(peak_tf, fg.dfma_peak(local, 200000, stream)[0])
+    dmma_tf = fg.dmma_peak(local, 20000, stream)[0]       # FP64 tensor path (shares the FP64 units with DFMA): context
     res_dev = torch.zeros(16 * len(plans), dtype=torch.float64, device=dev)
 
     def step_async(k):
@@ -222,7 +223,7 @@ def main_fg(args):
                        "kernel_ms": {"double_pass": ms_d, "dd_pass": ms_q, "share_double": ms_d / max(ms_d + ms_q, 1e-9)},
                        "exec_tflops_double_pass": execf / (ms_d * 1e-3) / 1e12},
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": traffic,
-                         "kernel": "fg_eval_kernel<double,1,256>", "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
+                         "kernel": "fg_eval_kernel<double,1,256>", "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)", "dmma_peak": dmma_tf,
                          "frac_executed": execf / (ms_d * 1e-3) / 1e12 / peak_tf},
             "e2e": {"value": total / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 80 * len(plans)},
             "gpu_launches": launches, "clocks": clk}

@@ -151,6 +151,9 @@ int fg_sample_eval_dump(const fg_plan*, uint64_t first, uint64_t n, uint64_t see
  * returns achieved TFLOP/s (FMA = 2) over `iters` dependent-chain steps x 8 chains per thread on all SMs. */
 int fg_dfma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms);
 
+/* fg_dmma_peak: the same for the FP64 tensor path (mma.sync m8n8k4 f64, 8 independent accumulator pairs per warp). */
+int fg_dmma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms);
+
 const char* fg_strerror(int code);
 const char* fg_last_error_message(void);
 const char* fg_version(void);

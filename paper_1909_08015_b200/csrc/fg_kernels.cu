@@ -252,6 +252,21 @@ __global__ void fg_dfma_kernel(double* out, int iters, double a, double b) {
   out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// FP64 tensor peak: 8 independent DMMA m8n8k4 accumulator pairs per warp (shares the FP64 units with DFMA)
+__global__ void fg_dmma_kernel(double* out, int iters, double a, double b) {
+  double c0[8], c1[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { c0[i] = i + threadIdx.x * 1e-9; c1[i] = -i; }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0[i]), "+d"(c1[i]) : "d"(a), "d"(b));
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += c0[i] + c1[i];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace fg
 
 // =================================================================================================
@@ -625,6 +640,26 @@ int fg_dfma_peak(int32_t device, int32_t iters, void* stream, double* tflops, do
   float ms = 0; CU(cudaEventElapsedTime(&ms, e0, e1));
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   double flops = 2.0 * 8.0 * (double)iters * threads * blocks;
+  *tflops = flops / (ms * 1e-3) / 1e12; if (ms_out) *ms_out = ms;
+  return FG_OK;
+}
+
+int fg_dmma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms_out) {
+  if (!tflops || iters <= 0) return fail(FG_E_ARG, "bad argument");
+  int ndev = 0; if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(FG_E_CUDA, "no CUDA device");
+  CU(cudaSetDevice(device));
+  cudaDeviceProp prop; CU(cudaGetDeviceProperties(&prop, device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const int threads = 256, blocks = prop.multiProcessorCount * 8;
+  DevBuf out; CUB(out.alloc((size_t)threads * blocks * sizeof(double)));
+  cudaEvent_t e0, e1; CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  fg_dmma_kernel<<<blocks, threads, 0, st>>>((double*)out.d, iters / 8 + 1, 1e-3, 1.0);   // warm-up
+  CU(cudaEventRecord(e0, st));
+  fg_dmma_kernel<<<blocks, threads, 0, st>>>((double*)out.d, iters, 1e-3, 1.0);
+  CU(cudaEventRecord(e1, st)); CU(cudaEventSynchronize(e1));
+  float ms = 0; CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  const double flops = 2.0 * 8 * 8 * 4 * 8.0 * (double)iters * ((double)threads * blocks / 32.0);
   *tflops = flops / (ms * 1e-3) / 1e12; if (ms_out) *ms_out = ms;
   return FG_OK;
 }

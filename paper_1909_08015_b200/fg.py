@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libfg.so")
 EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
            "fg_plan_info", "fg_host_plan", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
-           "fg_dfma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
+           "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
 
 
 class FgError(RuntimeError):
@@ -83,6 +83,7 @@ def lib():
         L.fg_eval_points.argtypes = [vp, vp, C.c_uint64, C.c_int32, vp] + [vp] * 4
         L.fg_sample_eval_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp] + [vp] * 3
         L.fg_dfma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.fg_dmma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         for f in ("fg_strerror", "fg_last_error_message", "fg_version"):
             getattr(L, f).restype = C.c_char_p
         L.fg_strerror.argtypes = [C.c_int]
@@ -260,6 +261,13 @@ def dfma_peak(device=0, iters=200000, stream=None):
     """fg_dfma_peak: measured FP64-FMA throughput (TFLOP/s, FMA = 2) and kernel time in ms."""
     t = C.c_double(); ms = C.c_double()
     _check(lib().fg_dfma_peak(int(device), int(iters), _stream(stream), C.byref(t), C.byref(ms)))
+    return t.value, ms.value
+
+
+def dmma_peak(device=0, iters=20000, stream=None):
+    """fg_dmma_peak: measured FP64 tensor-core (DMMA m8n8k4) throughput (TFLOP/s) and kernel time in ms."""
+    t = C.c_double(); ms = C.c_double()
+    _check(lib().fg_dmma_peak(int(device), int(iters), _stream(stream), C.byref(t), C.byref(ms)))
     return t.value, ms.value
 
 
