@@ -280,7 +280,10 @@ static int fail(int code, const std::string& m) { g_err = m; return code; }
 
 struct fg_graph { Graph g; };
 
-static const int NT_D = 256, S_D = 1;     // double pass: max threads per block (launch bound), samples per thread
+#ifndef FG_NT_D
+#define FG_NT_D 256
+#endif
+static const int NT_D = FG_NT_D, S_D = 1;     // double pass: max threads per block (launch bound), samples per thread
 static const int NT_Q = 192, S_Q = 1;     // double-double pass
 static const uint64_t SLAB = 1ull << 24;  // samples per launch (bounds the re-evaluation queue)
 

@@ -10,7 +10,9 @@
 #define FG_NDEG 6          // polynomial in t: degrees 0..5
 #define FG_KMAX 4          // free variables of one numerator record (dense 2^k table); further ones are enumerated
 #define FG_MAXF 10         // product factors of one record
+#ifndef FG_CHUNK_BYTES
 #define FG_CHUNK_BYTES 32768  // numerator stream is cut into chunks of this size (records and tiles never straddle)
+#endif
 #define FG_VPAD 8          // padding (elements) of the row stride of the per-sample operand table V in shared memory
 #define FG_MAXSE 4         // self-energy children of one element
 #define FG_MAXVC 5         // vertexlike children of one element
