@@ -459,18 +459,18 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
     mma_monomials<T>(k, qx, a, aq, mono[s]);
     if (ABS == 2) for (int J = 0; J < 4 * steps; ++J) monoa[s][J] = t_abs_d(mono[s][J]);
   }
-  const int tile_bytes = 8 * (int)sizeof(FgRecM) + steps * 32 * (int)sizeof(double);
+  const int tile_bytes = FG_TILE_BYTES(steps);
   int q0 = 0, qstep = 1;
   if (st.split) { q0 = (fg_lane() - st.rr) & 31; qstep = 32; st.rr += ntiles * 8; }
   for (int q = q0; q < ntiles * 8; q += qstep) {
     const int t = q >> 3, n = q & 7;
     const unsigned char* pt = p + (size_t)t * tile_bytes;
-    const FgRecM* recs = (const FgRecM*)pt; const double* __restrict__ fr = (const double*)(pt + 8 * sizeof(FgRecM));
+    const FgRecM* recs = (const FgRecM*)pt; const FgMmaCoef* __restrict__ fr = (const FgMmaCoef*)(pt + 8 * sizeof(FgRecM));
     const double cab = (double)recs[n].cabs;
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       T qv = T(0.0); double qa = 0.0;
-      for (int J = 0; J < 4 * steps; ++J) { const double c = fr[(J >> 2) * 32 + n * 4 + (J & 3)]; qv = qv + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
+      for (int J = 0; J < 4 * steps; ++J) { const double c = (double)fr[(J >> 2) * 32 + n * 4 + (J & 3)]; qv = qv + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
       T bp = T(1.0); for (int f = 0; f < nf; ++f) bp = bp * Vt[(int)recs[n].fidx[f] * vs + s];
       st.acc[0][s] = st.acc[0][s] + bp * qv;
       if (ABS == 1) st.aab[0][s] = fma(t_abs_d(bp), cab, st.aab[0][s]);
@@ -482,7 +482,7 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
 #if defined(__CUDACC__)
 // Tensor-core path of a group (double pass, one sample per thread, whole warp converged).  DMMA m8n8k4:
 //   A (8 samples x 4 monomials): lane (r = lane/4, c = lane%4) holds monomial 4*step + c of sample 8*b + r;
-//   B (4 monomials x 8 records): lane holds coef[4*step + c] of record r -> one conflict-free LDS.64 per step;
+//   B (4 monomials x 8 records): lane holds coef[4*step + c] of record r -> one conflict-free LDS.32 per step (float, exact);
 //   D (8 x 8): lane holds records 2c, 2c+1 of sample 8*b + r.
 // Each lane then weights its two record values with their products of beta's and keeps per-lane partial sums for the four
 // row blocks b; out[0..3] = value partials, out[4..7] = |.| partials (reduced over the quad by the caller).
@@ -494,13 +494,13 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 template <int NF, int K, bool QX, int NT2>
 __device__ __forceinline__ void mma_tiles(const unsigned char* __restrict__ p, const double* __restrict__ Vw, int vs, int lane, int r, int c,
                                           int v0, int v1, int v2, int v3, int vq, double* acc, double* aab, double (*pf)[NF > 0 ? NF : 1]) {
-  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
+  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS);
   double B[NT2][STEPS], cab[NT2][2]; int ff[NT2][2][NF > 0 ? NF : 1], keep[NT2][2];
 #pragma unroll
   for (int u = 0; u < NT2; ++u) {
     const unsigned char* pt = p + u * TILE;
 #pragma unroll
-    for (int st = 0; st < STEPS; ++st) B[u][st] = ((const double*)(pt + 8 * sizeof(FgRecM)))[st * 32 + lane];
+    for (int st = 0; st < STEPS; ++st) B[u][st] = (double)((const FgMmaCoef*)(pt + 8 * sizeof(FgRecM)))[st * 32 + lane];
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const uint4 h = *(const uint4*)(pt + (2 * c + e) * 16);
@@ -573,7 +573,7 @@ __device__ __forceinline__ void mma_tiles(const unsigned char* __restrict__ p, c
 template <int NF, int K, bool QX>
 __device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int vs, int ne, double* __restrict__ out) {
   __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
-  constexpr int STEPS = mma_steps(K, QX), TILE = 8 * (int)sizeof(FgRecM) + STEPS * 32 * (int)sizeof(double);
+  constexpr int STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS);
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int vq = ne * vs;
   double acc[4], aab[4], pf[4][NF > 0 ? NF : 1];
@@ -676,7 +676,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
       }
 #endif
       if (!done) run_group_mma_dyn<T, S, ABS>(p, nrec, nf, k, flags, gh.vidx, Vt, vs, ne, st);
-      p += nrec * (8 * (int)sizeof(FgRecM) + mma_steps(k, (flags & FG_REC_QEXT) != 0) * 32 * (int)sizeof(double));
+      p += nrec * FG_TILE_BYTES(mma_steps(k, (flags & FG_REC_QEXT) != 0));
       continue;
     }
     if (!done) run_group_dyn<T, S, ABS>(p, nrec, nf, k, flags, Vt, vs, ne, st);

@@ -607,7 +607,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       for (int gi = 0; gi < ngroups; ++gi) {
         FgGroupHdr g; std::memcpy(&g, &P.d_chunks[o], sizeof(g));
         const bool qx = (g.flags & FG_REC_QEXT) != 0;
-        size_t body = (g.flags & FG_REC_MMA) ? (size_t)g.nrec * (8 * sizeof(FgRecM) + (size_t)mma_steps(g.k, qx) * 32 * sizeof(double))
+        size_t body = (g.flags & FG_REC_MMA) ? (size_t)g.nrec * (size_t)FG_TILE_BYTES(mma_steps(g.k, qx))
                                              : (size_t)g.nrec * (((g.flags & FG_REC_WIDE) ? sizeof(FgRecW) : sizeof(FgRecC)) + (size_t)rec_ncoef_host(g.k, g.flags) * sizeof(double));
         offs.push_back(o); sizes.push_back(sizeof(FgGroupHdr) + body); o += sizeof(FgGroupHdr) + body;
       }
@@ -639,9 +639,12 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       while (j < nr && cls(N.recs[j]) == cls(N.recs[i]) && std::memcmp(N.recs[j].vidx, N.recs[i].vidx, sizeof(N.recs[i].vidx)) == 0) ++j;
       const HRecord& r0 = N.recs[i];
       const bool qx = (r0.flags & FG_REC_QEXT) != 0;
-      const bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= 2 && (j - i) >= FG_MMA_MINREC;
+      bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= 2 && (j - i) >= FG_MMA_MINREC;
+      if (mma) {     // tiles store float: only if every coefficient of the run survives the round trip unchanged
+        for (size_t t = i; t < j && mma; ++t) for (double c : N.recs[t].coef) if ((double)(FgMmaCoef)c != c) { mma = false; break; }
+      }
       if (mma) {
-        const int steps = mma_steps(r0.k, qx); const size_t tile_bytes = 8 * sizeof(FgRecM) + (size_t)steps * 32 * sizeof(double);
+        const int steps = mma_steps(r0.k, qx); const size_t tile_bytes = (size_t)FG_TILE_BYTES(steps);
         const int R = (int)(j - i), ntiles = (R + 7) / 8;
         // record shown to lane c (of every quad) in tile t, slot e: depth-first index c*2*ntiles + 2t + e
         auto rec_at = [&](int t, int n) -> const HRecord* { int d = (n >> 1) * 2 * ntiles + 2 * t + (n & 1); return d < R ? &N.recs[i + d] : nullptr; };
@@ -660,9 +663,9 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
             }
             std::memcpy(&P.d_chunks[base + cur + n * sizeof(FgRecM)], &h, sizeof(h));
           }
-          double* fr = (double*)&P.d_chunks[base + cur + 8 * sizeof(FgRecM)];
+          FgMmaCoef* fr = (FgMmaCoef*)&P.d_chunks[base + cur + 8 * sizeof(FgRecM)];
           for (int st = 0; st < steps; ++st) for (int n = 0; n < 8; ++n) for (int x = 0; x < 4; ++x) {
-            const HRecord* r = rec_at(t, n); fr[st * 32 + n * 4 + x] = r ? mma_coef(*r, st, x) : 0.0;
+            const HRecord* r = rec_at(t, n); fr[st * 32 + n * 4 + x] = r ? (FgMmaCoef)mma_coef(*r, st, x) : (FgMmaCoef)0;
           }
           cur += tile_bytes; ++gn;
           N.exec_flops += 8.0 * (8.0 * steps + 4.0);

@@ -88,11 +88,16 @@ static_assert(sizeof(FgRecC) == 16 && sizeof(FgRecW) == 32, "record header sizes
 //   main  steps t < 2^(k-2):        mlo[x] * mhi[t],  mlo = {1, a0, a1, a0 a1}, mhi[t] = prod_{bit i of t} a_{2+i}
 //   low-q steps (q-extension):      {aq0, aq0 a1, aq1, aq1 a0}[x] * mhi[t]
 //   high-q steps, j = 2..k-1:       aq_j * mlo[x] * (product over the subset t' of the other high variables)
-// A tile = 8 x FgRecM (product factors, cabs) + steps x 32 doubles in B-fragment order (lane = 4*record + x).
+// A tile = 8 x FgRecM (product factors, cabs) + steps x 32 FgMmaCoef in B-fragment order (lane = 4*record + x).
+// The coefficients of a tile are stored as float: the planner makes a tensor-core group only of records whose
+// coefficients float holds exactly (integers times powers of two at every loop count met so far), so the double the
+// kernel converts back to is the same number; half the stream bytes, twice the tiles per chunk.
 // Lane c of a quad weights records 2c, 2c+1 of every tile; the planner deals the records of a run out so that these form
 // one contiguous stretch of the depth-first matching order, and keep = leading product factors shared with the lane's
 // previous record (prefix products stay in registers).
 // The group header carries the free variables (vidx) and nrec = number of tiles.
+typedef float FgMmaCoef;
+#define FG_TILE_BYTES(steps) (8 * (int)sizeof(FgRecM) + (steps) * 32 * (int)sizeof(FgMmaCoef))
 struct alignas(16) FgRecM { uint8_t fidx[FG_NFC]; uint8_t keep; uint8_t pad[6]; float cabs; };
 // nseq / seq_bytes (tensor-core groups): number and total size of the consecutive groups of the same class and
 // destination that start here inside this chunk (one kernel call runs them all).
