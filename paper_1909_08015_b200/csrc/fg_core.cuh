@@ -237,8 +237,9 @@ template <class T, int S, int K, bool AC = false, bool RC = false> struct QExt {
 template <class T, int S, bool AC, bool RC> struct QExt<T, S, 0, AC, RC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
 // Running state of one program: accumulators of the current destination.
-// part: per-lane DMMA partial sums.  split: the 32 lanes of a warp evaluate the SAME point and share its records out
-// (record i goes to lane i % 32); their partial sums are added when a destination is finished (short double-double queues).
+// part: per-lane DMMA partial sums.  split = w (0 = off, else 2..32): groups of w adjacent lanes evaluate the SAME point
+// and share its records out (record i goes to lane i % w); their partial sums are added when a destination is finished
+// (short double-double queues).
 template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part, split, rr; };
 
 FG_HD constexpr int rec_ncoef(int k, int flags) {
@@ -336,10 +337,11 @@ FG_HD int fg_lane() {
 #endif
 }
 #if defined(__CUDACC__)
-__device__ __forceinline__ double warp_sum(double v) { for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o); return v; }
-__device__ __forceinline__ dd warp_sum(dd v) { for (int o = 16; o > 0; o >>= 1) v = v + dd(__shfl_xor_sync(0xffffffffu, v.hi, o), __shfl_xor_sync(0xffffffffu, v.lo, o)); return v; }
+__device__ __forceinline__ double warp_sum(double v, int w) { for (int o = w >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o); return v; }
+__device__ __forceinline__ dd warp_sum(dd v, int w) { for (int o = w >> 1; o > 0; o >>= 1) v = v + dd(__shfl_xor_sync(0xffffffffu, v.hi, o), __shfl_xor_sync(0xffffffffu, v.lo, o)); return v; }
 #endif
-// split mode: add the partial sums of the 32 lanes (every lane ends up with the same totals)
+// split mode (st.split = w = 2..32 lanes per point): add the partial sums of the w lanes of a point (each of them ends up
+// with the same totals)
 template <class T, int S>
 FG_HD void fold_split(RecState<T, S>& st) {
 #if defined(__CUDA_ARCH__)
@@ -347,7 +349,7 @@ FG_HD void fold_split(RecState<T, S>& st) {
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
 #pragma unroll
-      for (int s = 0; s < S; ++s) { st.acc[c][s] = warp_sum(st.acc[c][s]); st.aab[c][s] = warp_sum(st.aab[c][s]); }
+      for (int s = 0; s < S; ++s) { st.acc[c][s] = warp_sum(st.acc[c][s], st.split); st.aab[c][s] = warp_sum(st.aab[c][s], st.split); }
     }
   }
 #endif
@@ -358,9 +360,9 @@ template <class T, int S, int ABS>
 FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, int k, int flags, const T* __restrict__ Vt, int vs, int ne, RecState<T, S>& st) {
   const bool wide = (flags & FG_REC_WIDE) != 0;
   const int stride = (wide ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double);
-  // split mode: record i of the running count goes to lane i % 32; every lane walks its own records (all lanes busy)
+  // split mode: record i of the running count goes to lane i % w of the point; every lane walks its own records
   int r0 = 0, rstep = 1;
-  if (st.split) { r0 = (fg_lane() - st.rr) & 31; rstep = 32; st.rr += nrec; }
+  if (st.split) { r0 = (fg_lane() - st.rr) & (st.split - 1); rstep = st.split; st.rr += nrec; }
   p += (size_t)r0 * stride;
   for (int r = r0; r < nrec; r += rstep, p += (size_t)rstep * stride) {
     const uint8_t* fidx = wide ? ((const FgRecW*)p)->fidx : ((const FgRecC*)p)->fidx;
@@ -461,7 +463,7 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
   }
   const int tile_bytes = FG_TILE_BYTES(steps);
   int q0 = 0, qstep = 1;
-  if (st.split) { q0 = (fg_lane() - st.rr) & 31; qstep = 32; st.rr += ntiles * 8; }
+  if (st.split) { q0 = (fg_lane() - st.rr) & (st.split - 1); qstep = st.split; st.rr += ntiles * 8; }
   for (int q = q0; q < ntiles * 8; q += qstep) {
     const int t = q >> 3, n = q & 7;
     const unsigned char* pt = p + (size_t)t * tile_bytes;

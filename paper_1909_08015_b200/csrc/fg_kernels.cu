@@ -140,17 +140,22 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
   T* Vt = Vsm + tid * S;
   T* Sc = (T*)A.scratch + (size_t)blockIdx.x * (size_t)P.scratch_slots * ss + tid * S;
   const uint64_t nwork = A.idlist ? (uint64_t)*A.idcount : A.n;
-  // short double-double queues: one point per WARP, its records shared out over the lanes (32x shorter latency)
-  // (a split round is ~7x shorter than a round with one point per thread, so up to 6 split rounds still win)
-  const int split = (is_dd<T>::value && S == 1 && nwork * 32 <= 6ull * gridDim.x * NT) ? 1 : 0;
-  const uint64_t per_batch = split ? (uint64_t)(NT / 32) : (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
+  // short double-double queues: one point per group of w = 2..32 lanes, its records dealt out to the lanes.  A round
+  // then takes about 0.115 + 0.885 / w of a round with one point per thread (measured at w = 32: ~7x shorter) and
+  // holds 1/w of the points; w minimises rounds x time per round (the same choice in every block)
+  int split = 0;
+  if (is_dd<T>::value && S == 1 && nwork > 0) {
+    const double cap = (double)gridDim.x * NT; double best = ceil((double)nwork / cap);
+    for (int w = 2; w <= 32; w <<= 1) { const double c = ceil((double)nwork * w / cap) * (0.115 + 0.885 / w); if (c < best) { best = c; split = w; } }
+  }
+  const uint64_t per_batch = split ? (uint64_t)(NT / split) : (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
   dd sy(0.0), sy2(0.0); unsigned long long nflag = 0, nrej = 0, nbig = 0;
   const int M = P.M;
   for (uint64_t batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
     double z[S][FG_MAXM], mant[S]; int ex[S]; bool valid[S], bad[S]; uint64_t oid[S];
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      const uint64_t ord = split ? batch * per_batch + (uint64_t)(tid >> 5) : batch * per_batch + (uint64_t)s * NT + tid;
+      const uint64_t ord = split ? batch * per_batch + (uint64_t)(tid / split) : batch * per_batch + (uint64_t)s * NT + tid;
       valid[s] = ord < nwork; bad[s] = false; mant[s] = 0.5; ex[s] = 1; oid[s] = 0;
       if (valid[s]) {
         oid[s] = A.idlist ? (uint64_t)A.idlist[ord] : ord;
@@ -167,7 +172,7 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
     eval_points<T, S, is_dd<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp, split);
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      if (!valid[s] || (split && (tid & 31) != 0)) continue;
+      if (!valid[s] || (split && (tid & (split - 1)) != 0)) continue;
       const double Id = to_double(I[s]);
       double af = growth[s] * growth[s]; af = af * af * af;      // |A|, |A^q| <= 1 is assumed by cabs; amax^6 otherwise
       // running error estimate: K * u * sum|terms| with u = 2^-53 (double pass) or 2^-104 (double-double pass)

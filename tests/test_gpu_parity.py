@@ -254,3 +254,29 @@ def test_five_loop_sampled_outputs(fg):            # config 5 in the launch conf
     assert np.all(np.abs(e0["I"][ok] - Iq[ok]) <= 1e-12 * np.abs(Iq[ok]))
     e1 = plan.eval_points(z, mode=1)
     assert np.all(np.abs(e1["I_double"] - Iq)[ok] <= np.maximum(e0["err"][ok], 1e-12 * np.abs(Iq[ok])))
+
+
+@pytest.mark.gpu
+def test_double_double_pass_same_values_at_every_queue_length(fg):
+    """The double-double pass deals the records of a point out to groups of w = 2..32 lanes, w chosen from the queue
+    length.  The value of a point must not depend on that choice: the same 300 points are evaluated in
+    queues of growing length (w = 32 ... 2, then one point per thread, then several rounds) and compared with the
+    oracle's __float128 and with each other."""
+    g = G3[2]
+    plan, orc = pair(fg, g[0], g[1], False)
+    zb = plan.sample_dump(0, 300, 7, words=False)["z"]
+    _, Iq, _ = orc.eval(zb, rel_tol=1e-12)
+    ref = None
+    for reps in (1, 10, 24, 47, 95, 200, 420):
+        z = np.ascontiguousarray(np.tile(zb, (reps, 1)))
+        e = plan.eval_points(z, mode=2)
+        I = e["I"].reshape(reps, 300); fl = e["flags"].reshape(reps, 300)
+        res = (fl & 6) == 0                       # resolved; a point at the edge of the tolerance may flip with the summation order
+        assert (res != res[0]).mean() < 0.01
+        ok = np.isfinite(Iq) & (Iq != 0) & res.all(axis=0)
+        assert ok.mean() > 0.9
+        assert np.all(np.abs(I[:, ok] - Iq[ok]) <= 1e-12 * np.abs(Iq[ok]))
+        if ref is None:
+            ref = (I[0], ok)
+        both = ok & ref[1]
+        assert np.all(np.abs(I[:, both] - ref[0][both]) <= 1e-14 * np.abs(ref[0][both]))
