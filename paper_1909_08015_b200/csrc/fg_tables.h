@@ -66,7 +66,9 @@ struct FgTermDev {
 #define FG_REC_WIDE 4      // records use the wide header (nf > FG_NFC): generic slow path
 #define FG_REC_MMA 8       // tensor-core group: records that share their free variables, stored as 8-record tiles
 #define FG_NFC 5           // product factors of a compact record (= Wick pairs, <= n)
+#ifndef FG_MMA_MINREC
 #define FG_MMA_MINREC 3    // a run of records with equal free variables becomes a tensor-core group from this length on
+#endif
 struct alignas(16) FgRecC {   // compact record header, 16 bytes, followed by the coefficient tables (even count of doubles)
   uint8_t keep;
   uint8_t fidx[FG_NFC];
