@@ -80,6 +80,12 @@ int fg_plan_set_tol(fg_plan*, double rel_tol, double abs_tol);
 int fg_plan_profile(fg_plan*, int32_t enable);
 int fg_plan_timing(const fg_plan*, double* ms3, int64_t* launches);
 
+/* Profiling builds only (-DFG_PHASE_PROF): warp-cycles (clock64, summed over all warps of the double-precision pass) spent in
+ * 0 sampler, 1 element geometry, 2 tensor-core record groups, 3 static scalar groups, 4 dynamic groups, 5 ring wait + chunk
+ * barrier, 6 node products, 7 forest sum + weights, 8 group dispatch / flush.  Returns 1 when the library was built with the
+ * counters, 0 when not (cycles stay 0).  reset != 0 clears them. */
+int fg_plan_phase_cycles(const fg_plan*, uint64_t* cycles16, int32_t reset);
+
 typedef struct {
   int32_t n_loops, M;                 /* loops, number of Feynman variables */
   int32_t n_subgraphs, n_forests, n_terms;       /* UV-divergent subgraphs incl. G; forests; (F,G') terms */

@@ -27,11 +27,13 @@ def needs_build():
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
-def build(force=False, verbose=False):
-    if not force and not needs_build():
+def build(force=False, verbose=False, defines=(), out=None):
+    """defines: extra -D macros (e.g. FG_PHASE_PROF for the per-phase cycle counters); out: library path (default LIB)."""
+    out = out or LIB
+    if not force and out == LIB and not needs_build():
         return LIB
     cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-           "-Xcompiler", "-fPIC,-fopenmp,-ffp-contract=off,-O2", "-shared", "-o", LIB] + SOURCES
+           "-Xcompiler", "-fPIC,-fopenmp,-ffp-contract=off,-O2", "-shared", "-o", out] + ["-D" + d for d in defines] + SOURCES
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     r = subprocess.run(cmd, cwd=CSRC, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
@@ -39,9 +41,10 @@ def build(force=False, verbose=False):
         sys.stderr.write(r.stdout)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + r.stdout[-4000:])
-    return LIB
+    return out
 
 
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose="--verbose" in sys.argv)
-    print(LIB)
+    defs = [a[2:] for a in sys.argv[1:] if a.startswith("-D")]
+    outs = [a[6:] for a in sys.argv[1:] if a.startswith("--out=")]
+    print(build(force="--force" in sys.argv or bool(defs) or bool(outs), verbose="--verbose" in sys.argv, defines=defs, out=outs[0] if outs else None))

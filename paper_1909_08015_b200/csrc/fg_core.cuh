@@ -240,7 +240,19 @@ template <class T, int S, bool AC, bool RC> struct QExt<T, S, 0, AC, RC> { stati
 // part: per-lane DMMA partial sums.  split = w (0 = off, else 2..32): groups of w adjacent lanes evaluate the SAME point
 // and share its records out (record i goes to lane i % w); their partial sums are added when a destination is finished
 // (short double-double queues).
-template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part, split, rr; };
+template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part, split, rr;
+#ifdef FG_PHASE_PROF
+  long long* prof; long long tlast;
+#endif
+};
+// Phase cycle counters of a profiling build (-DFG_PHASE_PROF; fg_plan_phase_cycles): per warp, clock64 deltas between marks.
+// 0 sampler, 1 geometry, 2 tensor-core groups, 3 static scalar groups, 4 dynamic groups, 5 ring wait + chunk barrier,
+// 6 node products, 7 forest sum + weights + tail, 8 program set-up / flush
+#if defined(FG_PHASE_PROF) && defined(__CUDA_ARCH__)
+#define FG_MARK(obj, i) do { const long long t_ = clock64(); (obj).prof[i] += t_ - (obj).tlast; (obj).tlast = t_; } while (0)
+#else
+#define FG_MARK(obj, i) do { } while (0)
+#endif
 
 FG_HD constexpr int rec_ncoef(int k, int flags) {
   return (((flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k) + 1) & ~1;
@@ -629,6 +641,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
   const int ngroups = ((const FgChunkHdr*)chunk)->ngroups;
   const unsigned char* p = chunk + sizeof(FgChunkHdr);
   for (int g = 0; g < ngroups; ++g) {
+    FG_MARK(st, 8);
     const FgGroupHdr gh = *(const FgGroupHdr*)p; p += sizeof(FgGroupHdr);
     const int nrec = gh.nrec, nf = gh.nf, k = gh.k, flags = gh.flags;
     if ((int)gh.dst != st.cur) {
@@ -674,14 +687,15 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
 #undef FG_MM
           default: done = false; break;
         }
-        if (done) { p = pe; g += nseq - 1; continue; }
+        if (done) { FG_MARK(st, 2); p = pe; g += nseq - 1; continue; }
       }
 #endif
       if (!done) run_group_mma_dyn<T, S, ABS>(p, nrec, nf, k, flags, gh.vidx, Vt, vs, ne, st);
+      FG_MARK(st, 4);
       p += nrec * FG_TILE_BYTES(mma_steps(k, (flags & FG_REC_QEXT) != 0));
       continue;
     }
-    if (!done) run_group_dyn<T, S, ABS>(p, nrec, nf, k, flags, Vt, vs, ne, st);
+    if (!done) { run_group_dyn<T, S, ABS>(p, nrec, nf, k, flags, Vt, vs, ne, st); FG_MARK(st, 4); } else FG_MARK(st, 3);
     p += nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));
   }
 }

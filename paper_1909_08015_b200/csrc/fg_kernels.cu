@@ -32,6 +32,7 @@ struct RunArgs {
   int do_flag;
   double* partials;                                            // [gridDim.x][8]
   void* scratch;
+  unsigned long long* phase_cycles;                            // [16] profiling build only (FG_PHASE_PROF), else NULL
 };
 
 struct Accum { double sy[2], sy2[2]; unsigned long long nflag, nrej, nbig, n; };
@@ -48,7 +49,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2]; };
+struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2];
+#ifdef FG_PHASE_PROF
+  long long* prof; long long tlast;
+#endif
+};
 
 // a6: run the record stream of one program for the S samples of this thread
 template <class T, int S, int ABS>
@@ -67,6 +72,9 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
   }
   RecState<T, S> st; st.cur = -1; st.has_part = 0; st.split = split; st.rr = 0;
+#ifdef FG_PHASE_PROF
+  st.prof = ring.prof; st.tlast = ring.tlast;
+#endif
   const int nc = N.ncomp, rawv = sm.rawv, rawa = sm.rawa;
   auto flush = [&](int dst, const T (*acc)[S], const double (*aab)[S]) {
     for (int c = 0; c < nc; ++c) {
@@ -77,12 +85,19 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
   for (int ch = 0; ch < nch; ++ch) {
     const int b = ch & 1;
     mbar_wait(&ring.bar[b], ring.phase[b]); ring.phase[b] ^= 1u;
+    FG_MARK(st, 5);
     run_chunk<T, S, ABS>(ring.buf + b * FG_CHUNK_BYTES, Vt, vs, ne, st, flush);
+    FG_MARK(st, 8);
     __syncthreads();   // every thread is done with buffer b
+    FG_MARK(st, 5);
     if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], used[ch + 2]); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, used[ch + 2], &ring.bar[b]); }
   }
   fold_mma_partials(st);
   if (st.cur >= 0) { fold_split(st); flush(st.cur, st.acc, st.aab); }
+  FG_MARK(st, 8);
+#ifdef FG_PHASE_PROF
+  ring.tlast = st.tlast;
+#endif
 }
 
 // a5-a7 for the S points of this thread
@@ -108,6 +123,7 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
       if (am > amx[s] || !(am == am)) amx[s] = am;
       if (cp > amp[s] || !(cp == cp)) amp[s] = cp;
     }
+    FG_MARK(ring, 1);
     for (int ni = P.geom_num_begin[g]; ni < P.geom_num_begin[g + 1]; ++ni) {
       const FgNumDev N = P.nums[ni];
       run_program<T, S, ABS>(P, N, sm, ring, Vt, vs, (int)E.ne, Sc, ss, split);
@@ -115,6 +131,7 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
 #pragma unroll
         for (int s = 0; s < S; ++s) { finish_node<T, false>(P, sm, N.node_begin + k, Sc + s, ss); if (ABS) finish_node<T, true>(P, sm, N.node_begin + k, Sc + s, ss); }
       }
+      FG_MARK(ring, 6);
     }
   }
 #pragma unroll
@@ -132,6 +149,9 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
   const int NT = blockDim.x;
   extern __shared__ __align__(128) unsigned char smem[];
   ChunkRing ring; ring.buf = smem; ring.bar = (uint64_t*)(smem + 2 * FG_CHUNK_BYTES); ring.phase[0] = ring.phase[1] = 0u;
+#ifdef FG_PHASE_PROF
+  long long prof[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}; ring.prof = prof; ring.tlast = clock64();
+#endif
   T* Vsm = (T*)(smem + 2 * FG_CHUNK_BYTES + 128);
   const int tid = threadIdx.x;
   if (tid == 0) { mbar_init(&ring.bar[0], 1); mbar_init(&ring.bar[1], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
@@ -168,6 +188,7 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
       }
       if (!valid[s] || bad[s]) for (int v = 0; v < M; ++v) z[s][v] = 1.0 / M;
     }
+    FG_MARK(ring, 0);
     T I[S]; double Iabs[S], growth[S], amp[S];
     eval_points<T, S, is_dd<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp, split);
 #pragma unroll
@@ -202,7 +223,11 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
       if (A.outErr) A.outErr[oid[s]] = err;
       if (A.outFlags) A.outFlags[oid[s]] = is_dd<T>::value ? (uint8_t)(A.outFlags[oid[s]] | fl) : fl;
     }
+    FG_MARK(ring, 7);
   }
+#ifdef FG_PHASE_PROF
+  if (A.phase_cycles && (tid & 31) == 0) for (int k = 0; k < 9; ++k) atomicAdd(&A.phase_cycles[k], (unsigned long long)prof[k]);
+#endif
   // a10: warp shuffle -> block -> one partial per block
   double cnt[3] = {(double)nflag, (double)nrej, (double)nbig};
   for (int off = 16; off > 0; off >>= 1) { sy = sy + shfl_dd(sy, off); sy2 = sy2 + shfl_dd(sy2, off); for (int k = 0; k < 3; ++k) cnt[k] += __shfl_down_sync(0xffffffffu, cnt[k], off); }
@@ -296,7 +321,7 @@ struct fg_plan {
   HostPlan H; FgPlanDev D; int device = 0, sms = 0;
   std::vector<void*> allocs;
   void* scratch = nullptr; double* partials = nullptr; Accum* accum = nullptr; fg_result* result_dev = nullptr;
-  uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr;
+  uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr; unsigned long long* phase_cycles = nullptr;
   int grid_d = 0, grid_q = 0, nt_d = 0, nt_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
   int64_t table_bytes = 0;
   int profile = 0; cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; double ms[3] = {0, 0, 0}; long long launches = 0, flagged_last = 0;
@@ -407,6 +432,7 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   if (e == cudaSuccess) e = dmalloc((void**)&p->result_dev, sizeof(fg_result));
   if (e == cudaSuccess) e = dmalloc((void**)&p->flag_list, SLAB * sizeof(uint32_t));
   if (e == cudaSuccess) e = dmalloc((void**)&p->flag_count, sizeof(unsigned long long));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->phase_cycles, 16 * sizeof(unsigned long long));
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
   *out = p; return FG_OK;
 }
@@ -430,6 +456,20 @@ int fg_plan_timing(const fg_plan* p, double* ms3, int64_t* launches) {
   if (ms3) for (int k = 0; k < 3; ++k) ms3[k] = p->ms[k];
   if (launches) *launches = p->launches;
   return FG_OK;
+}
+
+int fg_plan_phase_cycles(const fg_plan* cp, uint64_t* cycles16, int32_t reset) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
+  if (!p) return fail(FG_E_ARG, "NULL plan");
+  std::lock_guard<std::mutex> lk(p->mu);
+  CU(cudaSetDevice(p->device)); CU(cudaDeviceSynchronize());
+  if (cycles16) CU(cudaMemcpy(cycles16, p->phase_cycles, 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  if (reset) CU(cudaMemset(p->phase_cycles, 0, 16 * sizeof(unsigned long long)));
+#ifdef FG_PHASE_PROF
+  return 1;
+#else
+  return FG_OK;
+#endif
 }
 
 int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
@@ -503,7 +543,7 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
                     double* dI, double* dId, double* dY, double* dErr, uint8_t* dFl, bool finalize, fg_result* out_dev) {
   RunArgs A; std::memset(&A, 0, sizeof(A));
   A.first = first; A.n = n; A.seed = seed; A.zin = zin; A.outI = dI; A.outId = dId; A.outY = dY; A.outErr = dErr; A.outFlags = dFl;
-  A.scratch = p->scratch;
+  A.scratch = p->scratch; A.phase_cycles = p->phase_cycles;
   int nparts = 0;
   if (mode != 2) {
     CU(cudaMemsetAsync(p->flag_count, 0, sizeof(unsigned long long), st));
@@ -518,7 +558,7 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
     nparts = p->grid_d;
   } else CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
   if (mode == 0 || mode == 2) {
-    RunArgs B = A; B.do_flag = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
+    RunArgs B = A; B.phase_cycles = nullptr; B.do_flag = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
     if (mode == 0) { B.idlist = p->flag_list; B.idcount = p->flag_count; }
     if (p->profile && mode == 2) { CU(cudaEventRecord(p->ev[0], st)); CU(cudaEventRecord(p->ev[1], st)); }
     fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, p->nt_q, p->smem_q, st>>>(p->D, B);

@@ -585,6 +585,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
   }
   P.d_geom_num_begin.assign(P.geoms.size() + 1, 0);
   int raw_max = 0;
+  std::map<std::vector<int>, std::array<long, 3>> hist;   // (mma, nf, k, qx, two) -> records, tiles, groups   (FG_PLAN_HIST=1 prints it)
   for (size_t i = 0; i < P.nums.size(); ++i) {
     HNum& N = P.nums[i]; FgNumDev d; std::memset(&d, 0, sizeof(d));
     d.geom = N.geom; d.op = N.op; d.ncomp = N.ncomp; d.nse = N.nse;
@@ -670,6 +671,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
           cur += tile_bytes; ++gn;
           N.exec_flops += 8.0 * (8.0 * steps + 4.0);
         }
+        { auto& h = hist[{1, r0.nf, r0.k, qx ? 1 : 0, 0}]; h[0] += R; h[1] += ntiles; h[2] += 1; }
         for (size_t t = i; t < j; ++t) N.algo_flops += std::max(0, N.recs[t].nf - 1);
         close_group();
         i = j; continue;
@@ -688,6 +690,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
         else { FgRecC h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)keep; std::memcpy(h.fidx, r.fidx, sizeof(h.fidx)); std::memcpy(h.vidx, r.vidx, sizeof(h.vidx)); h.cabs = cab; std::memcpy(&P.d_chunks[base + cur], &h, sizeof(h)); cur += sizeof(h); }
         std::memcpy(&P.d_chunks[base + cur], r.coef.data(), r.coef.size() * sizeof(double)); cur += r.coef.size() * sizeof(double);
         ++gn; prev = &r;
+        { auto& h = hist[{0, r.nf, r.k, (r.flags & FG_REC_QEXT) ? 1 : 0, (r.flags & FG_REC_TWO) ? 1 : 0}]; h[0] += 1; if (t == i) h[2] += 1; }
         const int nco = (r.flags & FG_REC_TWO) ? 2 : 1;
         N.exec_flops += std::max(0, r.nf - std::max(keep, 1)) + nco * (2.0 * ((1 << r.k) - 1) + 4.0) + ((r.flags & FG_REC_QEXT) ? r.k * (2.0 * ((1 << r.k) / 2 - 1) + 2.0) : 0.0);
         N.algo_flops += std::max(0, r.nf - std::max(keep, 1));
@@ -714,6 +717,10 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     FgTermDev d; std::memset(&d, 0, sizeof(d)); d.top = t.top; d.sign = t.sign; d.nmem = (int)t.geoms.size();
     for (int k = 0; k < d.nmem; ++k) d.geom[k] = t.geoms[k];
     P.d_terms.push_back(d);
+  }
+  if (std::getenv("FG_PLAN_HIST")) {
+    std::fprintf(stderr, "fg_plan: record classes (mma nf k qx two): records tiles runs\n");
+    for (auto& kv : hist) std::fprintf(stderr, "  %d %d %d %d %d : %ld %ld %ld\n", kv.first[0], kv.first[1], kv.first[2], kv.first[3], kv.first[4], kv.second[0], kv.second[1], kv.second[2]);
   }
   P.raw_slots = raw_max;
   // scratch per sample: [U,W per geom][raw value][raw abs][node value 2*NDEG][node abs 2*NDEG]

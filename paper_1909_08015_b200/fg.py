@@ -9,10 +9,10 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfg.so")
+LIB_PATH = os.environ.get("FG_LIB") or os.path.join(_HERE, "libfg.so")     # FG_LIB: a variant build (profiling counters)
 
 EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
-           "fg_plan_info", "fg_host_plan", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
+           "fg_plan_info", "fg_plan_phase_cycles", "fg_host_plan", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
            "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
 
@@ -73,6 +73,7 @@ def lib():
         L.fg_plan_profile.argtypes = [vp, C.c_int32]
         L.fg_plan_timing.argtypes = [vp, vp, vp]
         L.fg_plan_info.argtypes = [vp, C.POINTER(fg_plan_stats)]
+        L.fg_plan_phase_cycles.argtypes = [vp, vp, C.c_int32]
         L.fg_plan_structure.argtypes = [vp, vp, vp, C.c_int32]
         L.fg_plan_tables.argtypes = [vp, vp, vp]
         L.fg_integrate.argtypes = [vp, C.c_uint64, C.c_uint64, vp, C.POINTER(fg_result)]
@@ -171,6 +172,12 @@ class Plan:
         ms = np.zeros(3); n = np.zeros(1, dtype=np.int64)
         _check(lib().fg_plan_timing(self.h, _p(ms), _p(n)))
         return dict(ms_double=ms[0], ms_dd=ms[1], ms_reduce=ms[2], launches=int(n[0]))
+
+    def phase_cycles(self, reset=True):
+        """fg_plan_phase_cycles: (built_with_counters, warp-cycles per phase) of a -DFG_PHASE_PROF build."""
+        c = np.zeros(16, dtype=np.uint64)
+        rc = _check(lib().fg_plan_phase_cycles(self.h, _p(c), int(bool(reset))))
+        return bool(rc), c
 
     def structure(self):
         ns = self.stats["n_subgraphs"]
