@@ -119,7 +119,8 @@ typedef struct {
   double sum_y[2];        /* double-double (hi, lo) */
   double sum_y2[2];
   uint64_t n_samples;
-  uint64_t n_flagged;     /* samples re-evaluated in double-double */
+  uint64_t n_flagged;     /* samples re-evaluated in double-double (second rung) */
+  uint64_t n_flagged2;    /* of those: samples re-evaluated again in quad-double (third rung) */
   uint64_t n_rejected;    /* samples that contributed 0: degenerate point, non-finite value, or not resolved by the
                              double-double rung */
   uint64_t n_pdf_big_exp; /* samples whose pdf left the double range, kept as x*2^j */

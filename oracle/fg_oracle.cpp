@@ -43,6 +43,97 @@
 
 typedef __float128 quad;
 
+
+// ------------------------------------------------------------------------------------------
+// O11 (tool)  BF: plain binary floating point with a 256-bit significand, truncating arithmetic.
+// value = sign * (m[3] m[2] m[1] m[0])_2^64 * 2^(e - 256); normalised (top bit of m[3] set) or zero (sign == 0).
+// Used for the third, widest evaluation of a sample: it labels the points at which the __float128 value itself
+// is unreliable (cancellation beyond 113 bits) and serves as the reference there (the paper's ladder
+// ends at a 256-bit mantissa as well).  Every operation is exact up to one truncation of the result (relative error
+// < 2^-254); division is a Newton reciprocal (a few units of 2^-254).  Pinned against exact rational arithmetic in
+// tests/test_oracle_pins.py.
+// ------------------------------------------------------------------------------------------
+typedef unsigned __int128 u128;
+struct BF {
+  int sign; long e; uint64_t m[4];
+  BF() : sign(0), e(0) { m[0] = m[1] = m[2] = m[3] = 0; }
+  BF(double x) : sign(0), e(0) {
+    m[0] = m[1] = m[2] = m[3] = 0;
+    if (x == 0.0 || !std::isfinite(x)) return;
+    int ex; double f = std::frexp(std::fabs(x), &ex);          // f in [0.5, 1)
+    m[3] = (uint64_t)std::ldexp(f, 64); e = ex; sign = x < 0 ? -1 : 1;   // exact: 53 bits
+  }
+  explicit operator double() const {
+    if (!sign) return 0.0;
+    // round the top 64 bits to 53 (to nearest); the lower limbs only decide ties, which are of no consequence here
+    return sign * std::ldexp((double)m[3], (int)(e - 64));
+  }
+};
+static int bf_cmp_mag(const BF& a, const BF& b) {              // compares |a| and |b| (both non-zero)
+  if (a.e != b.e) return a.e < b.e ? -1 : 1;
+  for (int i = 3; i >= 0; --i) if (a.m[i] != b.m[i]) return a.m[i] < b.m[i] ? -1 : 1;
+  return 0;
+}
+static void bf_shr(uint64_t m[4], long d) {                    // m >>= d (truncating)
+  if (d >= 256) { m[0] = m[1] = m[2] = m[3] = 0; return; }
+  int w = (int)(d / 64), b = (int)(d % 64);
+  for (int i = 0; i < 4; ++i) {
+    uint64_t lo = (i + w < 4) ? m[i + w] : 0, hi = (i + w + 1 < 4) ? m[i + w + 1] : 0;
+    m[i] = b ? (lo >> b) | (hi << (64 - b)) : lo;
+  }
+}
+static void bf_normalise(BF& r) {                              // shift left until the top bit is set
+  if (!(r.m[0] | r.m[1] | r.m[2] | r.m[3])) { r.sign = 0; r.e = 0; return; }
+  while (!r.m[3]) { r.m[3] = r.m[2]; r.m[2] = r.m[1]; r.m[1] = r.m[0]; r.m[0] = 0; r.e -= 64; }
+  int z = __builtin_clzll(r.m[3]);
+  if (z) { r.m[3] = (r.m[3] << z) | (r.m[2] >> (64 - z)); r.m[2] = (r.m[2] << z) | (r.m[1] >> (64 - z)); r.m[1] = (r.m[1] << z) | (r.m[0] >> (64 - z)); r.m[0] <<= z; r.e -= z; }
+}
+static BF operator-(BF a) { a.sign = -a.sign; return a; }
+static BF operator+(const BF& a, const BF& b) {
+  if (!a.sign) return b;
+  if (!b.sign) return a;
+  const BF* x = &a; const BF* y = &b;
+  if (bf_cmp_mag(a, b) < 0) std::swap(x, y);                   // |x| >= |y|
+  BF r = *x; uint64_t t[4] = {y->m[0], y->m[1], y->m[2], y->m[3]};
+  bf_shr(t, x->e - y->e);
+  if (x->sign == y->sign) {
+    u128 c = 0;
+    for (int i = 0; i < 4; ++i) { c += (u128)r.m[i] + t[i]; r.m[i] = (uint64_t)c; c >>= 64; }
+    if (c) { bf_shr(r.m, 1); r.m[3] |= (uint64_t)1 << 63; r.e += 1; }
+  } else {
+    uint64_t br = 0;
+    for (int i = 0; i < 4; ++i) { u128 d = (u128)r.m[i] - t[i] - br; r.m[i] = (uint64_t)d; br = (uint64_t)(d >> 64) & 1; }
+    bf_normalise(r);
+  }
+  return r;
+}
+static BF operator-(const BF& a, const BF& b) { return a + (-b); }
+static BF operator*(const BF& a, const BF& b) {
+  BF r; if (!a.sign || !b.sign) return r;
+  uint64_t p[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (int i = 0; i < 4; ++i) {                                // schoolbook 4 x 4 limbs
+    u128 c = 0;
+    for (int j = 0; j < 4; ++j) { c += (u128)a.m[i] * b.m[j] + p[i + j]; p[i + j] = (uint64_t)c; c >>= 64; }
+    p[i + 4] = (uint64_t)c;
+  }
+  r.sign = a.sign * b.sign; r.e = a.e + b.e;
+  for (int i = 0; i < 4; ++i) r.m[i] = p[i + 4];               // top 256 bits (truncation)
+  if (!(r.m[3] >> 63)) { r.m[3] = (r.m[3] << 1) | (r.m[2] >> 63); r.m[2] = (r.m[2] << 1) | (r.m[1] >> 63); r.m[1] = (r.m[1] << 1) | (r.m[0] >> 63); r.m[0] = (r.m[0] << 1) | (p[3] >> 63); r.e -= 1; }
+  return r;
+}
+static BF operator/(const BF& a, const BF& b) {
+  if (!b.sign) { std::fprintf(stderr, "fg_oracle: BF division by zero\n"); std::abort(); }
+  // reciprocal of the significand f = b * 2^-e in [0.5, 1) by Newton: x <- x + x (1 - f x); 53 -> 106 -> 212 -> 424 bits
+  BF f = b; f.e = 0; f.sign = 1;
+  BF x(1.0 / (double)f), one(1.0);
+  for (int it = 0; it < 4; ++it) x = x + x * (one - f * x);
+  BF r = a * x; r.e -= b.e; if (r.sign) r.sign *= b.sign;
+  return r;
+}
+static BF& operator+=(BF& a, const BF& b) { a = a + b; return a; }
+static BF& operator-=(BF& a, const BF& b) { a = a - b; return a; }
+static BF& operator*=(BF& a, const BF& b) { a = a * b; return a; }
+
 // ------------------------------------------------------------------------------------------
 // O9  Philox4x32-10 (Salmon et al. 2011; named in PAPER.md:370)
 // ------------------------------------------------------------------------------------------
@@ -369,39 +460,45 @@ static void dirac_matching_table(const std::vector<Tok>& toks, int nslots, int n
   }
 }
 
-// the same coefficient for ONE pattern by explicit 4x4 matrices and explicit index sums
-// (slow; pins dirac_matching_table in tests)
+// the same coefficient for ONE pattern by explicit 4x4 Dirac matrices and explicit sums over the Lorentz index of every
+// chord (photon or Wick pair): Tr[F * string], the string read token by token, gamma^rho at the first end of a chord and
+// gamma_rho = g_rr gamma^rho at the second, gamma^0 at the unmatched slots of `tmask_slots`, gamma^nu at `qslot`.
+// No Clifford sign rules, no parity trick, no Walsh-Hadamard step: this pins dirac_matching_table (and, through the
+// tests, the planner's tables).  The recursion only shares the matrix product of the common prefix between index
+// assignments; 4^(chords) leaves.
+struct ExplicitRun {
+  const std::vector<Tok>* toks; std::vector<int> role; int qslot; uint32_t tmask; int nchord_ph; int ext, nu; Mat4 G[4]; std::vector<int> val;
+  cplx go(size_t pos, const Mat4& P, double metric) {
+    if (pos == toks->size()) return metric * mat_trace(P);
+    const Tok& tk = (*toks)[pos];
+    if (tk.kind == 1) return go(pos + 1, mat_mul(P, G[ext]), metric);
+    int chord;
+    if (tk.kind == 0) chord = tk.id;
+    else {
+      if (tk.id == qslot) return go(pos + 1, mat_mul(P, G[nu]), metric);
+      if (role[tk.id] < 0) return ((tmask >> tk.id) & 1) ? go(pos + 1, mat_mul(P, G[0]), metric) : go(pos + 1, P, metric);
+      chord = nchord_ph + role[tk.id];
+    }
+    if (val[chord] < 0) {
+      cplx s = 0;
+      for (int mu = 0; mu < 4; ++mu) { val[chord] = mu; s += go(pos + 1, mat_mul(P, G[mu]), metric); }
+      val[chord] = -1;
+      return s;
+    }
+    int mu = val[chord];
+    return go(pos + 1, mat_mul(P, G[mu]), metric * G_DIAG[mu]);
+  }
+};
 static double dirac_explicit(const std::vector<Tok>& toks, int nslots, int nchord_ph, const Matching& m,
                              int qslot, uint32_t tmask_slots, const std::vector<Piece>& pieces) {
-  std::vector<int> role(nslots, -1);
-  for (size_t k = 0; k < m.pairs.size(); ++k) { role[m.pairs[k][0]] = (int)k; role[m.pairs[k][1]] = (int)k; }
-  int nch = nchord_ph + (int)m.pairs.size();
-  Mat4 G[4]; for (int mu = 0; mu < 4; ++mu) G[mu] = mat_gamma(mu);
+  ExplicitRun R; R.toks = &toks; R.role.assign(nslots, -1); R.qslot = qslot; R.tmask = tmask_slots; R.nchord_ph = nchord_ph;
+  for (size_t k = 0; k < m.pairs.size(); ++k) { R.role[m.pairs[k][0]] = (int)k; R.role[m.pairs[k][1]] = (int)k; }
+  for (int mu = 0; mu < 4; ++mu) R.G[mu] = mat_gamma(mu);
   double total = 0;
   for (const Piece& pc : pieces) {
-    long nassign = 1; for (int k = 0; k < nch; ++k) nassign *= 4;
-    cplx sum = 0;
-    for (long as = 0; as < nassign; ++as) {
-      std::vector<int> val(nch); long t = as; for (int k = 0; k < nch; ++k) { val[k] = t & 3; t >>= 2; }
-      std::vector<int> seen(nch, 0);
-      Mat4 P = mat_identity(); double metric = 1;
-      for (int mu : pc.F) P = mat_mul(P, G[mu]);
-      for (const Tok& tk : toks) {
-        if (tk.kind == 1) { P = mat_mul(P, G[pc.ext]); continue; }
-        int chord = -1;
-        if (tk.kind == 0) chord = tk.id;
-        else {
-          if (tk.id == qslot) { P = mat_mul(P, G[pc.nu]); continue; }
-          if (role[tk.id] < 0) { if ((tmask_slots >> tk.id) & 1) P = mat_mul(P, G[0]); continue; }
-          chord = nchord_ph + role[tk.id];
-        }
-        P = mat_mul(P, G[val[chord]]);
-        if (seen[chord]) metric *= G_DIAG[val[chord]];
-        seen[chord] = 1;
-      }
-      sum += metric * mat_trace(P);
-    }
-    total += pc.w * sum.real();
+    R.ext = pc.ext; R.nu = pc.nu; R.val.assign(nchord_ph + m.pairs.size(), -1);
+    Mat4 P = mat_identity(); for (int mu : pc.F) P = mat_mul(P, R.G[mu]);
+    total += pc.w * R.go(0, P, 1.0).real();
   }
   return total;
 }
@@ -740,34 +837,41 @@ template <class T> static Poly<T> pmul(const Poly<T>& a, const Poly<T>& b) { Pol
 
 template <class T> struct GeomVal { T U, W; std::vector<T> A, Aq, beta; int ne; bool done = false; };
 
+// O5: Kirchhoff polynomials of one element at the line parameters z (indexed by global line id), by explicit
+// enumeration: U = sum over spanning trees of the product of the z of the lines NOT in the tree; U beta_ij = signed sum
+// over the spanning unicyclic subgraphs whose cycle holds i and j; A_j = 1 - sum_e z_e beta_je; W = sum z_j z_e beta_je;
+// A^q_j = xi^q_j/2 - sum_e z_e beta_je xi^q_e/2 (xi^q = -1 before the site of v_x, +1 after).  This one function serves
+// eval_point (every integrand value) and fgo_geom_eval (the matrix-tree pins).
+template <class T>
+static void geom_values(const ElemGeom& E, const T* z, GeomVal<T>& V) {
+  int ne = (int)E.own_e.size(); V.ne = ne;
+  auto zl = [&](int q) -> T { return q < ne ? z[E.own_e[q]] : z[E.own_ph[q - ne]]; };
+  T U = 0;
+  for (auto& S : E.Usets) { T p = 1; for (int q : S) p *= zl(q); U += p; }
+  std::vector<T> Ub(ne * ne, (T)0);
+  for (auto& bs : E.Bsets) { T p = 1; for (int q : bs.lines) p *= zl(q); for (auto& pr : bs.pairs) { if (pr[2] > 0) Ub[pr[0] * ne + pr[1]] += p; else Ub[pr[0] * ne + pr[1]] -= p; } }
+  V.U = U; V.beta.assign(ne * ne, (T)0);
+  for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) { T b = Ub[i * ne + j] / U; V.beta[i * ne + j] = b; V.beta[j * ne + i] = b; }
+  V.A.assign(ne, (T)0); V.Aq.assign(ne, (T)0);
+  // xi^q of own lines from the slots
+  std::vector<int> xiq(ne, 0); for (auto& s : E.slots) if (s.child < 0) xiq[s.own_e] = s.xiq;
+  T W = 0;
+  for (int j = 0; j < ne; ++j) {
+    T s = 0, sq = 0;
+    for (int e = 0; e < ne; ++e) { s += zl(e) * V.beta[j * ne + e]; sq += zl(e) * V.beta[j * ne + e] * (T)(0.5 * xiq[e]); }
+    V.A[j] = (T)1 - s; V.Aq[j] = (T)(0.5 * xiq[j]) - sq;
+    W += zl(j) * s;
+  }
+  V.W = W;
+}
+
 template <class T>
 T Oracle::eval_point(const T* zvars, double* dbg) const {
   int n = g.n;
   std::vector<T> z(3 * n);
   for (int v = 0; v < M; ++v) for (int id : var_lines[v]) z[id] = zvars[v] / (T)(double)var_lines[v].size();
   std::vector<GeomVal<T>> gv(geoms.size());
-  for (size_t gi = 0; gi < geoms.size(); ++gi) {
-    const ElemGeom& E = geoms[gi]; GeomVal<T>& V = gv[gi];
-    int ne = (int)E.own_e.size(); V.ne = ne;
-    auto zl = [&](int q) -> T { return q < ne ? z[E.own_e[q]] : z[E.own_ph[q - ne]]; };
-    T U = 0;
-    for (auto& S : E.Usets) { T p = 1; for (int q : S) p *= zl(q); U += p; }
-    std::vector<T> Ub(ne * ne, (T)0);
-    for (auto& bs : E.Bsets) { T p = 1; for (int q : bs.lines) p *= zl(q); for (auto& pr : bs.pairs) { if (pr[2] > 0) Ub[pr[0] * ne + pr[1]] += p; else Ub[pr[0] * ne + pr[1]] -= p; } }
-    V.U = U; V.beta.assign(ne * ne, (T)0);
-    for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) { T b = Ub[i * ne + j] / U; V.beta[i * ne + j] = b; V.beta[j * ne + i] = b; }
-    V.A.assign(ne, (T)0); V.Aq.assign(ne, (T)0);
-    // xi^q of own lines from the slots
-    std::vector<int> xiq(ne, 0); for (auto& s : E.slots) if (s.child < 0) xiq[s.own_e] = s.xiq;
-    T W = 0;
-    for (int j = 0; j < ne; ++j) {
-      T s = 0, sq = 0;
-      for (int e = 0; e < ne; ++e) { s += zl(e) * V.beta[j * ne + e]; sq += zl(e) * V.beta[j * ne + e] * (T)(0.5 * xiq[e]); }
-      V.A[j] = (T)1 - s; V.Aq[j] = (T)(0.5 * xiq[j]) - sq;
-      W += zl(j) * s;
-    }
-    V.W = W;
-  }
+  for (size_t gi = 0; gi < geoms.size(); ++gi) geom_values<T>(geoms[gi], z.data(), gv[gi]);
   // node values (children have smaller node ids than their parents)
   std::vector<std::array<Poly<T>, 2>> nv(nodes.size());
   for (size_t nd = 0; nd < nodes.size(); ++nd) {
@@ -987,37 +1091,32 @@ void fgo_tables(void* h, double* deg1, double* Z1) { Oracle* o = (Oracle*)h; siz
 
 // Kirchhoff debug: for geom gi at full-line z: U, W, and beta (ne x ne), A, Aq; returns ne
 int fgo_geom_eval(void* h, int gi, const double* zlines, double* U, double* W, double* beta, double* A, double* Aq,
-                  int* own_lines /* ne own_e ids then l own_ph ids */, int* nl_out, int* ends /* 2 per own line */, int* eta_rows_unused) {
-  Oracle* o = (Oracle*)h; (void)eta_rows_unused;
-  // evaluate through the generic path with merge disabled semantic: zlines are per LINE
-  Oracle tmp = *o; tmp.merge = 0; tmp.var_lines.clear(); for (int id = 0; id < 3 * o->g.n; ++id) tmp.var_lines.push_back({id}); tmp.M = 3 * o->g.n;
-  // replicate the geometry part of eval_point
-  const ElemGeom& E = tmp.geoms[gi]; int ne = (int)E.own_e.size();
-  auto zl = [&](int q) -> double { return q < ne ? zlines[E.own_e[q]] : zlines[E.own_ph[q - ne]]; };
-  double u = 0; for (auto& S : E.Usets) { double p = 1; for (int q : S) p *= zl(q); u += p; }
-  std::vector<double> Ub(ne * ne, 0.0);
-  for (auto& bs : E.Bsets) { double p = 1; for (int q : bs.lines) p *= zl(q); for (auto& pr : bs.pairs) Ub[pr[0] * ne + pr[1]] += pr[2] * p; }
-  for (int i = 0; i < ne; ++i) for (int j = i; j < ne; ++j) { beta[i * ne + j] = beta[j * ne + i] = Ub[i * ne + j] / u; }
-  std::vector<int> xiq(ne, 0); for (auto& s : E.slots) if (s.child < 0) xiq[s.own_e] = s.xiq;
-  double w = 0;
-  for (int j = 0; j < ne; ++j) { double s = 0, sq = 0; for (int e = 0; e < ne; ++e) { s += zl(e) * beta[j * ne + e]; sq += zl(e) * beta[j * ne + e] * 0.5 * xiq[e]; } A[j] = 1 - s; Aq[j] = 0.5 * xiq[j] - sq; w += zl(j) * s; }
-  *U = u; *W = w;
+                  int* own_lines /* ne own_e ids then l own_ph ids */, int* nl_out, int* ends /* 2 per own line */, int* xiq_out /* per own electron line, or NULL */) {
+  Oracle* o = (Oracle*)h;
+  const ElemGeom& E = o->geoms[gi]; int ne = (int)E.own_e.size();
+  GeomVal<double> V; geom_values<double>(E, zlines, V);      // the function eval_point uses
+  for (int i = 0; i < ne * ne; ++i) beta[i] = V.beta[i];
+  for (int j = 0; j < ne; ++j) { A[j] = V.A[j]; Aq[j] = V.Aq[j]; }
+  *U = V.U; *W = V.W;
   for (int q = 0; q < ne; ++q) own_lines[q] = E.own_e[q];
   for (size_t q = 0; q < E.own_ph.size(); ++q) own_lines[ne + q] = E.own_ph[q];
+  if (xiq_out) { for (int q = 0; q < ne; ++q) xiq_out[q] = 0; for (auto& sl : E.slots) if (sl.child < 0) xiq_out[sl.own_e] = sl.xiq; }
   *nl_out = (int)E.line_ends.size();
   for (size_t q = 0; q < E.line_ends.size(); ++q) { ends[2 * q] = E.line_ends[q][0]; ends[2 * q + 1] = E.line_ends[q][1]; }
   return ne;
 }
 
-// Dirac pin: max |fast - explicit| over up to `maxpat` patterns of every num of this oracle
+// Dirac pin: max |table - explicit| over about `maxpat_per_num` stored patterns of every num of this oracle, spread evenly
+// over its table (all numbers of pairs, q-slot patterns, both components of self-energy elements)
 double fgo_dirac_selfcheck(void* h, int maxpat_per_num, long* n_checked) {
   Oracle* o = (Oracle*)h; double worst = 0; long cnt = 0;
   for (auto& N : o->nums) {
     const ElemGeom& E = o->geoms[N.geom]; int st = o->subs[E.sub].type; int ns = (int)E.slots.size();
-    // also check a few zero coefficients: walk all (matching, T) for small cases
     long step = std::max<long>(1, (long)N.pats.size() / std::max(1, maxpat_per_num));
-    for (size_t k = 0; k < N.pats.size(); k += step) {
-      const Pattern& p = N.pats[k];
+    long npick = ((long)N.pats.size() + step - 1) / step;
+    #pragma omp parallel for schedule(dynamic, 1) reduction(max : worst) reduction(+ : cnt)
+    for (long i = 0; i < npick; ++i) {
+      const Pattern& p = N.pats[i * step];
       for (int comp = 0; comp < (st == 0 ? 2 : 1); ++comp) {
         auto pcs = pieces_for(N.op, st, comp, p.qslot >= 0, o->printed_projector);
         double e = dirac_explicit(E.toks, ns, E.l, E.matchings[p.match], p.qslot, p.tmask, pcs);
@@ -1026,6 +1125,25 @@ double fgo_dirac_selfcheck(void* h, int maxpat_per_num, long* n_checked) {
     }
   }
   if (n_checked) *n_checked = cnt; return worst;
+}
+
+// Description of element geometry gi: out = [a, b, type, nslots, l, nchildren, (a, b) of every child]; returns ints written.
+int fgo_geom_desc(void* h, int gi, int* out) {
+  Oracle* o = (Oracle*)h; const ElemGeom& E = o->geoms[gi]; const Sub& S = o->subs[E.sub];
+  int w = 0; out[w++] = S.a; out[w++] = S.b; out[w++] = S.type; out[w++] = (int)E.slots.size(); out[w++] = E.l; out[w++] = (int)E.children.size();
+  for (int c : E.children) { out[w++] = o->subs[c].a; out[w++] = o->subs[c].b; }
+  return w;
+}
+
+// One coefficient by explicit matrices for an ARBITRARY pattern of element gi (stored or not: zeros are checked too):
+// operator op, component comp (self-energy elements), Wick pairs (slot ids in string order), the slot that carries
+// gamma^nu (or -1), and the bit mask of unmatched slots that carry gamma^0.  Without the factor (-1/2)^pairs.
+double fgo_dirac_explicit(void* h, int gi, int op, int comp, int npairs, const int* pairs, int qslot, unsigned tmask) {
+  Oracle* o = (Oracle*)h; const ElemGeom& E = o->geoms[gi]; int st = o->subs[E.sub].type; int ns = (int)E.slots.size();
+  Matching m; std::vector<int> used(ns, 0);
+  for (int k = 0; k < npairs; ++k) { m.pairs.push_back({pairs[2 * k], pairs[2 * k + 1]}); used[pairs[2 * k]] = used[pairs[2 * k + 1]] = 1; }
+  for (int sl = 0; sl < ns; ++sl) if (!used[sl]) m.unmatched.push_back(sl);
+  return dirac_explicit(E.toks, ns, E.l, m, qslot, tmask, pieces_for(op, st, comp, qslot >= 0, o->printed_projector));
 }
 
 // integrand at n points (z over the M variables).  I_d: double evaluation; I_q: __float128 evaluation
@@ -1043,6 +1161,36 @@ void fgo_eval(void* h, const double* z, long n, double rel_tol, double abs_tol, 
   }
 }
 
+// Third evaluation (O11): the integrand in 256-bit arithmetic, rounded to double, and the relative distance of the
+// __float128 value from it, |I_q - I_w| / |I_w| (computed in 256 bits).  A point is "hard for the oracle's __float128"
+// when that distance exceeds the tolerance of a comparison; the 256-bit value is the reference there.
+void fgo_eval_wide(void* h, const double* z, long n, double* I_w, double* I_q, double* dist_q) {
+  Oracle* o = (Oracle*)h; int M = o->M;
+  #pragma omp parallel for schedule(dynamic, 4)
+  for (long i = 0; i < n; ++i) {
+    BF zw[16]; quad zq[16];
+    for (int v = 0; v < M; ++v) { zw[v] = BF(z[i * M + v]); zq[v] = (quad)z[i * M + v]; }
+    BF w = o->eval_point<BF>(zw, nullptr);
+    quad q = o->eval_point<quad>(zq, nullptr);
+    // q as BF: split the quad into two doubles (exact: 113 <= 53 + 53 + ...; the remainder after two pieces is kept too)
+    double q0 = (double)q; quad r1 = q - (quad)q0; double q1 = (double)r1; double q2 = (double)(r1 - (quad)q1);
+    BF qw = BF(q0) + BF(q1) + BF(q2);
+    BF diff = qw - w; diff.sign = diff.sign ? 1 : 0;
+    BF aw = w; aw.sign = aw.sign ? 1 : 0;
+    if (I_w) I_w[i] = (double)w;
+    if (I_q) I_q[i] = (double)q;
+    if (dist_q) dist_q[i] = aw.sign ? (double)(diff / aw) : (diff.sign ? INFINITY : 0.0);
+  }
+}
+
+// BF arithmetic pin: out = a op b with a = a0 + a1 + a2, b = b0 + b1 + b2 (exact sums of doubles), returned as three
+// doubles r0 + ... + r4 (successive roundings; together they carry the whole 256-bit result).
+void fgo_bf_op(int op, const double* a3, const double* b3, double* r3) {
+  BF a = BF(a3[0]) + BF(a3[1]) + BF(a3[2]), b = BF(b3[0]) + BF(b3[1]) + BF(b3[2]);
+  BF r = op == 0 ? a + b : op == 1 ? a - b : op == 2 ? a * b : a / b;
+  for (int k = 0; k < 5; ++k) { r3[k] = (double)r; r = r - BF(r3[k]); }
+}
+
 void fgo_sample(void* h, uint64_t seed, uint64_t first, long n, int32_t* comp, uint8_t* order, double* z, double* pdf_mant, int32_t* pdf_exp, uint8_t* bad) {
   Oracle* o = (Oracle*)h; int M = o->M;
   #pragma omp parallel for schedule(static)
@@ -1053,7 +1201,7 @@ void fgo_sample(void* h, uint64_t seed, uint64_t first, long n, int32_t* comp, u
   }
 }
 
-// O10 estimator over samples [first, first+n): y = I/g.  use_quad: y from the __float128 integrand.
+// O10 estimator over samples [first, first+n): y = I/g.  use_quad: 1 = y from the __float128 integrand, 2 = from the 256-bit one.
 // out: [sum_y, sum_y2, n_flagged, n_rejected, n_pdf_big_exp, mean, variance]
 void fgo_integrate(void* h, uint64_t seed, uint64_t first, long n, int use_quad, double rel_tol, double abs_tol, double* out) {
   Oracle* o = (Oracle*)h; int M = o->M;
@@ -1065,8 +1213,9 @@ void fgo_integrate(void* h, uint64_t seed, uint64_t first, long n, int use_quad,
     if (s.bad) { ++nrej; continue; }
     double d = o->eval_point<double>(s.z, nullptr), val = d;
     if (use_quad) {
-      quad zq[16]; for (int v = 0; v < M; ++v) zq[v] = (quad)s.z[v];
-      double q = (double)o->eval_point<quad>(zq, nullptr);
+      double q;
+      if (use_quad == 2) { BF zw[16]; for (int v = 0; v < M; ++v) zw[v] = BF(s.z[v]); q = (double)o->eval_point<BF>(zw, nullptr); }     // 256-bit reference
+      else { quad zq[16]; for (int v = 0; v < M; ++v) zq[v] = (quad)s.z[v]; q = (double)o->eval_point<quad>(zq, nullptr); }
       if (std::isfinite(q) && std::isfinite(d) && std::fabs(d - q) > std::max(rel_tol * std::fabs(q), abs_tol * std::ldexp(s.pdf_mant, s.pdf_exp))) ++nfl;
       val = q;
     }

@@ -41,10 +41,16 @@ def lib():
         L.fgo_sample.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_long] + [C.c_void_p] * 6
         L.fgo_integrate.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_long, C.c_int, C.c_double, C.c_double,
                                     C.c_void_p]
+        L.fgo_eval_wide.argtypes = [C.c_void_p, C.c_void_p, C.c_long, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.fgo_bf_op.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.fgo_geom_eval.restype = C.c_int
         L.fgo_geom_eval.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 10
         L.fgo_dirac_selfcheck.restype = C.c_double
         L.fgo_dirac_selfcheck.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.fgo_geom_desc.restype = C.c_int
+        L.fgo_geom_desc.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.fgo_dirac_explicit.restype = C.c_double
+        L.fgo_dirac_explicit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_uint]
         L.fgo_u01.restype = C.c_double
         L.fgo_u01.argtypes = [C.c_uint32, C.c_uint32]
         L.fgo_enumerate.argtypes = [C.c_int, C.c_void_p, C.c_int]
@@ -135,6 +141,15 @@ class Oracle:
         lib().fgo_eval(self.h, _p(z), n, rel_tol, abs_tol, int(quad), _p(Id), _p(Iq), _p(fl), _p(td))
         return (Id, Iq, fl, td) if terms else (Id, Iq, fl)
 
+    def eval_wide(self, z):
+        """(I_w, I_q, dist): integrand in 256-bit arithmetic and in __float128 (both rounded to double) and the relative
+        distance |I_q - I_w| / |I_w| of the two."""
+        z = np.ascontiguousarray(z, dtype=np.float64).reshape(-1, self.M)
+        n = len(z)
+        Iw = np.zeros(n); Iq = np.zeros(n); dist = np.zeros(n)
+        lib().fgo_eval_wide(self.h, _p(z), n, _p(Iw), _p(Iq), _p(dist))
+        return Iw, Iq, dist
+
     def sample(self, seed, first, n):
         M = self.M
         comp = np.zeros(n, dtype=np.int32); order = np.zeros((n, M), dtype=np.uint8); z = np.zeros((n, M))
@@ -142,9 +157,10 @@ class Oracle:
         lib().fgo_sample(self.h, seed, first, n, _p(comp), _p(order), _p(z), _p(pm), _p(pe), _p(bad))
         return dict(comp=comp, order=order, z=z, pdf_mant=pm, pdf_exp=pe, bad=bad)
 
-    def integrate(self, seed, first, n, quad=False, rel_tol=1e-12, abs_tol=0.0):
+    def integrate(self, seed, first, n, quad=False, rel_tol=1e-12, abs_tol=0.0, wide=False):
+        """quad: y from the __float128 integrand; wide: from the 256-bit one (the reference at ill-conditioned points)."""
         out = np.zeros(8)
-        lib().fgo_integrate(self.h, seed, first, n, int(quad), rel_tol, abs_tol, _p(out))
+        lib().fgo_integrate(self.h, seed, first, n, 2 if wide else int(quad), rel_tol, abs_tol, _p(out))
         return dict(sum_y=out[0], sum_y2=out[1], n_flagged=int(out[2]), n_rejected=int(out[3]), n_pdf_big_exp=int(out[4]),
                     mean=out[5], variance=out[6], n_samples=n)
 
@@ -152,15 +168,34 @@ class Oracle:
         zl = np.ascontiguousarray(zlines, dtype=np.float64)
         U = np.zeros(1); W = np.zeros(1); beta = np.zeros(400); A = np.zeros(20); Aq = np.zeros(20)
         own = np.zeros(40, dtype=np.int32); nl = np.zeros(1, dtype=np.int32); ends = np.zeros(80, dtype=np.int32)
-        ne = lib().fgo_geom_eval(self.h, gi, _p(zl), _p(U), _p(W), _p(beta), _p(A), _p(Aq), _p(own), _p(nl), _p(ends), None)
+        xiq = np.zeros(20, dtype=np.int32)
+        ne = lib().fgo_geom_eval(self.h, gi, _p(zl), _p(U), _p(W), _p(beta), _p(A), _p(Aq), _p(own), _p(nl), _p(ends), _p(xiq))
         nlines = int(nl[0])
-        return dict(ne=ne, U=U[0], W=W[0], beta=beta[:ne * ne].reshape(ne, ne).copy(), A=A[:ne].copy(), Aq=Aq[:ne].copy(),
+        return dict(ne=ne, U=U[0], W=W[0], beta=beta[:ne * ne].reshape(ne, ne).copy(), A=A[:ne].copy(), Aq=Aq[:ne].copy(), xiq=xiq[:ne].copy(),
                     own=own[:nlines].copy(), ends=ends[:2 * nlines].reshape(nlines, 2).copy())
+
+    def geom_desc(self, gi):
+        buf = np.zeros(64, dtype=np.int32)
+        w = lib().fgo_geom_desc(self.h, gi, _p(buf))
+        return dict(a=int(buf[0]), b=int(buf[1]), type=int(buf[2]), nslots=int(buf[3]), l=int(buf[4]),
+                    children=[(int(buf[6 + 2 * k]), int(buf[7 + 2 * k])) for k in range(int(buf[5]))])
+
+    def dirac_explicit(self, gi, op, comp, pairs, qslot, tmask):
+        """Coefficient of one pattern of element gi from explicit 4x4 matrices (without (-1/2)^pairs)."""
+        pr = np.asarray(pairs, dtype=np.int32).reshape(-1)
+        return lib().fgo_dirac_explicit(self.h, gi, int(op), int(comp), len(pr) // 2, _p(pr), int(qslot), int(tmask))
 
     def dirac_selfcheck(self, maxpat=50):
         cnt = np.zeros(1, dtype=np.int64)
         w = lib().fgo_dirac_selfcheck(self.h, maxpat, _p(cnt))
         return w, int(cnt[0])
+
+
+def bf_op(op, a3, b3):
+    """The oracle's 256-bit arithmetic on a = sum(a3), b = sum(b3): op 0 +, 1 -, 2 *, 3 /; result as five doubles."""
+    a = np.asarray(a3, dtype=np.float64); b = np.asarray(b3, dtype=np.float64); r = np.zeros(5)
+    lib().fgo_bf_op(int(op), _p(a), _p(b), _p(r))
+    return r
 
 
 def threads():

@@ -236,11 +236,10 @@ template <class T, int S, int K, bool AC = false, bool RC = false> struct QExt {
 };
 template <class T, int S, bool AC, bool RC> struct QExt<T, S, 0, AC, RC> { static FG_HD void run(const double*, const T (*)[S], const T (*)[S], T*) {} };
 
-// Running state of one program: accumulators of the current destination.
-// part: per-lane DMMA partial sums.  split = w (0 = off, else 2..32): groups of w adjacent lanes evaluate the SAME point
+// Running state of one program: accumulators of the current destination.  split = w (0 = off, else 2..32): groups of w adjacent lanes evaluate the SAME point
 // and share its records out (record i goes to lane i % w); their partial sums are added when a destination is finished
 // (short double-double queues).
-template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; double part[8]; int cur, has_part, split, rr;
+template <class T, int S> struct RecState { T acc[2][S]; double aab[2][S]; int cur, split, rr;
 #ifdef FG_PHASE_PROF
   long long* prof; long long tlast;
 #endif
@@ -480,155 +479,17 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
     const int t = q >> 3, n = q & 7;
     const unsigned char* pt = p + (size_t)t * tile_bytes;
     const FgRecM* recs = (const FgRecM*)pt; const FgMmaCoef* __restrict__ fr = (const FgMmaCoef*)(pt + 8 * sizeof(FgRecM));
-    const double cab = (double)recs[n].cabs;
+    const double cab = fg_cab16_value(recs[n].cab16);
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       T qv = T(0.0); double qa = 0.0;
-      for (int J = 0; J < 4 * steps; ++J) { const double c = (double)fr[(J >> 2) * 32 + n * 4 + (J & 3)]; qv = qv + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
+      for (int J = 0; J < 4 * steps; ++J) { const double c = fg_mma_coef_value(fr[(J >> 2) * 32 + n * 4 + (J & 3)]); qv = qv + mono[s][J] * T(c); if (ABS == 2) qa += monoa[s][J] * fabs(c); }
       T bp = T(1.0); for (int f = 0; f < nf; ++f) bp = bp * Vt[(int)recs[n].fidx[f] * vs + s];
       st.acc[0][s] = st.acc[0][s] + bp * qv;
       if (ABS == 1) st.aab[0][s] = fma(t_abs_d(bp), cab, st.aab[0][s]);
       if (ABS == 2) st.aab[0][s] = fma(t_abs_d(bp), qa, st.aab[0][s]);
     }
   }
-}
-
-#if defined(__CUDACC__)
-// Tensor-core path of a group (double pass, one sample per thread, whole warp converged).  DMMA m8n8k4:
-//   A (8 samples x 4 monomials): lane (r = lane/4, c = lane%4) holds monomial 4*step + c of sample 8*b + r;
-//   B (4 monomials x 8 records): lane holds coef[4*step + c] of record r -> one conflict-free LDS.32 per step (float, exact);
-//   D (8 x 8): lane holds records 2c, 2c+1 of sample 8*b + r.
-// Each lane then weights its two record values with their products of beta's and keeps per-lane partial sums for the four
-// row blocks b; out[0..3] = value partials, out[4..7] = |.| partials (reduced over the quad by the caller).
-__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
-// NT2 (1 or 2) consecutive tiles share the monomials (A fragments) of a row block: the loads of a, a^q and the monomial
-// products are paid once per 8 or 16 records.
-template <int NF, int K, bool QX, int NT2>
-__device__ __forceinline__ void mma_tiles(const unsigned char* __restrict__ p, const double* __restrict__ Vw, int vs, int lane, int r, int c,
-                                          int v0, int v1, int v2, int v3, int vq, double* acc, double* aab, double (*pf)[NF > 0 ? NF : 1]) {
-  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS);
-  double B[NT2][STEPS], cab[NT2][2]; int ff[NT2][2][NF > 0 ? NF : 1], keep[NT2][2];
-#pragma unroll
-  for (int u = 0; u < NT2; ++u) {
-    const unsigned char* pt = p + u * TILE;
-#pragma unroll
-    for (int st = 0; st < STEPS; ++st) B[u][st] = (double)((const FgMmaCoef*)(pt + 8 * sizeof(FgRecM)))[st * 32 + lane];
-#pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      const uint4 h = *(const uint4*)(pt + (2 * c + e) * 16);
-      cab[u][e] = (double)__uint_as_float(h.w); keep[u][e] = (int)((h.y >> 8) & 255u);
-#pragma unroll
-      for (int i = 0; i < NF; ++i) ff[u][e][i] = (int)((i < 4 ? (h.x >> (8 * i)) : h.y) & 255u) * vs;
-    }
-  }
-#pragma unroll
-  for (int b = 0; b < 4; ++b) {
-    const double* __restrict__ Vs = Vw + 8 * b + r;
-    const double a0 = Vs[v0], a1 = Vs[v1];
-    const double a2 = K > 2 ? Vs[v2] : 1.0, a3 = K > 3 ? Vs[v3] : 1.0;
-    const double a01 = a0 * a1;
-    const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
-    double hi[NM]; hi[0] = 1.0;
-    if (K > 2) hi[1] = a2;
-    if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
-    double d[NT2][2];
-#pragma unroll
-    for (int u = 0; u < NT2; ++u) { d[u][0] = 0.0; d[u][1] = 0.0; dmma884(d[u][0], d[u][1], mlo, B[u][0]); }
-#pragma unroll
-    for (int tt = 1; tt < NM; ++tt) {
-      const double m = mlo * hi[tt];
-#pragma unroll
-      for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], m, B[u][tt]);
-    }
-    if (QX) {
-      const double q0 = Vs[v0 + vq], q1 = Vs[v1 + vq];
-      const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
-#pragma unroll
-      for (int tt = 0; tt < NM; ++tt) {
-        const double m = tt ? mq * hi[tt] : mq;
-#pragma unroll
-        for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], m, B[u][NM + tt]);
-      }
-      if (K == 3) {
-        const double m = mlo * Vs[v2 + vq];
-#pragma unroll
-        for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], m, B[u][2 * NM]);
-      }
-      if (K == 4) {
-        const double m2 = mlo * Vs[v2 + vq], m3 = mlo * Vs[v3 + vq];
-        const double mm[4] = {m2, m2 * a3, m3, m3 * a2};
-#pragma unroll
-        for (int tt = 0; tt < 4; ++tt) {
-#pragma unroll
-          for (int u = 0; u < NT2; ++u) dmma884(d[u][0], d[u][1], mm[tt], B[u][2 * NM + tt]);
-        }
-      }
-    }
-    // products of beta's of this lane's records (tile by tile, slot by slot: the lane's depth-first stretch); the prefix
-    // stack of the row block survives from record to record
-#pragma unroll
-    for (int u = 0; u < NT2; ++u) {
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        double bp = 1.0;
-        if (NF > 0) {
-#pragma unroll
-          for (int i = 0; i < NF; ++i) if (i >= keep[u][e]) pf[b][i] = (i == 0) ? Vs[ff[u][e][i]] : pf[b][i > 0 ? i - 1 : 0] * Vs[ff[u][e][i]];
-          bp = pf[b][NF > 0 ? NF - 1 : 0];
-        }
-        acc[b] = fma(bp, d[u][e], acc[b]); aab[b] = fma(fabs(bp), cab[u][e], aab[b]);
-      }
-    }
-  }
-}
-
-template <int NF, int K, bool QX>
-__device__ __noinline__ void run_group_mma_fast(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int vs, int ne, double* __restrict__ out) {
-  __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
-  constexpr int STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS);
-  const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
-  const int vq = ne * vs;
-  double acc[4], aab[4], pf[4][NF > 0 ? NF : 1];
-#pragma unroll
-  for (int b = 0; b < 4; ++b) { acc[b] = out[b]; aab[b] = out[4 + b]; }
-  for (int g = 0; g < nseq; ++g) {       // consecutive groups of this class (same destination), each with its own free variables
-    const uint4 gw = *(const uint4*)p; p += sizeof(FgGroupHdr);
-    const int ntiles = (int)(gw.x & 0xffffu);
-    const int v0 = (int)((gw.y >> 16) & 255u) * vs, v1 = (int)(gw.y >> 24) * vs, v2 = (int)(gw.z & 255u) * vs, v3 = (int)((gw.z >> 8) & 255u) * vs;
-#pragma unroll
-    for (int b = 0; b < 4; ++b) for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[b][i] = 1.0;
-    int t = 0;
-    for (; t + 2 <= ntiles; t += 2, p += 2 * TILE) mma_tiles<NF, K, QX, 2>(p, Vw, vs, lane, r, c, v0, v1, v2, v3, vq, acc, aab, pf);
-    if (t < ntiles) { mma_tiles<NF, K, QX, 1>(p, Vw, vs, lane, r, c, v0, v1, v2, v3, vq, acc, aab, pf); p += TILE; }
-  }
-#pragma unroll
-  for (int b = 0; b < 4; ++b) { out[b] = acc[b]; out[4 + b] = aab[b]; }
-}
-#endif
-
-// Fold the per-lane DMMA partial sums into the accumulators of the owning threads: quad-reduce, then lane L takes the
-// sums of its own sample from lane 4*(L%8), row block L/8.  Called when the destination changes.
-template <class T, int S>
-FG_HD void fold_mma_partials(RecState<T, S>& st) {
-#if defined(__CUDA_ARCH__)
-  if constexpr (!is_dd<T>::value && S == 1) {
-    if (st.has_part) {
-      const int lane = threadIdx.x & 31, src = (lane & 7) << 2, myb = lane >> 3;
-      double mv = 0.0, ma = 0.0;
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        double v = st.part[b], w = st.part[4 + b];
-        v += __shfl_xor_sync(0xffffffffu, v, 1); w += __shfl_xor_sync(0xffffffffu, w, 1);
-        v += __shfl_xor_sync(0xffffffffu, v, 2); w += __shfl_xor_sync(0xffffffffu, w, 2);
-        v = __shfl_sync(0xffffffffu, v, src); w = __shfl_sync(0xffffffffu, w, src);
-        if (b == myb) { mv = v; ma = w; }
-      }
-      st.acc[0][0] = st.acc[0][0] + T(mv); st.aab[0][0] += ma; st.has_part = 0;
-    }
-  }
-#endif
 }
 
 // All groups of one chunk.  flush(dst, acc, aab) stores the finished accumulators of a destination.
@@ -645,14 +506,13 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
     const FgGroupHdr gh = *(const FgGroupHdr*)p; p += sizeof(FgGroupHdr);
     const int nrec = gh.nrec, nf = gh.nf, k = gh.k, flags = gh.flags;
     if ((int)gh.dst != st.cur) {
-      fold_mma_partials(st);
       if (st.cur >= 0) { fold_split(st); flush(st.cur, st.acc, st.aab); }
       st.cur = gh.dst;
 #pragma unroll
       for (int s = 0; s < S; ++s) { st.acc[0][s] = T(0.0); st.acc[1][s] = T(0.0); st.aab[0][s] = 0.0; st.aab[1][s] = 0.0; }
     }
     bool done = false;
-    if constexpr (!is_dd<T>::value && ABS != 2) {
+    if constexpr (!is_dd<T>::value && ABS != 2) {      // (host harness; the device's double pass has its own chunk loop, fg_stream.cuh)
       if (!(flags & (FG_REC_WIDE | FG_REC_TWO | FG_REC_MMA))) {
         done = true;
         const bool qx = (flags & FG_REC_QEXT) != 0;
@@ -671,25 +531,6 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
       }
     }
     if (flags & FG_REC_MMA) {
-#if defined(__CUDA_ARCH__)
-      if constexpr (!is_dd<T>::value && ABS == 1 && S == 1) {
-        done = true;
-        if (!st.has_part) { st.has_part = 1; for (int b = 0; b < 8; ++b) st.part[b] = 0.0; }
-        const double* Vw = (const double*)Vt - (threadIdx.x & 31);
-        const bool qx = (flags & FG_REC_QEXT) != 0;
-        // consecutive tensor-core groups of the same class and destination are run by one call (run length and size
-        // come from the planner)
-        const unsigned char* p0 = p - sizeof(FgGroupHdr); const int nseq = gh.nseq; const unsigned char* pe = p0 + gh.seq_bytes;
-        switch (nf * 8 + k) {
-#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_fast<NF, K, true>(p0, nseq, Vw, vs, ne, st.part); else run_group_mma_fast<NF, K, false>(p0, nseq, Vw, vs, ne, st.part); break;
-          FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
-          FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
-#undef FG_MM
-          default: done = false; break;
-        }
-        if (done) { FG_MARK(st, 2); p = pe; g += nseq - 1; continue; }
-      }
-#endif
       if (!done) run_group_mma_dyn<T, S, ABS>(p, nrec, nf, k, flags, gh.vidx, Vt, vs, ne, st);
       FG_MARK(st, 4);
       p += nrec * FG_TILE_BYTES(mma_steps(k, (flags & FG_REC_QEXT) != 0));

@@ -1,13 +1,17 @@
 // fg_kernels.cu — sm_100a kernels of the hot path and the C ABI (include/fg.h).
 //
-// One persistent launch per precision rung (blocks of samples, deferred higher-precision passes):
-//   fg_eval_kernel<double>  draws a sample per Philox counter, evaluates every forest term, estimates the round-off
-//                           error, queues ill-conditioned samples, accumulates y = I/g in compensated FP64;
-//   fg_eval_kernel<dd>      re-evaluates the queued samples in double-double;
+// Launches per slab of samples (blocks of samples, deferred higher-precision passes):
+//   fg_geom_kernel<L>       a1-a5 for a wave of samples: Philox, Hepp-sector sample + pdf, element geometry (double-double
+//                           inside, rounded once) -> operand tables V (beta, A, A^q), U, W per element in HBM;
+//   fg_stream_kernel        a6-a10 of the double-precision pass: persistent, one block of 512 threads per SM serves batches
+//                           of 256 samples; V of one element comes in by bulk TMA, the numerator record stream runs on the
+//                           FP64 tensor path (fg_stream.cuh), then node products, forest sum, round-off estimate, queueing
+//                           of ill-conditioned samples, y = I/g in compensated FP64;
+//   fg_eval_kernel<dd|qd>   re-evaluates the queued samples in double-double, then quad-double (whole path in one kernel);
 //   fg_reduce_kernel        folds the per-block partial sums in a fixed order (deterministic).
 // The numerator coefficient stream is block-uniform: it is pulled through a two-stage shared-memory ring with
 // 1-D bulk TMA copies (cp.async.bulk + mbarrier) while the FP64 pipe works on the previous chunk.  Per-sample
-// operands (beta, A, A^q) live in shared memory, per-sample polynomials in an L2-resident scratch.
+// operands (beta, A, A^q) live in shared memory, per-sample polynomials in a per-block scratch.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -20,6 +24,7 @@
 #include "../../include/fg.h"
 #include "fg_core.cuh"
 #include "fg_plan.hpp"
+#include "fg_stream.cuh"
 
 namespace fg {
 
@@ -33,9 +38,15 @@ struct RunArgs {
   double* partials;                                            // [gridDim.x][8]
   void* scratch;
   unsigned long long* phase_cycles;                            // [16] profiling build only (FG_PHASE_PROF), else NULL
+  // wave of the double-precision pass: ordinals [ord0, ord0 + nb * FG_ST_SAMPLES) of the slab, tables written by fg_geom_kernel
+  uint64_t ord0; int nb;
+  double* gV;      // [nb][vtot][FG_ST_VS]   operand tables of all element geometries
+  double* gUW;     // [nb][2 * ngeom][FG_ST_SAMPLES]
+  double* gMisc;   // [nb][FG_GM_ROWS][FG_ST_SAMPLES]: pdf mantissa, pdf exponent, state, z of the merged variable, amax, amp
 };
+enum { FG_GM_MANT = 0, FG_GM_EX, FG_GM_STATE, FG_GM_ZM, FG_GM_AMAX, FG_GM_AMP, FG_GM_ROWS };
 
-struct Accum { double sy[2], sy2[2]; unsigned long long nflag, nrej, nbig, n; };
+struct Accum { double sy[2], sy2[2]; unsigned long long nflag, nflag2, nrej, nbig, n; };
 
 // ---- mbarrier / bulk-copy helpers (sm_90+ PTX; SASS: UBLKCP, SYNCS) -------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -71,7 +82,7 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     mbar_expect_tx(&ring.bar[0], used[0]); bulk_g2s(ring.buf, g0, used[0], &ring.bar[0]);
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
   }
-  RecState<T, S> st; st.cur = -1; st.has_part = 0; st.split = split; st.rr = 0;
+  RecState<T, S> st; st.cur = -1; st.split = split; st.rr = 0;
 #ifdef FG_PHASE_PROF
   st.prof = ring.prof; st.tlast = ring.tlast;
 #endif
@@ -92,7 +103,6 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
     FG_MARK(st, 5);
     if (threadIdx.x == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], used[ch + 2]); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, used[ch + 2], &ring.bar[b]); }
   }
-  fold_mma_partials(st);
   if (st.cur >= 0) { fold_split(st); flush(st.cur, st.acc, st.aab); }
   FG_MARK(st, 8);
 #ifdef FG_PHASE_PROF
@@ -142,7 +152,63 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
   }
 }
 
+
+// Precision rungs.  unit: round-off unit of the running error estimate K * u * sum|terms|;
+// geom_unit: relative error of the geometry step per unit of its conditioning `amp`.
+template <class T> struct prec;
+template <> struct prec<double> { static const int rung = 0; static __device__ double unit(double e, double af) { return e * af; } static __device__ double geom_unit() { return 0x1p-109; } };
+template <> struct prec<dd> { static const int rung = 1; static __device__ double unit(double e, double) { return e * 0x1p-51; } static __device__ double geom_unit() { return 0x1p-109; } };
+
+// a8-a9 for one sample: round-off estimate against the tolerance, queueing / rejection, y = I/g, compensated sums
+struct TailAcc { dd sy, sy2; unsigned long long nflag, nrej, nbig; };
+template <class T>
+__device__ __forceinline__ void sample_tail(const FgPlanDev& P, const RunArgs& A, T I, double Iabs, double growth, double amp, double mant, int ex, bool bad, uint64_t oid, TailAcc& ta) {
+  const double Id = to_double(I);
+  double af = growth * growth; af = af * af * af;      // |A|, |A^q| <= 1 is assumed by cabs; amax^6 otherwise
+  // running error estimate: K * u * sum|terms| with u = 2^-53 (double pass), 2^-104 (double-double) or 2^-205 (quad-double)
+  // plus the conditioning of the geometry step (double-double, or quad-double in the last rung), DESIGN.md "precision"
+  const double err = (prec<T>::unit(P.err_eps, af) + amp * prec<T>::geom_unit()) * Iabs;
+  uint8_t fl = 0; double y = 0.0;
+  if (!A.idlist && (ex > 1023 || ex < -1021)) ++ta.nbig;
+  if (bad) { ++ta.nrej; fl = 2; }
+  else {
+    const double tol = fmax(P.rel_tol * fabs(Id), ldexp(P.abs_tol * mant, ex));
+    const bool over = !(err <= tol);
+    if (over && A.do_flag) {
+      fl = prec<T>::rung == 0 ? 1 : 8; ++ta.nflag;          // queued for the next rung
+      if (A.flag_list) { const unsigned long long pos = atomicAdd(A.flag_count, 1ull); A.flag_list[pos] = (uint32_t)oid; }
+    } else if (over && prec<T>::rung > 0) {
+      fl = 4; ++ta.nrej;     // not resolved by the last rung: contributes 0 and is counted
+    } else {
+      const T yq = I / T(mant);
+      y = ldexp(to_double(yq), -ex);
+      if (!isfinite(y)) { ++ta.nrej; fl |= 2; y = 0.0; }
+      else { ta.sy = dd_add_d(ta.sy, y); ta.sy2 = ta.sy2 + two_prod(y, y); }
+    }
+  }
+  if (A.outI) A.outI[oid] = Id;
+  if (A.outId && prec<T>::rung == 0) A.outId[oid] = Id;
+  if (A.outY) A.outY[oid] = y;
+  if (A.outErr && (prec<T>::rung == 0 || !A.idlist)) A.outErr[oid] = err;
+  if (A.outFlags) A.outFlags[oid] = prec<T>::rung > 0 ? (uint8_t)(A.outFlags[oid] | fl) : fl;
+}
+
 __device__ __forceinline__ dd shfl_dd(dd v, int off) { return dd(__shfl_down_sync(0xffffffffu, v.hi, off), __shfl_down_sync(0xffffffffu, v.lo, off)); }
+
+// a10: warp shuffle -> block -> one partial per block (added to what the block left there in earlier waves of the slab)
+__device__ __forceinline__ void block_reduce_tail(TailAcc& ta, double* red /* shared, 8 doubles per warp */, double* partial, int flag_slot) {
+  const int tid = threadIdx.x, nw = blockDim.x >> 5;
+  double cnt[3] = {(double)ta.nflag, (double)ta.nrej, (double)ta.nbig};
+  for (int off = 16; off > 0; off >>= 1) { ta.sy = ta.sy + shfl_dd(ta.sy, off); ta.sy2 = ta.sy2 + shfl_dd(ta.sy2, off); for (int k = 0; k < 3; ++k) cnt[k] += __shfl_down_sync(0xffffffffu, cnt[k], off); }
+  __syncthreads();
+  if ((tid & 31) == 0) { double* r = red + (tid >> 5) * 8; r[0] = ta.sy.hi; r[1] = ta.sy.lo; r[2] = ta.sy2.hi; r[3] = ta.sy2.lo; r[4] = cnt[0]; r[5] = cnt[1]; r[6] = cnt[2]; }
+  __syncthreads();
+  if (tid == 0) {
+    dd a(partial[0], partial[1]), b(partial[2], partial[3]); double c[3] = {0.0, partial[5], partial[6]};
+    for (int w = 0; w < nw; ++w) { const double* r = red + w * 8; a = a + dd(r[0], r[1]); b = b + dd(r[2], r[3]); for (int k = 0; k < 3; ++k) c[k] += r[4 + k]; }
+    partial[0] = a.hi; partial[1] = a.lo; partial[2] = b.hi; partial[3] = b.lo; partial[flag_slot] += c[0]; partial[5] = c[1]; partial[6] = c[2];   // slot 4: queued for double-double, 7: for quad-double
+  }
+}
 
 template <class T, int S, int MAXNT>
 __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const RunArgs A) {
@@ -169,7 +235,7 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
     for (int w = 2; w <= 32; w <<= 1) { const double c = ceil((double)nwork * w / cap) * (0.115 + 0.885 / w); if (c < best) { best = c; split = w; } }
   }
   const uint64_t per_batch = split ? (uint64_t)(NT / split) : (uint64_t)NT * S, nbatch = (nwork + per_batch - 1) / per_batch;
-  dd sy(0.0), sy2(0.0); unsigned long long nflag = 0, nrej = 0, nbig = 0;
+  TailAcc ta; ta.sy = dd(0.0); ta.sy2 = dd(0.0); ta.nflag = ta.nrej = ta.nbig = 0;
   const int M = P.M;
   for (uint64_t batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
     double z[S][FG_MAXM], mant[S]; int ex[S]; bool valid[S], bad[S]; uint64_t oid[S];
@@ -194,69 +260,173 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       if (!valid[s] || (split && (tid & (split - 1)) != 0)) continue;
-      const double Id = to_double(I[s]);
-      double af = growth[s] * growth[s]; af = af * af * af;      // |A|, |A^q| <= 1 is assumed by cabs; amax^6 otherwise
-      // running error estimate: K * u * sum|terms| with u = 2^-53 (double pass) or 2^-104 (double-double pass)
-      // plus the conditioning of the (always double-double) geometry step, amp * 2^-104 / 32
-      const double err = ((is_dd<T>::value ? P.err_eps * 0x1p-51 : P.err_eps * af) + amp[s] * 0x1p-109) * Iabs[s];
-      uint8_t fl = 0; double y = 0.0;
-      if (!A.idlist && (ex[s] > 1023 || ex[s] < -1021)) ++nbig;
-      if (bad[s]) { ++nrej; fl = 2; }
-      else {
-        const double tol = fmax(P.rel_tol * fabs(Id), ldexp(P.abs_tol * mant[s], ex[s]));
-        const bool over = !(err <= tol);
-        if (!is_dd<T>::value && A.do_flag && over) {
-          fl = 1; ++nflag;
-          if (A.flag_list) { const unsigned long long pos = atomicAdd(A.flag_count, 1ull); A.flag_list[pos] = (uint32_t)oid[s]; }
-        } else if (is_dd<T>::value && over) {
-          fl = 4; ++nrej;     // not resolved by the last rung: contributes 0 and is counted
-        } else {
-          const T yq = I[s] / T(mant[s]);
-          y = ldexp(to_double(yq), -ex[s]);
-          if (!isfinite(y)) { ++nrej; fl |= 2; y = 0.0; }
-          else { sy = dd_add_d(sy, y); sy2 = sy2 + two_prod(y, y); }
-        }
-      }
-      if (A.outI) A.outI[oid[s]] = Id;
-      if (A.outId) A.outId[oid[s]] = Id;
-      if (A.outY) A.outY[oid[s]] = y;
-      if (A.outErr) A.outErr[oid[s]] = err;
-      if (A.outFlags) A.outFlags[oid[s]] = is_dd<T>::value ? (uint8_t)(A.outFlags[oid[s]] | fl) : fl;
+      sample_tail<T>(P, A, I[s], Iabs[s], growth[s], amp[s], mant[s], ex[s], bad[s], oid[s], ta);
     }
     FG_MARK(ring, 7);
   }
 #ifdef FG_PHASE_PROF
   if (A.phase_cycles && (tid & 31) == 0) for (int k = 0; k < 9; ++k) atomicAdd(&A.phase_cycles[k], (unsigned long long)prof[k]);
 #endif
-  // a10: warp shuffle -> block -> one partial per block
-  double cnt[3] = {(double)nflag, (double)nrej, (double)nbig};
-  for (int off = 16; off > 0; off >>= 1) { sy = sy + shfl_dd(sy, off); sy2 = sy2 + shfl_dd(sy2, off); for (int k = 0; k < 3; ++k) cnt[k] += __shfl_down_sync(0xffffffffu, cnt[k], off); }
-  __syncthreads();
-  double* red = (double*)smem;   // the ring is idle now
-  if ((tid & 31) == 0) { double* r = red + (tid >> 5) * 8; r[0] = sy.hi; r[1] = sy.lo; r[2] = sy2.hi; r[3] = sy2.lo; r[4] = cnt[0]; r[5] = cnt[1]; r[6] = cnt[2]; }
-  __syncthreads();
-  if (tid == 0) {
-    dd a(0.0), b(0.0); double c[3] = {0, 0, 0};
-    for (int w = 0; w < NT / 32; ++w) { const double* r = red + w * 8; a = a + dd(r[0], r[1]); b = b + dd(r[2], r[3]); for (int k = 0; k < 3; ++k) c[k] += r[4 + k]; }
-    double* o = A.partials + (size_t)blockIdx.x * 8;
-    o[0] = a.hi; o[1] = a.lo; o[2] = b.hi; o[3] = b.lo; o[4] = c[0]; o[5] = c[1]; o[6] = c[2]; o[7] = 0.0;
+  block_reduce_tail(ta, (double*)smem /* the ring is idle now */, A.partials + (size_t)blockIdx.x * 8, prec<T>::rung == 0 ? 4 : 7);
+}
+
+// ---- double-precision pass, first kernel: a1-a5 for one wave of samples ------------------------------------------
+// One thread per sample, one block per batch of FG_ST_SAMPLES samples.  Writes, per batch: the operand tables V of every
+// element geometry (rows of FG_ST_VS doubles: the row layout of the stream kernel's shared memory, so that one bulk copy
+// brings a whole table in), U and W per geometry, and the per-sample record (pdf, state, conditioning).
+__global__ void __launch_bounds__(FG_ST_SAMPLES) fg_geom_kernel(const FgPlanDev P, const RunArgs A) {
+  const int tid = threadIdx.x, batch = blockIdx.x, M = P.M;
+  const uint64_t ord = A.ord0 + (uint64_t)batch * FG_ST_SAMPLES + tid;
+  const bool valid = ord < A.n;
+  double z[FG_MAXM], mant = 0.5; int ex = 1; bool bad = false;
+  if (valid) {
+    if (A.zin) { for (int v = 0; v < M; ++v) z[v] = A.zin[ord * M + v]; }
+    else {
+      Sample sp; draw_sample(P, P.Z1, P.Z3, A.first + ord, A.seed, sp);
+      for (int v = 0; v < M; ++v) z[v] = sp.z[v];
+      mant = sp.mant; ex = sp.ex; bad = sp.bad;
+    }
   }
+  if (!valid || bad) for (int v = 0; v < M; ++v) z[v] = 1.0 / M;
+  double zl[FG_MAXLINES];
+  for (int v = 0; v < M; ++v) {
+    const int l0 = P.var_line0[v], l1 = P.var_line1[v];
+    if (l1 == 255) zl[l0] = z[v]; else { zl[l0] = 0.5 * z[v]; zl[l1] = 0.5 * z[v]; }
+  }
+  double amx = 1.0, amp = 1.0;
+  double* Vb = A.gV + (size_t)batch * P.vtot * FG_ST_VS + tid;
+  double* UWb = A.gUW + (size_t)batch * 2 * P.ngeom * FG_ST_SAMPLES + tid;
+  for (int g = 0; g < P.ngeom; ++g) {
+    const FgGeomDev E = P.geoms[g];
+    double U, W, am, cp;
+    geom_eval<double>(E, zl, Vb + (size_t)P.geom_voff[g] * FG_ST_VS, FG_ST_VS, U, W, am, cp);
+    UWb[(2 * g) * FG_ST_SAMPLES] = U; UWb[(2 * g + 1) * FG_ST_SAMPLES] = W;
+    if (am > amx || !(am == am)) amx = am;
+    if (cp > amp || !(cp == cp)) amp = cp;
+  }
+  double* Mb = A.gMisc + (size_t)batch * FG_GM_ROWS * FG_ST_SAMPLES + tid;
+  Mb[FG_GM_MANT * FG_ST_SAMPLES] = mant; Mb[FG_GM_EX * FG_ST_SAMPLES] = (double)ex;
+  Mb[FG_GM_STATE * FG_ST_SAMPLES] = !valid ? 2.0 : (bad ? 1.0 : 0.0);
+  Mb[FG_GM_ZM * FG_ST_SAMPLES] = P.merge_var >= 0 ? z[P.merge_var] : 1.0;
+  Mb[FG_GM_AMAX * FG_ST_SAMPLES] = amx; Mb[FG_GM_AMP * FG_ST_SAMPLES] = amp;
+}
+
+// ---- double-precision pass, second kernel: a6-a10 ------------------------------------------------------------------
+// shared memory: [ring 2 x FG_CHUNK_BYTES][3 mbarriers, 128 B][exchange buffer 2 x FG_ST_SAMPLES doubles][V: vmax rows]
+#define FG_ST_XBUF_BYTES (2 * FG_ST_SAMPLES * 8)
+#define FG_ST_SMEM(vmax) (2 * FG_CHUNK_BYTES + 128 + FG_ST_XBUF_BYTES + (size_t)(vmax) * FG_ST_VS * 8)
+
+__device__ void run_program_s(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const double* V, int ne, double* Sc, double* xbuf) {
+  const int tid = threadIdx.x, ss = FG_ST_SAMPLES; const bool owner = tid < FG_ST_SAMPLES;
+  const int nslots = (1 << N.nse) * FG_NDEG * N.ncomp;
+  if (owner) for (int i = 0; i < nslots; ++i) { Sc[(sm.rawv + i) * ss] = 0.0; Sc[(sm.rawa + i) * ss] = 0.0; }
+  const int nch = N.chunk_count;
+  if (nch == 0) return;
+  const unsigned char* g0 = P.chunks + (size_t)N.chunk_begin * FG_CHUNK_BYTES;
+  const uint32_t* used = P.chunk_used + N.chunk_begin;
+  if (tid == 0) {
+    mbar_expect_tx(&ring.bar[0], used[0]); bulk_g2s(ring.buf, g0, used[0], &ring.bar[0]);
+    if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
+  }
+  StreamState st; st.cur = -1; st.has_part = 0; st.acc[0] = st.acc[1] = st.aab[0] = st.aab[1] = 0.0;
+#pragma unroll
+  for (int i = 0; i < 2 * FG_ST_NRB; ++i) st.part[i] = 0.0;
+#ifdef FG_PHASE_PROF
+  st.prof = ring.prof; st.tlast = ring.tlast;
+#endif
+  const int nc = N.ncomp, rawv = sm.rawv, rawa = sm.rawa;
+  auto flush = [&](int dst, const double* acc, const double* aab) {
+    for (int c = 0; c < nc; ++c) { Sc[(rawv + dst * nc + c) * ss] = acc[c]; Sc[(rawa + dst * nc + c) * ss] = aab[c]; }
+  };
+  for (int ch = 0; ch < nch; ++ch) {
+    const int b = ch & 1;
+    mbar_wait(&ring.bar[b], ring.phase[b]); ring.phase[b] ^= 1u;
+    FG_MARK(st, 5);
+    run_chunk_s(ring.buf + b * FG_CHUNK_BYTES, V, FG_ST_VS, ne, st, xbuf, flush);
+    FG_MARK(st, 8);
+    __syncthreads();   // every thread is done with buffer b
+    FG_MARK(st, 5);
+    if (tid == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], used[ch + 2]); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, used[ch + 2], &ring.bar[b]); }
+  }
+  fold_parts(st, xbuf);
+  if (st.cur >= 0 && owner) flush(st.cur, st.acc, st.aab);
+  FG_MARK(st, 8);
+#ifdef FG_PHASE_PROF
+  ring.tlast = st.tlast;
+#endif
+}
+
+__global__ void __launch_bounds__(FG_ST_THREADS, 1) fg_stream_kernel(const FgPlanDev P, const RunArgs A) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  ChunkRing ring; ring.buf = smem; ring.bar = (uint64_t*)(smem + 2 * FG_CHUNK_BYTES); ring.phase[0] = ring.phase[1] = 0u;
+#ifdef FG_PHASE_PROF
+  long long prof[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}; ring.prof = prof; ring.tlast = clock64();
+#endif
+  uint64_t* barV = ring.bar + 2; uint32_t phaseV = 0u;
+  double* xbuf = (double*)(smem + 2 * FG_CHUNK_BYTES + 128);
+  double* V = (double*)(smem + 2 * FG_CHUNK_BYTES + 128 + FG_ST_XBUF_BYTES);
+  const int tid = threadIdx.x, ss = FG_ST_SAMPLES; const bool owner = tid < FG_ST_SAMPLES;
+  if (tid == 0) { mbar_init(&ring.bar[0], 1); mbar_init(&ring.bar[1], 1); mbar_init(barV, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  __syncthreads();
+  const ScratchMap sm(P);
+  double* Sc = (double*)A.scratch + (size_t)blockIdx.x * (size_t)P.scratch_slots * ss + (owner ? tid : 0);
+  TailAcc ta; ta.sy = dd(0.0); ta.sy2 = dd(0.0); ta.nflag = ta.nrej = ta.nbig = 0;
+  for (int batch = blockIdx.x; batch < A.nb; batch += gridDim.x) {
+    double mant = 0.5, zm = 1.0, amx = 1.0, amp = 1.0; int ex = 1, state = 2;
+    if (owner) {
+      const double* Mb = A.gMisc + (size_t)batch * FG_GM_ROWS * FG_ST_SAMPLES + tid;
+      mant = Mb[FG_GM_MANT * FG_ST_SAMPLES]; ex = (int)Mb[FG_GM_EX * FG_ST_SAMPLES]; state = (int)Mb[FG_GM_STATE * FG_ST_SAMPLES];
+      zm = Mb[FG_GM_ZM * FG_ST_SAMPLES]; amx = Mb[FG_GM_AMAX * FG_ST_SAMPLES]; amp = Mb[FG_GM_AMP * FG_ST_SAMPLES];
+      const double* UWb = A.gUW + (size_t)batch * 2 * P.ngeom * FG_ST_SAMPLES + tid;
+      for (int k = 0; k < 2 * P.ngeom; ++k) Sc[k * ss] = UWb[k * FG_ST_SAMPLES];
+    }
+    FG_MARK(ring, 0);
+    for (int g = 0; g < P.ngeom; ++g) {
+      const int nv = P.geom_voff[g + 1] - P.geom_voff[g], ne = P.geoms[g].ne;
+      __syncthreads();                      // every warp is done with the previous operand table
+      if (tid == 0) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const unsigned char* src = (const unsigned char*)(A.gV + ((size_t)batch * P.vtot + P.geom_voff[g]) * FG_ST_VS);
+        const uint32_t bytes = (uint32_t)nv * FG_ST_VS * 8u;
+        mbar_expect_tx(barV, bytes);
+        for (uint32_t o = 0; o < bytes; o += 32768u) bulk_g2s((unsigned char*)V + o, src + o, bytes - o < 32768u ? bytes - o : 32768u, barV);
+      }
+      mbar_wait(barV, phaseV); phaseV ^= 1u;
+      FG_MARK(ring, 1);
+      for (int ni = P.geom_num_begin[g]; ni < P.geom_num_begin[g + 1]; ++ni) {
+        const FgNumDev N = P.nums[ni];
+        run_program_s(P, N, sm, ring, V, ne, Sc, xbuf);
+        if (owner) for (int k = 0; k < N.node_count; ++k) { finish_node<double, false>(P, sm, N.node_begin + k, Sc, ss); finish_node<double, true>(P, sm, N.node_begin + k, Sc, ss); }
+        FG_MARK(ring, 6);
+      }
+    }
+    if (owner && state != 2) {
+      double Iv, Ia; assemble<double, true>(P, sm, Sc, ss, Iv, Ia);
+      Iv *= zm; Ia *= zm;
+      sample_tail<double>(P, A, Iv, Ia, amx, amp, mant, ex, state == 1, A.ord0 + (uint64_t)batch * FG_ST_SAMPLES + tid, ta);
+    }
+    FG_MARK(ring, 7);
+  }
+#ifdef FG_PHASE_PROF
+  if (A.phase_cycles && (tid & 31) == 0) for (int k = 0; k < 9; ++k) atomicAdd(&A.phase_cycles[k], (unsigned long long)prof[k]);
+#endif
+  block_reduce_tail(ta, (double*)smem /* the ring is idle now */, A.partials + (size_t)blockIdx.x * 8, 4);
 }
 
 __global__ void fg_reduce_kernel(const double* partials, int nparts, Accum* acc, unsigned long long n_add, int finalize, fg_result* out) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   dd a(acc->sy[0], acc->sy[1]), b(acc->sy2[0], acc->sy2[1]);
-  double c[3] = {0, 0, 0};
-  for (int i = 0; i < nparts; ++i) { const double* r = partials + (size_t)i * 8; a = a + dd(r[0], r[1]); b = b + dd(r[2], r[3]); for (int k = 0; k < 3; ++k) c[k] += r[4 + k]; }
+  double c[4] = {0, 0, 0, 0};
+  for (int i = 0; i < nparts; ++i) { const double* r = partials + (size_t)i * 8; a = a + dd(r[0], r[1]); b = b + dd(r[2], r[3]); for (int k = 0; k < 4; ++k) c[k] += r[4 + k]; }
   acc->sy[0] = a.hi; acc->sy[1] = a.lo; acc->sy2[0] = b.hi; acc->sy2[1] = b.lo;
-  acc->nflag += (unsigned long long)c[0]; acc->nrej += (unsigned long long)c[1]; acc->nbig += (unsigned long long)c[2]; acc->n += n_add;
+  acc->nflag += (unsigned long long)c[0]; acc->nrej += (unsigned long long)c[1]; acc->nbig += (unsigned long long)c[2]; acc->nflag2 += (unsigned long long)c[3]; acc->n += n_add;
   if (finalize) {
     const double N = (double)acc->n;
     out->mean = to_double(a) / N;
     const dd v = b / dd(N * N) - a * a / dd(N * N * N);   // (17)
     out->variance = to_double(v);
     out->sum_y[0] = a.hi; out->sum_y[1] = a.lo; out->sum_y2[0] = b.hi; out->sum_y2[1] = b.lo;
-    out->n_samples = acc->n; out->n_flagged = acc->nflag; out->n_rejected = acc->nrej; out->n_pdf_big_exp = acc->nbig;
+    out->n_samples = acc->n; out->n_flagged = acc->nflag; out->n_flagged2 = acc->nflag2; out->n_rejected = acc->nrej; out->n_pdf_big_exp = acc->nbig;
   }
 }
 
@@ -310,19 +480,17 @@ static int fail(int code, const std::string& m) { g_err = m; return code; }
 
 struct fg_graph { Graph g; };
 
-#ifndef FG_NT_D
-#define FG_NT_D 256
-#endif
-static const int NT_D = FG_NT_D, S_D = 1;     // double pass: max threads per block (launch bound), samples per thread
-static const int NT_Q = 192, S_Q = 1;     // double-double pass
-static const uint64_t SLAB = 1ull << 24;  // samples per launch (bounds the re-evaluation queue)
+static const int NT_Q = 192, S_Q = 1;     // double-double pass: max threads per block (launch bound), samples per thread
+static const uint64_t SLAB = 1ull << 24;  // samples per slab (bounds the re-evaluation queue)
+static const size_t WAVE_BYTES = (size_t)3 << 30;   // budget of the operand tables one wave of the double pass keeps in HBM
 
 struct fg_plan {
   HostPlan H; FgPlanDev D; int device = 0, sms = 0;
   std::vector<void*> allocs;
   void* scratch = nullptr; double* partials = nullptr; Accum* accum = nullptr; fg_result* result_dev = nullptr;
   uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr; unsigned long long* phase_cycles = nullptr;
-  int grid_d = 0, grid_q = 0, nt_d = 0, nt_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
+  int grid_d = 0, grid_q = 0, nt_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
+  int wave_nb = 0; double *gV = nullptr, *gUW = nullptr, *gMisc = nullptr;   // wave buffers of the double pass (fg_geom_kernel -> fg_stream_kernel)
   int64_t table_bytes = 0;
   int profile = 0; cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; double ms[3] = {0, 0, 0}; long long launches = 0, flagged_last = 0;
   std::mutex mu;
@@ -405,26 +573,32 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
 #define UP(vec, field) do { int rc_ = upload(p, vec, &D.field); if (rc_ != FG_OK) { fg_plan_destroy(p); return rc_; } } while (0)
   UP(H.d_geoms, geoms); UP(H.d_nums, nums); UP(H.d_nodes, nodes); UP(H.d_terms, terms); UP(H.d_geom_num_begin, geom_num_begin);
   UP(H.d_chunks, chunks); UP(H.d_chunk_used, chunk_used); UP(H.Z1, Z1); UP(H.Z3, Z3);
+  UP(H.d_geom_voff, geom_voff);
 #undef UP
-  int vmax = 1; for (auto& E : H.geoms) vmax = std::max(vmax, E.ne * (E.ne + 1) / 2 + 2 * E.ne);
-  p->vmax = vmax;
-  // threads per block: as many warps as the per-sample operand table V (vmax entries) leaves room for in shared memory
+  D.vtot = H.vtot; D.vmax = H.vmax;
+  const int vmax = H.vmax; p->vmax = vmax;
   int smem_max = 0; cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+  // double pass: one persistent block of FG_ST_THREADS threads per SM, FG_ST_SAMPLES samples per batch
+  p->smem_d = FG_ST_SMEM(vmax);
+  if ((long)p->smem_d > (long)smem_max) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
+  // double-double pass: as many warps as the per-sample operand table V (vmax entries) leaves room for in shared memory
   const size_t ring_bytes = 2 * FG_CHUNK_BYTES + 128;
   auto fit = [&](int maxnt, size_t per_thread) { long nt = ((long)smem_max - (long)ring_bytes) / (long)per_thread - FG_VPAD; nt = std::min<long>(maxnt, nt / 32 * 32); return (int)nt; };
-  p->nt_d = fit(NT_D, (size_t)vmax * S_D * sizeof(double)); p->nt_q = fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd));
-  if (p->nt_d < 32 || p->nt_q < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
-  p->smem_d = ring_bytes + (size_t)vmax * (p->nt_d * S_D + FG_VPAD) * sizeof(double);
+  p->nt_q = fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd));
+  if (p->nt_q < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
   p->smem_q = ring_bytes + (size_t)vmax * (p->nt_q * S_Q + FG_VPAD) * sizeof(dd);
   // the attribute is per function, not per plan: always raise it to the device limit
   auto setattr = [&](const void* f) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max); };
-  e = setattr((const void*)fg_eval_kernel<double, S_D, NT_D>); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>);
+  e = setattr((const void*)fg_stream_kernel); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>);
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("shared memory: ") + cudaGetErrorString(e)); }
-  int bps_d = 1, bps_q = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_d, fg_eval_kernel<double, S_D, NT_D>, p->nt_d, p->smem_d);
+  int bps_q = 1;
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_q, fg_eval_kernel<dd, S_Q, NT_Q>, p->nt_q, p->smem_q);
-  p->grid_d = p->sms * std::max(1, std::min(bps_d, 4)); p->grid_q = p->sms * std::max(1, std::min(bps_q, 2));
-  size_t sc = (size_t)H.scratch_slots * std::max((size_t)p->nt_d * S_D * sizeof(double) * p->grid_d, (size_t)p->nt_q * S_Q * sizeof(dd) * p->grid_q);
+  p->grid_d = p->sms; p->grid_q = p->sms * std::max(1, std::min(bps_q, 2));
+  // a wave = a multiple of the grid in batches, bounded by the HBM budget of its operand tables
+  { const size_t per_batch = ((size_t)H.vtot * FG_ST_VS + (size_t)(2 * D.ngeom + FG_GM_ROWS) * FG_ST_SAMPLES) * sizeof(double);
+    long rounds = (long)(WAVE_BYTES / (per_batch * (size_t)p->grid_d)); rounds = std::max<long>(1, std::min<long>(rounds, 16));
+    p->wave_nb = (int)rounds * p->grid_d; }
+  size_t sc = (size_t)H.scratch_slots * std::max((size_t)FG_ST_SAMPLES * sizeof(double) * p->grid_d, (size_t)p->nt_q * S_Q * sizeof(dd) * p->grid_q);
   auto dmalloc = [&](void** d, size_t bytes) { cudaError_t e2 = cudaMalloc(d, bytes); if (e2 == cudaSuccess) { p->allocs.push_back(*d); cudaMemset(*d, 0, bytes); } return e2; };
   e = dmalloc(&p->scratch, sc);
   if (e == cudaSuccess) e = dmalloc((void**)&p->partials, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double));
@@ -433,6 +607,9 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   if (e == cudaSuccess) e = dmalloc((void**)&p->flag_list, SLAB * sizeof(uint32_t));
   if (e == cudaSuccess) e = dmalloc((void**)&p->flag_count, sizeof(unsigned long long));
   if (e == cudaSuccess) e = dmalloc((void**)&p->phase_cycles, 16 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->gV, (size_t)p->wave_nb * H.vtot * FG_ST_VS * sizeof(double));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->gUW, (size_t)p->wave_nb * 2 * D.ngeom * FG_ST_SAMPLES * sizeof(double));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->gMisc, (size_t)p->wave_nb * FG_GM_ROWS * FG_ST_SAMPLES * sizeof(double));
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
   *out = p; return FG_OK;
 }
@@ -472,17 +649,6 @@ int fg_plan_phase_cycles(const fg_plan* cp, uint64_t* cycles16, int32_t reset) {
 #endif
 }
 
-int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
-  if (!p || !s) return fail(FG_E_ARG, "NULL argument");
-  const HostPlan& H = p->H; std::memset(s, 0, sizeof(*s));
-  s->n_loops = H.g.n; s->M = H.M; s->n_subgraphs = (int)H.subs.size(); s->n_forests = (int)H.forests.size(); s->n_terms = (int)H.terms.size();
-  s->n_geoms = (int)H.geoms.size(); s->n_nums = (int)H.nums.size(); s->n_nodes = (int)H.nodes.size();
-  s->n_records = H.n_records; s->n_coefs = H.n_coefs; s->n_coefs_nonzero = H.n_nonzero;
-  s->table_bytes = p->table_bytes; s->stream_bytes = (int64_t)H.d_chunks.size();
-  s->flops_per_sample = H.algo_flops; s->exec_flops_per_sample = H.exec_flops; s->plan_seconds = H.plan_seconds;
-  return FG_OK;
-}
-
 static void fill_stats(const HostPlan& H, fg_plan_stats* s) {
   std::memset(s, 0, sizeof(*s));
   s->n_loops = H.g.n; s->M = H.M; s->n_subgraphs = (int)H.subs.size(); s->n_forests = (int)H.forests.size(); s->n_terms = (int)H.terms.size();
@@ -518,17 +684,15 @@ int fg_host_plan(const fg_graph* g, const fg_plan_opts* opts, fg_plan_stats* sta
   return dump_structure(H, subs, terms, terms_cap);
 }
 
+int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
+  if (!p || !s) return fail(FG_E_ARG, "NULL argument");
+  fill_stats(p->H, s); s->table_bytes = p->table_bytes;
+  return FG_OK;
+}
+
 int fg_plan_structure(const fg_plan* p, int32_t* subs, int32_t* terms, int32_t cap) {
   if (!p) return fail(FG_E_ARG, "NULL plan");
-  const HostPlan& H = p->H;
-  if (subs) for (size_t k = 0; k < H.subs.size(); ++k) { subs[4 * k] = H.subs[k].a; subs[4 * k + 1] = H.subs[k].b; subs[4 * k + 2] = H.subs[k].type; subs[4 * k + 3] = H.subs[k].chain; }
-  int w = 0;
-  if (terms) for (auto& t : H.terms) {
-    if (w + 3 + 2 * (int)t.members.size() > cap) return fail(FG_E_LIMIT, "terms buffer too small");
-    terms[w++] = t.sign; terms[w++] = t.gprime; terms[w++] = (int)t.members.size();
-    for (size_t k = 0; k < t.members.size(); ++k) { terms[w++] = t.members[k]; terms[w++] = t.ops[k]; }
-  }
-  return w;
+  return dump_structure(p->H, subs, terms, cap);
 }
 
 int fg_plan_tables(const fg_plan* p, double* deg, double* Z1) {
@@ -545,20 +709,25 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
   A.first = first; A.n = n; A.seed = seed; A.zin = zin; A.outI = dI; A.outId = dId; A.outY = dY; A.outErr = dErr; A.outFlags = dFl;
   A.scratch = p->scratch; A.phase_cycles = p->phase_cycles;
   int nparts = 0;
+  CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
   if (mode != 2) {
     CU(cudaMemsetAsync(p->flag_count, 0, sizeof(unsigned long long), st));
     A.flag_list = p->flag_list; A.flag_count = p->flag_count; A.do_flag = (mode == 0); A.partials = p->partials;
-    uint64_t nbatch = (n + (uint64_t)p->nt_d * S_D - 1) / ((uint64_t)p->nt_d * S_D);
-    int grid = (int)std::min<uint64_t>((uint64_t)p->grid_d, std::max<uint64_t>(nbatch, 1));
-    CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
+    A.gV = p->gV; A.gUW = p->gUW; A.gMisc = p->gMisc;
     if (p->profile) CU(cudaEventRecord(p->ev[0], st));
-    fg_eval_kernel<double, S_D, NT_D><<<grid, p->nt_d, p->smem_d, st>>>(p->D, A);
-    CU(cudaGetLastError()); ++p->launches;
+    const uint64_t nbatch = (n + FG_ST_SAMPLES - 1) / FG_ST_SAMPLES;
+    for (uint64_t b0 = 0; b0 < nbatch; b0 += (uint64_t)p->wave_nb) {      // waves: geometry of a wave, then its record streams
+      A.ord0 = b0 * FG_ST_SAMPLES; A.nb = (int)std::min<uint64_t>((uint64_t)p->wave_nb, nbatch - b0);
+      fg_geom_kernel<<<A.nb, FG_ST_SAMPLES, 0, st>>>(p->D, A);
+      CU(cudaGetLastError()); ++p->launches;
+      fg_stream_kernel<<<std::min(p->grid_d, A.nb), FG_ST_THREADS, p->smem_d, st>>>(p->D, A);
+      CU(cudaGetLastError()); ++p->launches;
+    }
     if (p->profile) CU(cudaEventRecord(p->ev[1], st));
     nparts = p->grid_d;
-  } else CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
+  }
   if (mode == 0 || mode == 2) {
-    RunArgs B = A; B.phase_cycles = nullptr; B.do_flag = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
+    RunArgs B = A; B.phase_cycles = nullptr; B.do_flag = 0; B.ord0 = 0; B.nb = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
     if (mode == 0) { B.idlist = p->flag_list; B.idcount = p->flag_count; }
     if (p->profile && mode == 2) { CU(cudaEventRecord(p->ev[0], st)); CU(cudaEventRecord(p->ev[1], st)); }
     fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, p->nt_q, p->smem_q, st>>>(p->D, B);

@@ -584,6 +584,9 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     P.d_geoms[i] = d;
   }
   P.d_geom_num_begin.assign(P.geoms.size() + 1, 0);
+  P.d_geom_voff.clear(); P.vtot = 0; P.vmax = 1;
+  for (auto& E : P.geoms) { const int nv = E.ne * (E.ne + 1) / 2 + 2 * E.ne; P.d_geom_voff.push_back(P.vtot); P.vtot += nv; P.vmax = std::max(P.vmax, nv); }
+  P.d_geom_voff.push_back(P.vtot);
   int raw_max = 0;
   std::map<std::vector<int>, std::array<long, 3>> hist;   // (mma, nf, k, qx, two) -> records, tiles, groups   (FG_PLAN_HIST=1 prints it)
   for (size_t i = 0; i < P.nums.size(); ++i) {
@@ -641,8 +644,8 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       const HRecord& r0 = N.recs[i];
       const bool qx = (r0.flags & FG_REC_QEXT) != 0;
       bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= 2 && (j - i) >= FG_MMA_MINREC;
-      if (mma) {     // tiles store float: only if every coefficient of the run survives the round trip unchanged
-        for (size_t t = i; t < j && mma; ++t) for (double c : N.recs[t].coef) if ((double)(FgMmaCoef)c != c) { mma = false; break; }
+      if (mma) {     // tiles store the high word of the double: only if every coefficient of the run has a zero low word
+        for (size_t t = i; t < j && mma; ++t) for (double c : N.recs[t].coef) { FgMmaCoef h; if (!fg_mma_coef_pack(c, &h)) { mma = false; break; } }
       }
       if (mma) {
         const int steps = mma_steps(r0.k, qx); const size_t tile_bytes = (size_t)FG_TILE_BYTES(steps);
@@ -656,7 +659,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
           for (int n = 0; n < 8; ++n) {
             FgRecM h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)r0.nf;
             if (const HRecord* r = rec_at(t, n)) {
-              std::memcpy(h.fidx, r->fidx, FG_NFC); h.cabs = std::max(r->cabs[0], r->cabs[1]);
+              std::memcpy(h.fidx, r->fidx, FG_NFC); h.cab16 = fg_cab16_pack((double)std::max(r->cabs[0], r->cabs[1]));
               const HRecord* pr = (n & 1) ? rec_at(t, n - 1) : (t > 0 && gn > 0 ? rec_at(t - 1, n + 1) : nullptr);   // gn == 0: first tile of a (re)opened group
               int keep = 0; if (pr) while (keep < r->nf && r->fidx[keep] == pr->fidx[keep]) ++keep;
               h.keep = (uint8_t)keep;
@@ -666,7 +669,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
           }
           FgMmaCoef* fr = (FgMmaCoef*)&P.d_chunks[base + cur + 8 * sizeof(FgRecM)];
           for (int st = 0; st < steps; ++st) for (int n = 0; n < 8; ++n) for (int x = 0; x < 4; ++x) {
-            const HRecord* r = rec_at(t, n); fr[st * 32 + n * 4 + x] = r ? (FgMmaCoef)mma_coef(*r, st, x) : (FgMmaCoef)0;
+            const HRecord* r = rec_at(t, n); FgMmaCoef h = 0; if (r) fg_mma_coef_pack(mma_coef(*r, st, x), &h); fr[st * 32 + n * 4 + x] = h;
           }
           cur += tile_bytes; ++gn;
           N.exec_flops += 8.0 * (8.0 * steps + 4.0);

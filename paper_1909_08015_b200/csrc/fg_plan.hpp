@@ -72,6 +72,7 @@ struct HostPlan {
   // flattened
   std::vector<FgGeomDev> d_geoms; std::vector<FgNumDev> d_nums; std::vector<FgNodeDev> d_nodes;
   std::vector<FgTermDev> d_terms; std::vector<int32_t> d_geom_num_begin; std::vector<unsigned char> d_chunks; std::vector<uint32_t> d_chunk_used;
+  std::vector<int32_t> d_geom_voff; int vtot = 0, vmax = 1;
   int raw_slots = 0, scratch_slots = 0;
   long n_records = 0, n_coefs = 0, n_nonzero = 0;
   double algo_flops = 0, exec_flops = 0, plan_seconds = 0;

@@ -1,0 +1,234 @@
+// fg_stream.cuh — a6 of the double-precision pass: the numerator record stream of one program, run by a block of
+// FG_ST_THREADS threads over a batch of FG_ST_SAMPLES samples whose operand tables V (beta, A, A^q) sit in shared memory
+// (DESIGN.md "kernels").  Tensor-core groups (FG_REC_MMA, fg_tables.h) are a dense contraction
+//   Q[sample][record] = sum_J mono_J[sample] * coef[J][record]
+// done with DMMA m8n8k4 (8 samples x 4 monomials x 8 records); sm_100a has no other FP64 tensor shape (the m16n8k4/k8/k16
+// f64 shapes of PTX lower to sequences of DMMA.8x8x4 here) and tcgen05 has no FP64 kind.
+//
+// Work split: warp w serves the 32 samples of sample group sg = w % 8 and the row blocks (8 samples each)
+// rb0 .. rb0 + FG_ST_NRB - 1 with rb0 = FG_ST_NRB * (w / 8); two warps share a sample group, so sixteen warps (four per
+// scheduler) stream the same tiles in step.  For one row block the monomials of a group are built ONCE (A fragments stay in
+// registers for all tiles of the group); per tile the lane loads its B fragment (one conflict-free LDS.32 per k-step: the
+// high word of the double), runs the k-steps, and weights its two record values with their products of beta's.
+#pragma once
+#include "fg_core.cuh"
+
+namespace fg {
+
+#ifndef FG_KO
+#define FG_KO 0      // knock-out experiments (timing only, results wrong): 1 no record epilogue, 2 no B loads, 4 no DMMA
+#endif
+#define FG_ST_THREADS 512
+#define FG_ST_SAMPLES 256
+#define FG_ST_NRB 2
+#define FG_ST_VS (FG_ST_SAMPLES + FG_VPAD)     // row stride of the operand table V (doubles)
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// A (8 samples x 4 monomials): lane (r = lane/4, c = lane%4) holds monomial 4*step + c of sample 8*b + r;
+// B (4 monomials x 8 records): lane holds coef[4*step + c] of record r;
+// D (8 x 8): lane holds records 2c, 2c+1 of sample 8*b + r.
+// The FG_ST_NRB row blocks of the warp go through a tile together: one B fragment and one decoded record header serve
+// them all (shared-memory wavefronts, not the FP64 pipe, are what this loop has to economise: ncu, profiles/).
+// part[bi] += value partial, part[FG_ST_NRB + bi] += |.| partial of row block rb0 + bi (reduced over the quad by fold_parts).
+template <int NF, int K, bool QX>
+__device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int ne, int rb0, double* __restrict__ part) {
+  __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
+  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS), NRB = FG_ST_NRB;
+  constexpr int ROWB = FG_ST_VS * 8;                 // bytes of one row of V
+  const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
+  const int vq = ne * ROWB;
+  const unsigned char* __restrict__ Vb = (const unsigned char*)(Vw + 8 * rb0 + r);     // sample of row block rb0; + 64 bytes per further row block
+  double av[NRB], ab[NRB];
+#pragma unroll
+  for (int bi = 0; bi < NRB; ++bi) { av[bi] = part[bi]; ab[bi] = part[NRB + bi]; }
+  for (int g = 0; g < nseq; ++g) {       // consecutive groups of this class (same destination), each with its own free variables
+    const uint4 gw = *(const uint4*)p; p += sizeof(FgGroupHdr);
+    const int ntiles = (int)(gw.x & 0xffffu);
+    const int v0 = (int)((gw.y >> 16) & 255u) * ROWB, v1 = (int)(gw.y >> 24) * ROWB, v2 = (int)(gw.z & 255u) * ROWB, v3 = (int)((gw.z >> 8) & 255u) * ROWB;
+    // the lane's column of the A fragments of every k-step (monomial order: fg_tables.h, mma_monomials), built once per group
+    double mono[NRB][STEPS];
+#pragma unroll
+    for (int bi = 0; bi < NRB; ++bi) {
+      const unsigned char* Vs = Vb + 64 * bi;
+      const double a0 = *(const double*)(Vs + v0), a1 = *(const double*)(Vs + v1);
+      const double a2 = K > 2 ? *(const double*)(Vs + v2) : 1.0, a3 = K > 3 ? *(const double*)(Vs + v3) : 1.0;
+      const double a01 = a0 * a1;
+      const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
+      double hi[NM]; hi[0] = 1.0;
+      if (K > 2) hi[1] = a2;
+      if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
+      mono[bi][0] = mlo;
+#pragma unroll
+      for (int tt = 1; tt < NM; ++tt) mono[bi][tt] = mlo * hi[tt];
+      if (QX) {
+        const double q0 = *(const double*)(Vs + v0 + vq), q1 = *(const double*)(Vs + v1 + vq);
+        const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
+        mono[bi][NM] = mq;
+#pragma unroll
+        for (int tt = 1; tt < NM; ++tt) mono[bi][NM + tt] = mq * hi[tt];
+        if (K == 3) mono[bi][2 * NM] = mlo * *(const double*)(Vs + v2 + vq);
+        if (K == 4) {
+          const double m2 = mlo * *(const double*)(Vs + v2 + vq), m3 = mlo * *(const double*)(Vs + v3 + vq);
+          mono[bi][2 * NM] = m2; mono[bi][2 * NM + 1] = m2 * a3; mono[bi][2 * NM + 2] = m3; mono[bi][2 * NM + 3] = m3 * a2;
+        }
+      }
+    }
+    double pf[NRB][NF > 0 ? NF : 1];
+#pragma unroll
+    for (int bi = 0; bi < NRB; ++bi) for (int i = 0; i < (NF > 0 ? NF : 1); ++i) pf[bi][i] = 1.0;
+    const unsigned char* __restrict__ pt = p;
+    for (int t = 0; t < ntiles; ++t, pt += TILE) {
+      const int* __restrict__ Bp = (const int*)(pt + 8 * sizeof(FgRecM)) + lane;
+      const uint4 hh = *(const uint4*)(pt + c * 16);                 // headers of the lane's records 2c, 2c+1
+      double d[NRB][2];
+#pragma unroll
+      for (int bi = 0; bi < NRB; ++bi) { d[bi][0] = 0.0; d[bi][1] = 0.0; }
+#pragma unroll
+      for (int st = 0; st < STEPS; ++st) {
+#if FG_KO & 2
+        const double b = __hiloint2double(lane + st, 0);
+#else
+        const double b = __hiloint2double(Bp[st * 32], 0);
+#endif
+#pragma unroll
+        for (int bi = 0; bi < NRB; ++bi) {
+#if FG_KO & 4
+          d[bi][0] = fma(mono[bi][st], b, d[bi][0]);
+#else
+          dmma884(d[bi][0], d[bi][1], mono[bi][st], b);
+#endif
+        }
+      }
+      // products of beta's of this lane's two records (the lane's depth-first stretch: the prefix stack survives from
+      // record to record within the group); the header is decoded once for all row blocks
+#if FG_KO & 1
+      for (int bi = 0; bi < NRB; ++bi) { av[bi] += d[bi][0] + d[bi][1]; ab[bi] += (double)hh.x; }
+#else
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const uint32_t w0 = e ? hh.z : hh.x, w1 = e ? hh.w : hh.y;
+        const double cab = fg_cab16_value(w1 >> 16);
+        if (NF > 0) {
+          const int keep = (int)((w1 >> 8) & 255u);
+#pragma unroll
+          for (int i = 0; i < NF; ++i) if (i >= keep) {
+            const int off = (int)__byte_perm(i < 4 ? w0 : w1, 0u, 0x4440 + (i & 3)) * ROWB;
+#pragma unroll
+            for (int bi = 0; bi < NRB; ++bi) {
+              const double v = *(const double*)(Vb + 64 * bi + off);
+              pf[bi][i] = (i == 0) ? v : pf[bi][i > 0 ? i - 1 : 0] * v;
+            }
+          }
+        }
+#pragma unroll
+        for (int bi = 0; bi < NRB; ++bi) {
+          const double bp = NF > 0 ? pf[bi][NF > 0 ? NF - 1 : 0] : 1.0;
+          av[bi] = fma(bp, d[bi][e], av[bi]); ab[bi] = fma(fabs(bp), cab, ab[bi]);
+        }
+      }
+#endif
+    }
+    p += (size_t)ntiles * TILE;
+  }
+#pragma unroll
+  for (int bi = 0; bi < NRB; ++bi) { part[bi] = av[bi]; part[NRB + bi] = ab[bi]; }
+}
+
+// Running state of one program in the stream kernel.  acc/aab: accumulators of the current destination (owner threads:
+// thread t < FG_ST_SAMPLES owns sample t of the batch); part: per-lane tensor-core partial sums (all threads).
+struct StreamState {
+  double acc[2], aab[2], part[2 * FG_ST_NRB]; int cur, has_part;
+#ifdef FG_PHASE_PROF
+  long long* prof; long long tlast;
+#endif
+};
+
+// Hand the tensor-core partial sums to the owner threads: quad-reduce, lane c == 0 of quad r posts the sums of sample
+// 32*sg + 8*b + r in the exchange buffer, the owner adds them.  Block-uniform (every warp walks the same stream), two
+// block barriers; called when the destination changes and at the end of a program.
+__device__ __forceinline__ void fold_parts(StreamState& st, double* __restrict__ xbuf) {
+  if (!st.has_part) return;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, sg = w & 7, rb0 = FG_ST_NRB * (w >> 3);
+#pragma unroll
+  for (int bi = 0; bi < FG_ST_NRB; ++bi) {
+    double v = st.part[bi], a = st.part[FG_ST_NRB + bi];
+    v += __shfl_xor_sync(0xffffffffu, v, 1); a += __shfl_xor_sync(0xffffffffu, a, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2); a += __shfl_xor_sync(0xffffffffu, a, 2);
+    if ((lane & 3) == 0) { const int smp = 32 * sg + 8 * (rb0 + bi) + (lane >> 2); xbuf[2 * smp] = v; xbuf[2 * smp + 1] = a; }
+    st.part[bi] = 0.0; st.part[FG_ST_NRB + bi] = 0.0;
+  }
+  __syncthreads();
+  if (tid < FG_ST_SAMPLES) { st.acc[0] += xbuf[2 * tid]; st.aab[0] += xbuf[2 * tid + 1]; }
+  __syncthreads();
+  st.has_part = 0;
+}
+
+// All groups of one chunk.  V: operand table of the batch (row stride vs); owner threads flush finished destinations.
+template <class Flush>
+__device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ chunk, const double* __restrict__ V, int vs, int ne, StreamState& st, double* xbuf, Flush&& flush) {
+  __builtin_assume(__isShared(chunk)); __builtin_assume(__isShared(V));
+  const int tid = threadIdx.x, w = tid >> 5;
+  const bool owner = tid < FG_ST_SAMPLES;
+  const double* Vt = V + (owner ? tid : 0);                      // the owner's column
+  const double* Vw = V + 32 * (w & 7); const int rb0 = FG_ST_NRB * (w >> 3);
+  const int ngroups = ((const FgChunkHdr*)chunk)->ngroups;
+  const unsigned char* p = chunk + sizeof(FgChunkHdr);
+  for (int g = 0; g < ngroups; ++g) {
+    FG_MARK(st, 8);
+    const FgGroupHdr gh = *(const FgGroupHdr*)p; p += sizeof(FgGroupHdr);
+    const int nrec = gh.nrec, nf = gh.nf, k = gh.k, flags = gh.flags;
+    if ((int)gh.dst != st.cur) {
+      fold_parts(st, xbuf);
+      if (st.cur >= 0 && owner) flush(st.cur, st.acc, st.aab);
+      st.cur = gh.dst; st.acc[0] = st.acc[1] = 0.0; st.aab[0] = st.aab[1] = 0.0;
+    }
+    const bool qx = (flags & FG_REC_QEXT) != 0;
+    if (flags & FG_REC_MMA) {
+      st.has_part = 1;
+      // consecutive tensor-core groups of the same class and destination are run by one call (run length and size come
+      // from the planner)
+      const unsigned char* p0 = p - sizeof(FgGroupHdr); const int nseq = gh.nseq;
+      switch (nf * 8 + k) {
+#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_rb<NF, K, true>(p0, nseq, Vw, ne, rb0, st.part); else run_group_mma_rb<NF, K, false>(p0, nseq, Vw, ne, rb0, st.part); break;
+        FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
+        FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
+#undef FG_MM
+        default: break;      // the planner makes tensor-core groups of these classes only
+      }
+      FG_MARK(st, 2);
+      p = p0 + gh.seq_bytes; g += nseq - 1; continue;
+    }
+    const int bytes = nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));
+    if (owner) {
+      bool done = false;
+      if (!(flags & (FG_REC_WIDE | FG_REC_TWO))) {
+        done = true;
+        switch (nf * 8 + k) {
+#define FG_CLS(NF, K) case NF * 8 + K: if (qx) run_group_static<double, 1, 1, NF, K, true>(p, nrec, Vt, vs, ne, &st.acc[0], &st.aab[0]); \
+                                        else run_group_static<double, 1, 1, NF, K, false>(p, nrec, Vt, vs, ne, &st.acc[0], &st.aab[0]); break;
+          FG_CLS(0, 0) FG_CLS(0, 1) FG_CLS(0, 2) FG_CLS(0, 3) FG_CLS(0, 4)
+          FG_CLS(1, 0) FG_CLS(1, 1) FG_CLS(1, 2) FG_CLS(1, 3) FG_CLS(1, 4)
+          FG_CLS(2, 0) FG_CLS(2, 1) FG_CLS(2, 2) FG_CLS(2, 3) FG_CLS(2, 4)
+          FG_CLS(3, 0) FG_CLS(3, 1) FG_CLS(3, 2) FG_CLS(3, 3) FG_CLS(3, 4)
+          FG_CLS(4, 0) FG_CLS(4, 1) FG_CLS(4, 2) FG_CLS(4, 3) FG_CLS(4, 4)
+          FG_CLS(5, 0) FG_CLS(5, 1) FG_CLS(5, 2) FG_CLS(5, 3) FG_CLS(5, 4)
+#undef FG_CLS
+          default: done = false; break;
+        }
+      }
+      if (done) FG_MARK(st, 3);
+      else {
+        RecState<double, 1> rs; rs.acc[0][0] = st.acc[0]; rs.acc[1][0] = st.acc[1]; rs.aab[0][0] = st.aab[0]; rs.aab[1][0] = st.aab[1]; rs.cur = st.cur; rs.split = 0; rs.rr = 0;
+        run_group_dyn<double, 1, 1>(p, nrec, nf, k, flags, Vt, vs, ne, rs);
+        st.acc[0] = rs.acc[0][0]; st.acc[1] = rs.acc[1][0]; st.aab[0] = rs.aab[0][0]; st.aab[1] = rs.aab[1][0];
+        FG_MARK(st, 4);
+      }
+    }
+    p += bytes;
+  }
+}
+
+}  // namespace fg

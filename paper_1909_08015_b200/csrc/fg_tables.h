@@ -90,21 +90,40 @@ static_assert(sizeof(FgRecC) == 16 && sizeof(FgRecW) == 32, "record header sizes
 //   main  steps t < 2^(k-2):        mlo[x] * mhi[t],  mlo = {1, a0, a1, a0 a1}, mhi[t] = prod_{bit i of t} a_{2+i}
 //   low-q steps (q-extension):      {aq0, aq0 a1, aq1, aq1 a0}[x] * mhi[t]
 //   high-q steps, j = 2..k-1:       aq_j * mlo[x] * (product over the subset t' of the other high variables)
-// A tile = 8 x FgRecM (product factors, cabs) + steps x 32 FgMmaCoef in B-fragment order (lane = 4*record + x).
-// The coefficients of a tile are stored as float: the planner makes a tensor-core group only of records whose
-// coefficients float holds exactly (integers times powers of two at every loop count met so far), so the double the
-// kernel converts back to is the same number; half the stream bytes, twice the tiles per chunk.
+// A tile = 8 x FgRecM (product factors, bound) + steps x 32 FgMmaCoef in B-fragment order (lane = 4*record + x).
+// The coefficients of a tile are stored as the HIGH 32-bit word of the double (sign, exponent, 20 mantissa bits): the
+// planner makes a tensor-core group only of records whose coefficients have a zero low word (integers below 2^21 times
+// powers of two: every coefficient met so far), so the double the kernel rebuilds with one register move is the same
+// number; half the stream bytes, twice the tiles per chunk, and no conversion instruction in the inner loop.
 // Lane c of a quad weights records 2c, 2c+1 of every tile; the planner deals the records of a run out so that these form
 // one contiguous stretch of the depth-first matching order, and keep = leading product factors shared with the lane's
 // previous record (prefix products stay in registers).
 // The group header carries the free variables (vidx) and nrec = number of tiles.
-typedef float FgMmaCoef;
+typedef int32_t FgMmaCoef;
+#if defined(__CUDA_ARCH__)
+__device__ __forceinline__ double fg_mma_coef_value(FgMmaCoef h) { return __hiloint2double(h, 0); }
+#else
+static inline double fg_mma_coef_value(FgMmaCoef h) { const uint64_t u = (uint64_t)(uint32_t)h << 32; double d; __builtin_memcpy(&d, &u, 8); return d; }
+#endif
+static inline bool fg_mma_coef_pack(double c, FgMmaCoef* out) {   // host: false if the low word is not zero
+  uint64_t u; __builtin_memcpy(&u, &c, 8); *out = (FgMmaCoef)(uint32_t)(u >> 32); return (u & 0xffffffffull) == 0;
+}
 #define FG_TILE_BYTES(steps) (8 * (int)sizeof(FgRecM) + (steps) * 32 * (int)sizeof(FgMmaCoef))
-struct alignas(16) FgRecM { uint8_t fidx[FG_NFC]; uint8_t keep; uint8_t pad[6]; float cabs; };
+// Record header of a tile, 8 bytes: product factors, shared prefix depth, and cab16 = the top 16 bits of the double
+// sum |coef| rounded UP (sign, exponent, 4 mantissa bits: a bound, at most 6 % above the sum).
+struct alignas(8) FgRecM { uint8_t fidx[FG_NFC]; uint8_t keep; uint16_t cab16; };
+#if defined(__CUDA_ARCH__)
+__device__ __forceinline__ double fg_cab16_value(uint32_t c) { return __hiloint2double((int)(c << 16), 0); }
+#else
+static inline double fg_cab16_value(uint32_t c) { const uint64_t u = (uint64_t)c << 48; double d; __builtin_memcpy(&d, &u, 8); return d; }
+#endif
+static inline uint16_t fg_cab16_pack(double c) {      // host: smallest representable value >= c (c >= 0)
+  uint64_t u; __builtin_memcpy(&u, &c, 8); uint64_t top = u >> 48; if (u & 0xffffffffffffull) ++top; return (uint16_t)top;
+}
 // nseq / seq_bytes (tensor-core groups): number and total size of the consecutive groups of the same class and
 // destination that start here inside this chunk (one kernel call runs them all).
 struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint16_t nseq; uint32_t seq_bytes; };
-static_assert(sizeof(FgRecM) == 16 && sizeof(FgGroupHdr) == 16, "group header sizes");
+static_assert(sizeof(FgRecM) == 8 && sizeof(FgGroupHdr) == 16, "group header sizes");
 struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
 
 // Everything the kernels need, passed by value.
@@ -118,6 +137,8 @@ struct FgPlanDev {
   const FgNodeDev* nodes;
   const FgTermDev* terms;
   const int32_t* geom_num_begin;      // nums are sorted by geometry: nums of geom g are [begin[g], begin[g+1])
+  const int32_t* geom_voff;           // row offset of the operand table of geom g in the per-batch table of all geometries
+  int32_t vtot, vmax;                 // rows of all geometries together; of the largest one
   const unsigned char* chunks;        // nchunk * FG_CHUNK_BYTES
   const uint32_t* chunk_used;         // bytes in use of every chunk (multiple of 16): what the TMA copy moves
   // density

@@ -42,13 +42,13 @@ class fg_plan_stats(C.Structure):
 
 class fg_result(C.Structure):
     _fields_ = [("mean", C.c_double), ("variance", C.c_double), ("sum_y", C.c_double * 2), ("sum_y2", C.c_double * 2),
-                ("n_samples", C.c_uint64), ("n_flagged", C.c_uint64), ("n_rejected", C.c_uint64),
+                ("n_samples", C.c_uint64), ("n_flagged", C.c_uint64), ("n_flagged2", C.c_uint64), ("n_rejected", C.c_uint64),
                 ("n_pdf_big_exp", C.c_uint64)]
 
     def as_dict(self):
         return dict(mean=self.mean, variance=self.variance, sum_y=(self.sum_y[0], self.sum_y[1]),
                     sum_y2=(self.sum_y2[0], self.sum_y2[1]), n_samples=int(self.n_samples),
-                    n_flagged=int(self.n_flagged), n_rejected=int(self.n_rejected),
+                    n_flagged=int(self.n_flagged), n_flagged2=int(self.n_flagged2), n_rejected=int(self.n_rejected),
                     n_pdf_big_exp=int(self.n_pdf_big_exp))
 
 
