@@ -51,7 +51,13 @@ void fg_graph_destroy(fg_graph*);
  *  D         exponent scale of the third component
  *  merge_ext_lines  1: the two electron lines at the external-photon vertex share one variable, M = 3n-1
  *            (fn.12); 0: M = 3n
- *  deg_table optional host array of 2^M doubles overriding Deg(s); NULL = built-in rule
+ *  deg_rule  0 = the built-in substitute rule R-Deg of DESIGN.md (the paper's own algorithm for Deg(s) is only in its Refs.
+ *            [42], [32]: PAPER.md:250); any other value is refused with FG_E_OPTS until that algorithm is available
+ *  deg_consts the six hand-chosen constants of that algorithm, eq. (15), in the order C_bigZ, C_bigF,
+ *            C_add, C_subI, C_subSE, C_subO (defaults 0.256, 0.839, 0.786, 0.2, 0, 0.2); carried for the paper's rule, not
+ *            used by rule 0
+ *  deg_table optional host array of 2^M doubles overriding Deg(s); NULL = deg_rule
+ *  structure_only  fg_host_plan only: stop after subgraphs, forests, terms and the Deg/Z tables (no Dirac tables)
  *  rel_tol, abs_tol  a sample whose estimated round-off error exceeds max(rel_tol*|I|, abs_tol*g) is
  *            re-evaluated in double-double (abs_tol plays the role of sigma/4 in (18))
  *  err_factor safety factor K of the running error estimate K*2^-53*sum|terms| (0 = default 8)                                 */
@@ -59,10 +65,13 @@ typedef struct {
   double C[4];
   double D;
   int32_t merge_ext_lines;
-  int32_t reserved;
+  int32_t deg_rule;
   const double* deg_table;
   double rel_tol, abs_tol;
   double err_factor;
+  double deg_consts[6];
+  int32_t structure_only;
+  int32_t reserved;
 } fg_plan_opts;
 void fg_plan_opts_default(fg_plan_opts* o);
 
@@ -104,6 +113,17 @@ int fg_plan_info(const fg_plan*, fg_plan_stats* out);
  * the Deg / Z_1 tables (2^M doubles each).  Any output pointer may be NULL.  For CPU tests of the host logic. */
 int fg_host_plan(const fg_graph*, const fg_plan_opts*, fg_plan_stats* stats, int32_t* subs, int32_t subs_cap,
                  int32_t* terms, int32_t terms_cap, double* deg, double* Z1);
+
+/* Host-only debug surface of the planner's Dirac algebra: the coefficient table of ONE Wick matching of ONE
+ * element = the UV-divergent subgraph on the vertex interval [a,b] with the child subgraphs `kids` (n_kids pairs a,b) shrunk.
+ * Slots are numbered in string order (from the outgoing end).  pairs: n_pairs matched slot pairs (i < j); qslot: the unmatched
+ * slot that carries gamma^nu (operator A only) or -1; op: 0 = A, 1 = U, 2 = L, 3 = L - U; comp: 0 / 1 = u / v of a
+ * self-energy element.  Output: gaps = the other unmatched slots (n_gaps of them), table[T] for every subset T of the gaps
+ * (bit g of T: gap g carries gamma^0 A_j), INCLUDING the factor (-1/2)^n_pairs of the Wick contractions.
+ * Returns the number of slots of the element, or a negative error code. */
+int fg_host_dirac_table(const fg_graph*, int32_t a, int32_t b, const int32_t* kids, int32_t n_kids, int32_t op, int32_t comp,
+                        const int32_t* pairs, int32_t n_pairs, int32_t qslot, double* table, int32_t table_cap, int32_t* gaps,
+                        int32_t* n_gaps);
 
 /* Structure dump for tests (expression (11)).
  *  subs: n_subgraphs rows (a, b, type 0 = self-energy / 1 = vertexlike, in_chain)

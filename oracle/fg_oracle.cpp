@@ -553,7 +553,7 @@ struct Oracle {
   // vertexlike child depends on the term, so a value is identified by its whole subtree)
   struct Node { int num; std::vector<int> kids; };   // kids aligned with geoms[].children
   std::vector<Node> nodes; std::map<std::vector<int>, int> node_index; std::vector<int> term_top;
-  bool printed_projector = true; bool structure_only = false;
+  bool printed_projector = true; int structure_only = 0;
   // density
   double C[4] = {0.9, 0.03, 0.01, 0.06}; double D = 0.75;
   std::vector<double> deg1, Z1, Z3; double lnZfull[4];
@@ -813,8 +813,10 @@ void Oracle::build_structure() {
         if (maximal) ch.push_back(c);
       }
       std::sort(ch.begin(), ch.end());
-      if (structure_only) continue;
-      int gi = build_geom(m, ch); tg.push_back(gi); int ni = build_num(gi, t.ops[k]); tn.push_back(ni);
+      if (structure_only == 1) continue;
+      int gi = build_geom(m, ch); tg.push_back(gi);
+      if (structure_only == 2) continue;                 // element geometries only (Dirac pins on single matchings)
+      int ni = build_num(gi, t.ops[k]); tn.push_back(ni);
       kids_of[m] = ch; num_of[m] = ni;
     }
     term_geom.push_back(tg); term_num.push_back(tn);
@@ -1064,7 +1066,7 @@ int fgo_count_undirected(int n) {
 }
 
 void* fgo_create(int n, int x, const int* photons, int merge, const double* C, double D, const double* deg_override, int printed_projector, int structure_only) {
-  Oracle* o = new Oracle(); o->structure_only = structure_only != 0;
+  Oracle* o = new Oracle(); o->structure_only = structure_only;
   if (!graph_make(n, x, photons, o->g)) { delete o; return nullptr; }
   o->merge = merge; o->printed_projector = printed_projector != 0;
   if (C) for (int k = 0; k < 4; ++k) o->C[k] = C[k];
@@ -1125,6 +1127,20 @@ double fgo_dirac_selfcheck(void* h, int maxpat_per_num, long* n_checked) {
     }
   }
   if (n_checked) *n_checked = cnt; return worst;
+}
+
+// The fast engine (dirac_matching_table) on ONE matching of element gi: table over the subsets of the gaps (unmatched slots
+// other than qslot, ascending); returns the number of gaps.  Without the factor (-1/2)^pairs.
+int fgo_dirac_table(void* h, int gi, int op, int comp, int npairs, const int* pairs, int qslot, double* table, int* gaps) {
+  Oracle* o = (Oracle*)h; const ElemGeom& E = o->geoms[gi]; int st = o->subs[E.sub].type; int ns = (int)E.slots.size();
+  Matching m; std::vector<int> used(ns, 0);
+  for (int k = 0; k < npairs; ++k) { m.pairs.push_back({pairs[2 * k], pairs[2 * k + 1]}); used[pairs[2 * k]] = used[pairs[2 * k + 1]] = 1; }
+  for (int sl = 0; sl < ns; ++sl) if (!used[sl]) m.unmatched.push_back(sl);
+  std::vector<double> tab;
+  dirac_matching_table(E.toks, ns, E.l, m, qslot, pieces_for(op, st, comp, qslot >= 0, o->printed_projector), tab);
+  int ng = 0; for (int sl : m.unmatched) if (sl != qslot) gaps[ng++] = sl;
+  for (size_t T = 0; T < tab.size(); ++T) table[T] = tab[T];
+  return ng;
 }
 
 // Description of element geometry gi: out = [a, b, type, nslots, l, nchildren, (a, b) of every child]; returns ints written.

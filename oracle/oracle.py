@@ -49,6 +49,8 @@ def lib():
         L.fgo_dirac_selfcheck.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.fgo_geom_desc.restype = C.c_int
         L.fgo_geom_desc.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.fgo_dirac_table.restype = C.c_int
+        L.fgo_dirac_table.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.fgo_dirac_explicit.restype = C.c_double
         L.fgo_dirac_explicit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_uint]
         L.fgo_u01.restype = C.c_double
@@ -97,7 +99,8 @@ class Oracle:
         if printed is None:
             printed = n <= 3          # the projector exactly as stated; its reduced form (pinned equal) above 3 loops
         dt = None if deg_table is None else np.ascontiguousarray(deg_table, dtype=np.float64)
-        self.h = lib().fgo_create(n, x, _p(ph), int(bool(merge)), _p(c4), float(D), _p(dt), int(bool(printed)), int(bool(structure_only)))
+        # structure_only: True / 1 = subgraphs, forests and terms only; 2 = also the element geometries (no numerator tables)
+        self.h = lib().fgo_create(n, x, _p(ph), int(bool(merge)), _p(c4), float(D), _p(dt), int(bool(printed)), int(structure_only))
         if not self.h:
             raise ValueError("invalid graph")
         info = np.zeros(8, dtype=np.int64)
@@ -179,6 +182,12 @@ class Oracle:
         w = lib().fgo_geom_desc(self.h, gi, _p(buf))
         return dict(a=int(buf[0]), b=int(buf[1]), type=int(buf[2]), nslots=int(buf[3]), l=int(buf[4]),
                     children=[(int(buf[6 + 2 * k]), int(buf[7 + 2 * k])) for k in range(int(buf[5]))])
+
+    def dirac_table(self, gi, op, comp, pairs, qslot):
+        """(gaps, table over the subsets of the gaps) of one matching of element gi from the oracle's fast engine."""
+        pr = np.asarray(pairs, dtype=np.int32).reshape(-1); tab = np.zeros(1 << 12); gaps = np.zeros(16, dtype=np.int32)
+        ng = lib().fgo_dirac_table(self.h, gi, int(op), int(comp), len(pr) // 2, _p(pr), int(qslot), _p(tab), _p(gaps))
+        return [int(v) for v in gaps[:ng]], tab[:1 << ng].copy()
 
     def dirac_explicit(self, gi, op, comp, pairs, qslot, tmask):
         """Coefficient of one pattern of element gi from explicit 4x4 matrices (without (-1/2)^pairs)."""

@@ -533,6 +533,8 @@ void fg_plan_opts_default(fg_plan_opts* o) {
   std::memset(o, 0, sizeof(*o));
   o->C[0] = 0.9; o->C[1] = 0.03; o->C[2] = 0.01; o->C[3] = 0.06; o->D = 0.75;   // Calc 2
   o->merge_ext_lines = 0; o->deg_table = nullptr; o->rel_tol = 1e-12; o->abs_tol = 0.0; o->err_factor = 0.0;
+  o->deg_rule = 0; const double c15[6] = {0.256, 0.839, 0.786, 0.2, 0.0, 0.2};   // eq. (15)
+  for (int k = 0; k < 6; ++k) o->deg_consts[k] = c15[k];
 }
 
 void fg_plan_destroy(fg_plan* p) {
@@ -551,6 +553,7 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(FG_E_CUDA, "no CUDA device: this library has no CPU path");
   if (device < 0 || device >= ndev) return fail(FG_E_ARG, "device out of range");
   fg_plan_opts o; if (opts) o = *opts; else fg_plan_opts_default(&o);
+  if (o.deg_rule != 0) return fail(FG_E_OPTS, "deg_rule: only rule 0 is available (the paper's Deg algorithm is in its Refs. [42], [32], PAPER.md:250)");
   PlanOpts po; for (int k = 0; k < 4; ++k) po.C[k] = o.C[k]; po.D = o.D; po.merge = o.merge_ext_lines ? 1 : 0;
   po.rel_tol = o.rel_tol; po.abs_tol = o.abs_tol; po.err_factor = o.err_factor;
   int M = 3 * g->g.n - (po.merge ? 1 : 0);
@@ -671,7 +674,9 @@ static int dump_structure(const HostPlan& H, int32_t* subs, int32_t* terms, int3
 int fg_host_plan(const fg_graph* g, const fg_plan_opts* opts, fg_plan_stats* stats, int32_t* subs, int32_t subs_cap, int32_t* terms, int32_t terms_cap, double* deg, double* Z1) {
   if (!g) return fail(FG_E_ARG, "graph is NULL");
   fg_plan_opts o; if (opts) o = *opts; else fg_plan_opts_default(&o);
+  if (o.deg_rule != 0) return fail(FG_E_OPTS, "deg_rule: only rule 0 is available (the paper's Deg algorithm is in its Refs. [42], [32], PAPER.md:250)");
   PlanOpts po; for (int k = 0; k < 4; ++k) po.C[k] = o.C[k]; po.D = o.D; po.merge = o.merge_ext_lines ? 1 : 0;
+  po.structure_only = o.structure_only != 0;
   int M = 3 * g->g.n - (po.merge ? 1 : 0);
   if (o.deg_table) po.deg_override.assign(o.deg_table, o.deg_table + ((size_t)1 << M));
   HostPlan H; std::string msg;
@@ -693,6 +698,22 @@ int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
 int fg_plan_structure(const fg_plan* p, int32_t* subs, int32_t* terms, int32_t cap) {
   if (!p) return fail(FG_E_ARG, "NULL plan");
   return dump_structure(p->H, subs, terms, cap);
+}
+
+int fg_host_dirac_table(const fg_graph* g, int32_t a, int32_t b, const int32_t* kids, int32_t n_kids, int32_t op, int32_t comp,
+                        const int32_t* pairs, int32_t n_pairs, int32_t qslot, double* table, int32_t table_cap, int32_t* gaps, int32_t* n_gaps) {
+  if (!g || !table || !gaps || !n_gaps || (n_kids && !kids) || (n_pairs && !pairs)) return fail(FG_E_ARG, "NULL argument");
+  std::vector<std::array<int, 2>> kv, pv;
+  for (int k = 0; k < n_kids; ++k) kv.push_back({kids[2 * k], kids[2 * k + 1]});
+  for (int k = 0; k < n_pairs; ++k) pv.push_back({pairs[2 * k], pairs[2 * k + 1]});
+  std::vector<double> tab; std::vector<int> gp; std::string msg;
+  int rc = dirac_table(g->g, a, b, kv, op, comp, pv, qslot, tab, gp, msg);
+  if (rc < 0) return fail(rc, msg);
+  if ((int)tab.size() > table_cap) return fail(FG_E_LIMIT, "table buffer too small");
+  std::memcpy(table, tab.data(), tab.size() * sizeof(double));
+  for (size_t k = 0; k < gp.size(); ++k) gaps[k] = gp[k];
+  *n_gaps = (int)gp.size();
+  return rc;
 }
 
 int fg_plan_tables(const fg_plan* p, double* deg, double* Z1) {

@@ -413,6 +413,24 @@ static void build_records(const HGeom& E, int type, HNum& N, bool& limit_hit) {
   }
 }
 
+// Debug surface (fg_host_dirac_table): the coefficient table of ONE matching of ONE element, straight from matching_table.
+int dirac_table(const Graph& g, int a, int b, const std::vector<std::array<int, 2>>& kid_iv, int op, int comp,
+                const std::vector<std::array<int, 2>>& pairs, int qslot, std::vector<double>& table, std::vector<int>& gaps, std::string& msg) {
+  std::vector<Sub> subs; Sub S;
+  if (!classify(g, a, b, S)) { msg = "[a,b] is not a UV-divergent subgraph"; return FG_E_ARG; }
+  subs.push_back(S); std::vector<int> kids;
+  for (auto& iv : kid_iv) { Sub K; if (!classify(g, iv[0], iv[1], K) || !contains(S, K)) { msg = "child interval is not a UV-divergent subgraph inside [a,b]"; return FG_E_ARG; } kids.push_back((int)subs.size()); subs.push_back(K); }
+  HGeom E = make_geom(g, subs, 0, kids);
+  const int ns = (int)E.slots.size();
+  Matching m; std::vector<int> used(ns, 0);
+  for (auto& pr : pairs) { if (pr[0] < 0 || pr[1] >= ns || pr[0] >= pr[1] || used[pr[0]] || used[pr[1]]) { msg = "bad pair"; return FG_E_ARG; } used[pr[0]] = used[pr[1]] = 1; m.pairs.push_back(pr); }
+  for (int sl = 0; sl < ns; ++sl) if (!used[sl]) m.unmatched.push_back(sl);
+  if (qslot >= 0 && (qslot >= ns || used[qslot])) { msg = "bad q slot"; return FG_E_ARG; }
+  gaps.clear(); for (int sl : m.unmatched) if (sl != qslot) gaps.push_back(sl);
+  matching_table(E, S.type, op, comp, m, qslot, qslot >= 0, gaps, table);
+  return ns;
+}
+
 // ------------------------------------------------------------------------------------------------
 // density tables.  Deg(s): the paper's algorithm (constants (15)) is only in
 // its Refs. [42],[32]; reading R-Deg is used unless the caller supplies a table.
@@ -571,6 +589,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     for (auto& t : P.terms) t.top = dnew[t.top];
     for (int i = 0; i < nd_n; ++i) P.nums[P.nodes[i].num].nodes.push_back(i);
   }
+  if (opts.structure_only) { build_density(P); P.plan_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count(); return FG_OK; }
   // Dirac tables -> records
   { bool limit_hit = false; for (auto& N : P.nums) build_records(P.geoms[N.geom], P.subs[P.geoms[N.geom].sub].type, N, limit_hit);
     if (limit_hit) { msg = "a numerator record needs more than FG_MAXF product factors"; return FG_E_LIMIT; } }

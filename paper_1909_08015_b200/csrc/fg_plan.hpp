@@ -55,6 +55,7 @@ struct PlanOpts {
   int merge = 0;
   std::vector<double> deg_override;
   double rel_tol = 1e-12, abs_tol = 0.0, err_factor = 0.0;
+  bool structure_only = false;                  // stop after the combinatorics and the density tables
 };
 
 struct HostPlan {
@@ -81,5 +82,9 @@ struct HostPlan {
 // returns FG_OK or an FG_E_* code; msg receives the detail
 int graph_from_edges(const int32_t* edges /* n_edges x (u,v,kind) */, int n_edges, int ext_vertex, Graph& g, std::string& msg);
 int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& msg);
+// coefficient table (over the subsets of `gaps`) of one matching of the element ([a,b] with the given children shrunk);
+// returns the number of slots or an FG_E_* code
+int dirac_table(const Graph& g, int a, int b, const std::vector<std::array<int, 2>>& kid_iv, int op, int comp,
+                const std::vector<std::array<int, 2>>& pairs, int qslot, std::vector<double>& table, std::vector<int>& gaps, std::string& msg);
 
 }  // namespace fg

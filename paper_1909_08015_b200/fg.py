@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("FG_LIB") or os.path.join(_HERE, "libfg.so")     # FG_LIB: a variant build (profiling counters)
 
 EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
-           "fg_plan_info", "fg_plan_phase_cycles", "fg_host_plan", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
+           "fg_plan_info", "fg_plan_phase_cycles", "fg_host_plan", "fg_host_dirac_table", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
            "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
 
@@ -28,8 +28,9 @@ class fg_edge(C.Structure):
 
 
 class fg_plan_opts(C.Structure):
-    _fields_ = [("C", C.c_double * 4), ("D", C.c_double), ("merge_ext_lines", C.c_int32), ("reserved", C.c_int32),
-                ("deg_table", C.c_void_p), ("rel_tol", C.c_double), ("abs_tol", C.c_double), ("err_factor", C.c_double)]
+    _fields_ = [("C", C.c_double * 4), ("D", C.c_double), ("merge_ext_lines", C.c_int32), ("deg_rule", C.c_int32),
+                ("deg_table", C.c_void_p), ("rel_tol", C.c_double), ("abs_tol", C.c_double), ("err_factor", C.c_double),
+                ("deg_consts", C.c_double * 6), ("structure_only", C.c_int32), ("reserved", C.c_int32)]
 
 
 class fg_plan_stats(C.Structure):
@@ -69,6 +70,7 @@ def lib():
         L.fg_plan_create.argtypes = [vp, C.POINTER(fg_plan_opts), C.c_int32, C.POINTER(vp)]
         L.fg_plan_destroy.argtypes = [vp]
         L.fg_host_plan.argtypes = [vp, C.POINTER(fg_plan_opts), C.POINTER(fg_plan_stats), vp, C.c_int32, vp, C.c_int32, vp, vp]
+        L.fg_host_dirac_table.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int32, C.c_int32, C.c_int32, vp, C.c_int32, C.c_int32, vp, C.c_int32, vp, vp]
         L.fg_plan_set_tol.argtypes = [vp, C.c_double, C.c_double]
         L.fg_plan_profile.argtypes = [vp, C.c_int32]
         L.fg_plan_timing.argtypes = [vp, vp, vp]
@@ -133,7 +135,7 @@ class Plan:
     """fg_plan_create (+ fg_plan_info, fg_integrate, ... on the plan)."""
 
     def __init__(self, graph, merge_ext_lines=False, C4=None, D=None, deg_table=None, rel_tol=1e-12, abs_tol=0.0,
-                 err_factor=0.0, device=0):
+                 err_factor=0.0, device=0, deg_rule=0, deg_consts=None):
         o = fg_plan_opts(); lib().fg_plan_opts_default(C.byref(o))
         if C4 is not None:
             for k in range(4):
@@ -141,7 +143,10 @@ class Plan:
         if D is not None:
             o.D = float(D)
         o.merge_ext_lines = int(bool(merge_ext_lines)); o.rel_tol = float(rel_tol); o.abs_tol = float(abs_tol)
-        o.err_factor = float(err_factor)
+        o.err_factor = float(err_factor); o.deg_rule = int(deg_rule)
+        if deg_consts is not None:
+            for k in range(6):
+                o.deg_consts[k] = float(deg_consts[k])
         self._deg = None
         if deg_table is not None:
             self._deg = np.ascontiguousarray(deg_table, dtype=np.float64); o.deg_table = self._deg.ctypes.data
@@ -234,9 +239,10 @@ class Plan:
 _OPS = {0: "A", 1: "U", 2: "L", 3: "L-U"}
 
 
-def host_plan(graph, merge_ext_lines=False, deg_table=None, tables=False):
+def host_plan(graph, merge_ext_lines=False, deg_table=None, tables=False, structure_only=False):
     """fg_host_plan: the planner alone (host, no device): (stats, subgraphs, terms[, Deg, Z_1])."""
     o = fg_plan_opts(); lib().fg_plan_opts_default(C.byref(o)); o.merge_ext_lines = int(bool(merge_ext_lines))
+    o.structure_only = int(bool(structure_only))
     keep = None
     if deg_table is not None:
         keep = np.ascontiguousarray(deg_table, dtype=np.float64); o.deg_table = keep.ctypes.data
@@ -256,6 +262,16 @@ def host_plan(graph, merge_ext_lines=False, deg_table=None, tables=False):
         n = 1 << stats["M"]
         return stats, ss, terms, deg[:n], z1[:n]
     return stats, ss, terms
+
+
+def host_dirac_table(graph, a, b, kids, op, comp, pairs, qslot=-1):
+    """fg_host_dirac_table: (n_slots, gaps, table over the subsets of the gaps) of one matching of one element."""
+    kd = np.asarray(kids, dtype=np.int32).reshape(-1); pr = np.asarray(pairs, dtype=np.int32).reshape(-1)
+    tab = np.zeros(1 << 12); gaps = np.zeros(16, dtype=np.int32); ng = np.zeros(1, dtype=np.int32)
+    ns = _check(lib().fg_host_dirac_table(graph.h, int(a), int(b), _p(kd), len(kd) // 2, int(op), int(comp), _p(pr), len(pr) // 2,
+                                          int(qslot), _p(tab), len(tab), _p(gaps), _p(ng)))
+    n = int(ng[0])
+    return ns, [int(v) for v in gaps[:n]], tab[:1 << n].copy()
 
 
 def result_merge(a, b):

@@ -13,6 +13,15 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "slow: long-running oracle check")
 
 
+def pytest_collection_modifyitems(config, items):
+    if os.environ.get("FG_RUN_SLOW"):
+        return
+    skip = pytest.mark.skip(reason="long-running oracle check: set FG_RUN_SLOW=1")
+    for it in items:
+        if "slow" in it.keywords:
+            it.add_marker(skip)
+
+
 def golden(name):
     return os.path.join(ROOT, "tests", "golden", name)
 

@@ -91,10 +91,18 @@ def test_dirac_coefficients_vs_explicit_matrices(n):
 
 
 def test_dirac_coefficients_three_loop_sampled():
-    for x, ph in inputs.all_graphs(3)[::17]:
+    for x, ph in inputs.all_graphs(3)[::5]:
         o = O.Oracle(x, ph, printed=False)
-        worst, cnt = o.dirac_selfcheck(12)
+        worst, cnt = o.dirac_selfcheck(40)
         assert cnt > 0 and worst < 1e-11
+
+
+def test_dirac_coefficients_four_loop_ladder_stored_tables():
+    """Stored tables of every (element, operator) of the 4-loop ladder of config 4, 60 patterns each spread over the table,
+    against explicit 4x4 matrices (the 5-loop tables are pinned matching by matching in test_dirac_and_subgraphs.py)."""
+    o = O.Oracle(4, [(0, 8), (1, 7), (2, 6), (3, 5)], printed=False)
+    worst, cnt = o.dirac_selfcheck(60)
+    assert cnt > 500 and worst < 1e-10
 
 
 def test_projector_printed_equals_reduced():
@@ -164,8 +172,41 @@ def test_matrix_tree_identity_and_beta():
             ze = z_own[:r["ne"]]
             assert np.allclose(r["A"], 1 - beta @ ze, atol=1e-12)
             assert abs(r["W"] - ze @ beta @ ze) < 1e-12
+            # A^q_j = xi^q_j / 2 - sum_e beta_je z_e xi^q_e / 2 with xi^q = -1 before the site of v_x and +1 after it
+            # (SURVEY O5).  xi^q is rebuilt here from the graph: own electron line q joins the sites ends[q]; the site of
+            # v_x is the one whose vertex interval holds x.
+            d = o.geom_desc(gi)
+            if d["a"] <= x <= d["b"]:
+                site_first_vertex = []; v = d["a"]
+                while v <= d["b"]:
+                    site_first_vertex.append(v)
+                    kid = [c for c in d["children"] if c[0] == v]
+                    v = (kid[0][1] if kid else v) + 1
+                xsite = max(k for k, fv in enumerate(site_first_vertex) if fv <= x)
+                xiq = np.array([-1.0 if r["ends"][q][1] <= xsite else 1.0 for q in range(r["ne"])])
+                assert np.array_equal(xiq, r["xiq"])
+                assert np.allclose(r["Aq"], 0.5 * xiq - beta @ (ze * 0.5 * xiq), atol=1e-12)
+                assert np.abs(r["Aq"]).max() > 0
+            else:
+                assert not r["xiq"].any() and not r["Aq"].any()
             checked += 1
     assert checked > 30
+
+
+def test_matrix_tree_identity_at_four_and_five_loops():
+    """The same identities on the elements of the 4-loop ladder, the graph of expression (11) and a config-5 graph with
+    self-energy children (geometry-only oracle: no Dirac tables are built)."""
+    rng = np.random.default_rng(12)
+    for x, ph in [(4, [(0, 8), (1, 7), (2, 6), (3, 5)]), (4, [(0, 10), (1, 9), (2, 3), (5, 7), (6, 8)]), inputs.config(5)["graphs"][17]]:
+        o = O.Oracle(x, ph, structure_only=2)
+        zl = rng.dirichlet(np.ones(3 * o.n))
+        for gi in range(o.n_geoms):
+            r = o.geom_eval(gi, zl); z_own = zl[r["own"]]; ze = z_own[:r["ne"]]
+            U, beta = _loop_matrix(r["ends"], r["ne"], z_own)
+            assert abs(U - r["U"]) <= 1e-12 * abs(U)
+            assert np.allclose(beta, r["beta"], rtol=0, atol=1e-11 * np.abs(beta).max())
+            assert np.allclose(r["A"], 1 - beta @ ze, atol=1e-11) and abs(r["W"] - ze @ beta @ ze) < 1e-11
+            assert np.allclose(r["Aq"], 0.5 * r["xiq"] - beta @ (ze * 0.5 * r["xiq"]), atol=1e-11)
 
 
 # ---------------------------------------------------------------- O5-O6 integrand
@@ -185,6 +226,17 @@ def test_one_loop_value_is_one_half():
     r = o.integrate(1, 0, 400000)
     assert abs(r["mean"] - float(FACTS["A1_2"][0])) < 4 * math.sqrt(r["variance"])
     assert math.sqrt(r["variance"]) < 2e-3
+
+
+@pytest.mark.slow
+def test_two_loop_sum_tight():                       # the same at 9x the samples: sigma < 0.004 (run with FG_RUN_SLOW=1)
+    target = float(FACTS["A1_4"][0]) - (119.0 / 36.0 - math.pi ** 2 / 3.0)
+    tot = var = 0.0
+    for x, ph in inputs.all_graphs(2):
+        r = O.Oracle(x, ph).integrate(1, 0, 14000000)
+        tot += r["mean"]; var += r["variance"]
+    assert math.sqrt(var) < 0.004
+    assert abs(tot - target) < 4 * math.sqrt(var), (tot, target, math.sqrt(var))
 
 
 def test_two_loop_sum():                             # PAPER.md:28 minus the closed-form VP-insertion graph
@@ -323,6 +375,49 @@ def test_estimator_formulas():
 
 
 # ---------------------------------------------------------------- O11 precision
+def test_wide_arithmetic_against_exact_rationals():
+    """The oracle's 256-bit arithmetic (the reference at ill-conditioned points) against Python's exact Fractions:
+    every operation correct to 2^-250 relative, massive cancellation included."""
+    from fractions import Fraction as F
+    rng = np.random.default_rng(1)
+    for t in range(600):
+        a3 = [rng.standard_normal() * 10.0 ** rng.integers(-20, 20), rng.standard_normal() * 1e-20, rng.standard_normal() * 1e-40]
+        b3 = [rng.standard_normal() * 10.0 ** rng.integers(-20, 20), rng.standard_normal() * 1e-18, rng.standard_normal() * 1e-37]
+        if t % 5 == 0:
+            b3 = [-a3[0] * (1 + 2.0 ** -40), a3[1], 0.0]          # a + b cancels 40 bits
+        a = sum(F(v) for v in a3); b = sum(F(v) for v in b3)
+        for op, want in enumerate((a + b, a - b, a * b, a / b)):
+            got = sum(F(float(v)) for v in O.bf_op(op, a3, b3))
+            assert want != 0 and abs((got - want) / want) < F(1, 2 ** 250), (op, a3, b3)
+
+
+def test_wide_evaluation_agrees_with_quad_where_quad_is_reliable():
+    """I in 256-bit arithmetic vs __float128: equal to double rounding on ordinary points; at points with heavy
+    cancellation the distance grows and the 256-bit value is the reference."""
+    o = O.Oracle(2, [(0, 4), (1, 3)])
+    z = o.sample(1, 0, 400)["z"]
+    Iw, Iq, dist = o.eval_wide(z)
+    Id, Iq2, _ = o.eval(z)
+    assert np.array_equal(Iq, Iq2)
+    assert np.all(dist < 1e-25) and np.all(np.abs(Iw - Iq) <= 1e-15 * np.abs(Iw))
+    # corners: the lines of the vertexlike subgraph scaled down.  At 1e-9 double is lost and __float128 still holds; at
+    # 1e-60 __float128 is lost too.  The 256-bit value is checked there by a symmetry that neither evaluation uses: the
+    # mirrored graph (other elements, other Dirac tables) at the mirrored point has the same integrand.
+    x, ph = 2, [(0, 4), (1, 3)]
+    xm, pm = inputs.mirror(x, ph); om = O.Oracle(xm, pm)
+    def mirrored(zz):                               # electron lines reversed; photons (0,4), (1,3) map onto themselves
+        return np.concatenate([zz[:, :4][:, ::-1], zz[:, 4:]], axis=1)
+    for scale, quad_ok in ((1e-9, True), (1e-60, False)):
+        zc = z[:16].copy(); zc[:, [1, 2, 5]] *= scale; zc /= zc.sum(axis=1, keepdims=True)
+        Iw, Iq, dist = o.eval_wide(zc); Id = o.eval(zc)[0]
+        Iwm = om.eval_wide(mirrored(zc))[0]
+        assert np.all(np.isfinite(Iw)) and np.all(np.abs(Iwm - Iw) <= 1e-14 * np.abs(Iw))
+        if quad_ok:
+            assert np.all(dist < 1e-12) and np.abs(Id - Iw).max() > 1e-9 * np.abs(Iw).max()
+        else:
+            assert np.median(dist) > 1e-3                          # __float128 is lost: 113 bits are not enough here
+
+
 def test_double_and_quad_agree_on_typical_points():
     o = O.Oracle(4, [(0, 6), (1, 5), (2, 3)])
     s = o.sample(1, 0, 3000)

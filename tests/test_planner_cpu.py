@@ -1,6 +1,8 @@
 """Host logic of the product's planner (fg_host_plan: no device, no kernels) against the paper and the oracle:
 subgraphs, forests and operator table, Deg/Z tables (bit-exact), and the number of
-non-zero Dirac coefficients, which the planner and the oracle obtain by two unrelated algebra engines."""
+non-zero Dirac coefficients.  The host combinatorics of the two sides were written from the same reading, so
+agreement here only shows that neither drifted; what pins them to the paper's definitions is tests/test_dirac_and_subgraphs.py
+(brute-force subgraphs, explicit 4x4 matrices) and the oracle pins of tests/test_oracle_pins.py."""
 import numpy as np
 import pytest
 
