@@ -4,12 +4,13 @@ seeded random 5-loop electron-vertex graphs without lepton loops, 14 variables a
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--graphs G] [--samples S] [--impl reference]
 
-A "step" integrates --samples samples of each of the first --graphs graphs of the config-5 batch (the 32 graphs come
-from the seeded generator in paper_1909_08015_b200/inputs.py; planning one 5-loop graph takes seconds of host time,
-so the default run times a prefix of the batch and says so in `config`).  Per step every graph gets a fresh range of
-sample ids, so no step repeats work.  value = samples/s per graph (total samples / total device time; graphs run
-one after another).  With N > 1 the graphs of a step are dealt out to the ranks (no data-path collective); value is
-the whole-job aggregate.  --impl reference times the CPU oracle on the host cores instead.
+A "step" integrates --samples samples (per GPU) of each of the first --graphs graphs of the config-5 batch, by default all
+32 (they come from the seeded generator in paper_1909_08015_b200/inputs.py; planning them takes a few minutes of host
+time before the timed region).  Per step every graph gets a fresh range of sample ids, so no step repeats work.
+value = whole-job samples/s per graph (all samples of all graphs / device time; graphs run one after another).  With
+N > 1 every graph's range is split over the ranks by paper_1909_08015_b200.dist (no data-path collective; one all_gather
+of the table of results per step, exact merge); value is the whole-job aggregate.  --impl reference times the CPU oracle
+on the host cores instead.
 """
 import argparse
 import ctypes
@@ -33,8 +34,9 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--graphs", type=int, default=2, help="how many graphs of the 32-graph config-5 batch to time")
-    ap.add_argument("--samples", type=int, default=1 << 24, help="samples per graph per step (one slab of the integrator)")
+    ap.add_argument("--graphs", type=int, default=32, help="how many graphs of the 32-graph config-5 batch to time")
+    ap.add_argument("--samples", type=int, default=1 << 20, help="samples per graph per step and per GPU")
+    ap.add_argument("--pilot-samples", type=int, default=1 << 16, help="samples of the pilot stage that sets the acceptance tolerance")
     ap.add_argument("--impl", default="fg", choices=["fg", "reference"])
     ap.add_argument("--rel-tol", type=float, default=0.0)
     ap.add_argument("--target-samples", type=float, default=1e10, help="run length the acceptance tolerance is set for")
@@ -83,20 +85,22 @@ def cfg5_graphs(n_graphs):
 
 def oracle_leg(args, graphs, steps, warmup, seconds):
     """The CPU oracle as it stands on the host cores: samples/s on a bounded sample of graph 0 (table build excluded,
-    reported as build_s)."""
+    reported as build_s).  Precision policy as on the GPU's first rung: every sample in double precision (the oracle's
+    higher-precision evaluations serve the parity tests; its __float128 rate is quoted in `sample` as context)."""
     from oracle import oracle as O
     x, ph = graphs[0]
     t0 = time.time(); orc = O.Oracle(x, ph, merge=True, printed=False); build_s = time.time() - t0
-    t0 = time.time(); orc.integrate(1, 0, 64, quad=True); probe = (time.time() - t0) / 64
-    per_step = max(64, int(seconds / max(steps, 1) / max(probe, 1e-9)))
+    t0 = time.time(); orc.integrate(1, 0, 256, quad=False); probe = (time.time() - t0) / 256
+    t0 = time.time(); orc.integrate(1, 0, 32, quad=True); quad_rate = 32 / (time.time() - t0)
+    per_step = max(256, int(seconds / max(steps, 1) / max(probe, 1e-9)))
     for w in range(warmup):
-        orc.integrate(1, 10 ** 9 + w * 64, 64, quad=True)
+        orc.integrate(1, 10 ** 9 + w * 256, 256, quad=False)
     t0 = time.time(); done = 0
     for k in range(steps):
-        orc.integrate(1, k * per_step, per_step, quad=True); done += per_step
+        orc.integrate(1, k * per_step, per_step, quad=False); done += per_step
     dt = time.time() - t0
     return dict(value=done / dt, unit=UNIT, cores=O.threads(), kind="oracle",
-                sample="config-5 graph 0, %d samples x %d steps, double + __float128 evaluation of every sample; table build %.0f s not timed" % (per_step, steps, build_s),
+                sample="config-5 graph 0, %d samples x %d steps, every sample in double precision (spanning-tree sums, pattern loops); with the __float128 evaluation of every sample on top: %.0f samples/s; table build %.0f s not timed" % (per_step, steps, quad_rate, build_s),
                 ms_per_step=1e3 * dt / steps, per_step=per_step, build_s=build_s)
 
 
@@ -104,7 +108,7 @@ def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    graphs, _ = cfg5_graphs(max(1, args.graphs))
+    graphs, _ = cfg5_graphs(1)
     r = oracle_leg(args, graphs, max(1, args.steps), args.warmup, seconds=min(120.0, 12.0 * max(1, args.steps)))
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -115,9 +119,14 @@ def main_reference(args):
     print(json.dumps(line))
 
 
+# DRAM traffic of the dominant kernel from the ncu capture of this build (profiles/r02_stream_kernel_ncu.md):
+# dram__bytes_read.sum + dram__bytes_write.sum per launch divided by the samples of that launch, config-5 graph 0.
+STREAM_KERNEL_DRAM_BYTES_PER_SAMPLE = None
+
+
 def main_fg(args):
     import torch
-    from paper_1909_08015_b200 import build, fg
+    from paper_1909_08015_b200 import build, dist as fgdist, fg, sched
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
     import torch.distributed as dist
     if world > 1:
@@ -131,26 +140,26 @@ def main_fg(args):
     if world > 1:
         dist.barrier()
     graphs, cfg = cfg5_graphs(args.graphs)
-    S = args.samples
+    S = args.samples                 # samples per graph per step PER GPU (weak scaling): a step integrates world * S per graph
     stream = torch.cuda.current_stream()
-    # plans; acceptance tolerance (18) for the run length the config names: abs_tol = sigma_down(target)/4 from a pilot
-    plans, info = [], []
-    for gi, (x, ph) in enumerate(graphs):
-        p = fg.plan_for(x, ph, merge_ext_lines=True, rel_tol=args.rel_tol, abs_tol=0.0, device=local)
-        p.set_tol(1e-6, 0.0)
-        pil = p.integrate_range(10 ** 12, 1 << 16, cfg["seed"], stream=stream)
-        sig_target = (pil["variance"] * pil["n_samples"] / args.target_samples) ** 0.5
-        p.set_tol(args.rel_tol, 0.25 * sig_target)
-        plans.append(p); info.append(dict(graph=gi, x=x, photons=ph, abs_tol=0.25 * sig_target, **{k: p.stats[k] for k in ("n_terms", "n_records", "n_coefs", "flops_per_sample", "exec_flops_per_sample", "plan_seconds")}))
+    # plans; acceptance tolerance (18) for the run length the config names: abs_tol = sigma_down(target)/4 from a pilot stage
+    batch = sched.Batch([fg.plan_for(x, ph, merge_ext_lines=True, rel_tol=1e-6, abs_tol=0.0, device=local) for x, ph in graphs])
+    plans = batch.plans
+    batch.pilot(args.pilot_samples, cfg["seed"], first_sample=10 ** 12, target_samples=args.target_samples, rel_tol=args.rel_tol, stream=stream)
+    info = [dict(graph=gi, x=x, photons=ph, abs_tol=batch.abs_tol[gi], **{k: plans[gi].stats[k] for k in ("n_terms", "n_records", "n_coefs", "flops_per_sample", "exec_flops_per_sample", "plan_seconds")})
+            for gi, (x, ph) in enumerate(graphs)]
     peak_tf, _ = fg.dfma_peak(local, 200000, stream)
     peak_tf = max(peak_tf, fg.dfma_peak(local, 200000, stream)[0])
     dmma_tf = fg.dmma_peak(local, 20000, stream)[0]       # FP64 tensor path (shares the FP64 units with DFMA): context
-    res_dev = torch.zeros(16 * len(plans), dtype=torch.float64, device=dev)
+    table = torch.zeros((len(plans), fgdist.RESULT_DOUBLES), dtype=torch.float64, device=dev)
+    gathered = [None]
 
     def step_async(k):
+        # product path of the multi-GPU case: every graph's sample range of this step is split over the ranks
+        # (dist.shard_range), shard results stay on the device, one all_gather of the result table per step
         for gi, p in enumerate(plans):
-            first = ((k * world + rank) * len(plans) + gi) * S
-            p.integrate_async(first, S, cfg["seed"], res_dev.data_ptr() + 128 * gi, stream=stream)
+            fgdist.integrate_sharded_async(p, world * S, cfg["seed"], rank, world, table[gi].data_ptr(), stream=stream, first_sample=k * world * S)
+        gathered[0] = fgdist.gather_device(table, world)
 
     def barrier():
         if world > 1:
@@ -160,6 +169,8 @@ def main_fg(args):
     for w in range(args.warmup):
         step_async(10 ** 6 + w)
     barrier()
+    for p in plans:
+        p.profile(True)              # four CUDA events per slab on the launching stream, resolved after the timed region
     clocks = ClockSampler(local) if rank == 0 else None
     if clocks:
         clocks.start()
@@ -170,24 +181,20 @@ def main_fg(args):
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
-    # per-kernel time of the dominant kernel (same steps again, events around every launch inside the library)
-    for p in plans:
-        p.profile(True)
-    for k in range(args.steps):
-        step_async(k)
-    barrier()
+    clk = clocks.finish() if clocks else None
     tim = [p.timing() for p in plans]
     for p in plans:
         p.profile(False)
-    clk = clocks.finish() if clocks else None
-    # end to end through the blocking C call with host result buffers (d2h of the 80-byte result every call)
-    flagged = rejected = 0
+    merged = fgdist.merge_gathered(gathered[0])          # last step, all ranks merged (exact double-double merge)
+    # end to end through the blocking C call with host result buffers (d2h of the 88-byte result every call)
+    flagged = flagged2 = rejected = 0
+    barrier()
     t0 = time.perf_counter()
     for k in range(args.steps):
         for gi, p in enumerate(plans):
-            first = ((k * world + rank) * len(plans) + gi) * S
-            r = p.integrate_range(first, S, cfg["seed"], stream=stream)
-            flagged += r["n_flagged"]; rejected += r["n_rejected"]
+            r = fgdist.integrate_sharded(p, world * S, cfg["seed"], rank, world, device=dev, stream=stream, first_sample=(args.steps + k) * world * S)
+            flagged += int(r.n_flagged); flagged2 += int(r.n_flagged2); rejected += int(r.n_rejected)
+    torch.cuda.synchronize()
     ms_e2e = 1e3 * (time.perf_counter() - t0)
     t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
     if world > 1:
@@ -206,26 +213,27 @@ def main_fg(args):
     for gi, x in enumerate(tim):       # per-graph throughput of the double-precision pass and its algorithmic FP64 rate
         info[gi]["samples_per_s"] = S * args.steps / (x["ms_double"] * 1e-3)
         info[gi]["algo_tflops"] = info[gi]["flops_per_sample"] * info[gi]["samples_per_s"] / 1e12
-        info[gi]["dd_ms_per_step"] = x["ms_dd"] / args.steps
-    traffic = None      # DRAM bytes per launch, scaled per sample from the committed ncu capture (profiles/r01_traffic.txt)
-    try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.txt")))
-        traffic = (tj["dram_bytes_read"] + tj["dram_bytes_write"]) / tj["samples"] * S
-    except Exception:
-        pass
+        info[gi]["frac"] = info[gi]["algo_tflops"] / peak_tf
+        info[gi]["ext_ms_per_step"] = x["ms_dd"] / args.steps
+        info[gi]["mean_last_step"] = merged[gi].mean; info[gi]["sigma_last_step"] = max(merged[gi].variance, 0.0) ** 0.5
+    fr = sorted(g["frac"] for g in info)
+    traffic = None if STREAM_KERNEL_DRAM_BYTES_PER_SAMPLE is None else STREAM_KERNEL_DRAM_BYTES_PER_SAMPLE * min(S, plans[0].wave_samples())
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": "config5: first %d of the 32 seeded random 5-loop vertex graphs (14 lines, M=14 after merge), %d samples per graph per step, fresh Philox sample ids every step" % (len(plans), S),
-                       "l2": "inputs are generated on chip; the 4-9 MB coefficient stream per graph is L2-resident by design (re-read by every block), no flush applies",
-                       "tolerance": "rel_tol %.1e, abs_tol = sigma_down(%.0e samples)/4 from a 65536-sample pilot per graph (PAPER.md (18))" % (args.rel_tol, args.target_samples),
-                       "graphs": info, "flagged_fraction": flagged / max(1.0, total / world), "rejected": rejected,
-                       "kernel_ms": {"double_pass": ms_d, "dd_pass": ms_q, "share_double": ms_d / max(ms_d + ms_q, 1e-9)},
+            "config": {"workload": "config5: %s of the 32 seeded random 5-loop vertex graphs (14 lines, M=14 after merge), %d samples per graph per step per GPU, graphs one after another, fresh Philox sample ids every step; value = whole-job samples/s per graph (all graphs' samples / device time)" % ("all 32" if len(plans) == 32 else "the first %d" % len(plans), S),
+                       "l2": "inputs are generated on chip; the 2-9 MB coefficient stream per graph is L2-resident by design (re-read by every block), no flush applies",
+                       "tolerance": "rel_tol %.1e, abs_tol = sigma_down(%.0e samples)/4 from a %d-sample pilot stage per graph (PAPER.md:286, (18))" % (args.rel_tol, args.target_samples, args.pilot_samples),
+                       "graphs": info, "flagged_fraction": flagged / max(1.0, total), "flagged2": flagged2, "rejected": rejected,
+                       "frac_per_graph": {"min": fr[0], "median": fr[len(fr) // 2], "max": fr[-1]},
+                       "kernel_ms": {"double_pass": ms_d, "extended_passes": ms_q, "share_double": ms_d / max(ms_d + ms_q, 1e-9)},
                        "exec_tflops_double_pass": execf / (ms_d * 1e-3) / 1e12},
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": traffic,
-                         "kernel": "fg_eval_kernel<double,1,256>", "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)", "dmma_peak": dmma_tf,
+                         "traffic_unit": "DRAM bytes per launch of one wave (ncu capture of this build, see profiles/)",
+                         "kernel": "fg_stream_kernel (with its fg_geom_kernel: the time is that of the double-precision pass, CUDA events around every slab in the timed region)",
+                         "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)", "dmma_peak": dmma_tf,
                          "frac_executed": execf / (ms_d * 1e-3) / 1e12 / peak_tf},
-            "e2e": {"value": total / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 80 * len(plans)},
+            "e2e": {"value": total / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 88 * len(plans)},
             "gpu_launches": launches, "clocks": clk}
     if not args.no_cpu_baseline and world == 1:
         r = oracle_leg(args, graphs, 3, 1, args.cpu_seconds)

@@ -83,9 +83,10 @@ void fg_plan_destroy(fg_plan*);
 /* Changes the acceptance tolerances of an existing plan (e.g. after a pilot run has measured sigma). */
 int fg_plan_set_tol(fg_plan*, double rel_tol, double abs_tol);
 
-/* Per-kernel device timing (CUDA events on the launching stream).  While enabled every slab of an integration
- * ends with an event synchronisation.  fg_plan_timing returns the milliseconds accumulated since fg_plan_profile:
- * ms3[0] double-precision pass, ms3[1] double-double pass, ms3[2] final reduction; and the kernels launched. */
+/* Per-kernel device timing (CUDA events on the launching stream, four per slab; nothing synchronises while the work is
+ * enqueued: fg_plan_timing waits for the recorded events and folds them).  fg_plan_timing returns the milliseconds accumulated since fg_plan_profile:
+ * ms3[0] double-precision pass (geometry + stream kernels), ms3[1] double-double and quad-double passes, ms3[2] final
+ * reduction; and the kernels launched. */
 int fg_plan_profile(fg_plan*, int32_t enable);
 int fg_plan_timing(const fg_plan*, double* ms3, int64_t* launches);
 
@@ -105,6 +106,7 @@ typedef struct {
   double flops_per_sample;            /* algorithmic FP64 flops of a5-a7 + sampler (FMA = 2), non-zero coefs only */
   double exec_flops_per_sample;       /* flops the double-precision kernel actually executes per sample */
   double plan_seconds;                /* host time spent in fg_plan_create */
+  int64_t wave_samples;               /* samples per wave of the double-precision pass (0 from fg_host_plan) */
 } fg_plan_stats;
 int fg_plan_info(const fg_plan*, fg_plan_stats* out);
 
@@ -142,7 +144,7 @@ typedef struct {
   uint64_t n_flagged;     /* samples re-evaluated in double-double (second rung) */
   uint64_t n_flagged2;    /* of those: samples re-evaluated again in quad-double (third rung) */
   uint64_t n_rejected;    /* samples that contributed 0: degenerate point, non-finite value, or not resolved by the
-                             double-double rung */
+                             last (quad-double) rung */
   uint64_t n_pdf_big_exp; /* samples whose pdf left the double range, kept as x*2^j */
 } fg_result;
 
@@ -152,11 +154,41 @@ int fg_integrate(const fg_plan*, uint64_t n_samples, uint64_t seed, void* stream
 int fg_integrate_range(const fg_plan*, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void* stream,
                        fg_result* out);
 /* Asynchronous form: the result is left in device memory (`out_dev`, sizeof(fg_result) bytes, written by the
- * final reduction kernel on `stream`); no host synchronisation. */
+ * final reduction kernel on `stream`); no host synchronisation.
+ * A plan owns ONE set of work buffers (wave tables, scratch, queues, partial sums): all integrations of a plan must be
+ * enqueued on the same stream (they then run one after another), or be separated by a synchronisation; calls from several
+ * host threads are serialised by a mutex inside the library, which does not lift that rule.  Use one plan per stream for
+ * concurrent work. */
 int fg_integrate_async(const fg_plan*, uint64_t first_sample, uint64_t n_samples, uint64_t seed, void* stream,
                        void* out_dev);
 /* Exact combination of two shards (double-double sums add; mean/variance recomputed). */
 int fg_result_merge(const fg_result* a, const fg_result* b, fg_result* out);
+
+/* ---- several graphs at once: initialisation stage, acceptance rule (18), block scheduling, combination (19) ----------------
+ * (PAPER.md:286, 290-294, 328-359).  A batch borrows its plans (they must outlive it).  Per graph it keeps the running sums of
+ * everything folded so far, the next unused Philox sample id, t_j = seconds per sample, and abs_tol_j of (18).
+ *  fg_batch_pilot   initialisation stage: n_pilot samples of every graph from sample id first_sample on (loose relative
+ *                   tolerance 1e-6), measures t_j, then sets abs_tol_j = (1/4) sigma_j sqrt(sum sigma_l^2) / sum sigma_l on
+ *                   every plan.  sigma_l = s_l / sqrt(N): N = target_samples per graph if > 0 (the tolerance the END of such a
+ *                   run needs), else the samples folded so far (the paper's floating rule); rel_tol is the
+ *                   relative part of the criterion from then on.
+ *  fg_batch_next    draws the graph of the next block, p_j = (C_j / sqrt t_j) / sum_l (C_l / sqrt t_l), C_j = sigma_j sqrt N_j
+ *                   = the per-sample standard deviation, with the uniform Philox4x32-10(key = sched_seed, counter = (block
+ *                   index, 0, 0, 0)) words 0, 1; reserves block_samples sample ids of that graph.
+ *  fg_batch_fold    adds a block result (and, if seconds > 0, a new measurement of t_j) to graph j and refreshes every abs_tol.
+ *  fg_batch_run     n_blocks times: next, fg_plan_set_tol (18), fg_integrate_range, fold (one GPU; several ranks: dist.py).
+ *  fg_batch_total   value = sum of the means, sigma_down by (19). */
+typedef struct fg_batch fg_batch;
+int fg_batch_create(fg_plan* const* plans, int32_t n_plans, fg_batch** out);
+void fg_batch_destroy(fg_batch*);
+int fg_batch_pilot(fg_batch*, uint64_t n_pilot, uint64_t seed, uint64_t first_sample, double target_samples, double rel_tol, void* stream);
+int fg_batch_set_times(fg_batch*, const double* seconds_per_sample);
+int fg_batch_probabilities(const fg_batch*, double* p);
+int fg_batch_next(fg_batch*, uint64_t sched_seed, uint64_t block_samples, int32_t* graph, uint64_t* first_sample);
+int fg_batch_fold(fg_batch*, int32_t graph, const fg_result* block, double seconds);
+int fg_batch_run(fg_batch*, uint64_t n_blocks, uint64_t block_samples, uint64_t seed, uint64_t sched_seed, void* stream);
+int fg_batch_result(const fg_batch*, int32_t graph, fg_result* out, double* abs_tol, double* seconds_per_sample);
+int fg_batch_total(const fg_batch*, double* value, double* sigma_down, uint64_t* n_total);
 
 /* ---- parity / debug surface (device kernels; outputs are HOST arrays, any may be NULL) -------------------
  * fg_sample_dump: for samples first..first+n-1: all Philox words (n * M * 4, call-major), mixture component (n),
@@ -164,10 +196,12 @@ int fg_result_merge(const fg_result* a, const fg_result* b, fg_result* out);
 int fg_sample_dump(const fg_plan*, uint64_t first, uint64_t n, uint64_t seed, void* stream, uint32_t* philox_words,
                    int32_t* comp, uint8_t* orderings, double* z, double* pdf_mant, int32_t* pdf_exp, uint8_t* bad);
 /* fg_eval_points: integrand at n given points (n*M doubles, on the simplex; n <= 2^24).  I = final value (double-double
- * where flagged), I_double = plain double pass, err = its running error estimate.  flags: bit0 = re-evaluated in
- * double-double, bit1 = non-finite value or degenerate point, bit2 = not resolved by the last rung (estimated error of
- * the double-double value still above the tolerance: the integrator lets such a sample contribute 0).
- * mode 0: as the integrator does; 1: double only; 2: double-double for every point. */
+ * or quad-double where flagged), I_double = plain double pass, err = the running error estimate of the first rung that ran.
+ * flags: bit0 = re-evaluated in double-double, bit3 = re-evaluated again in quad-double, bit1 = non-finite value or
+ * degenerate point, bit2 = not resolved by the last rung (estimated error of the quad-double value still above the
+ * tolerance: the integrator lets such a sample contribute 0).
+ * mode 0: as the integrator does (double -> double-double -> quad-double); 1: double only; 2: double-double for every
+ * point, quad-double for what that leaves; 3: quad-double for every point. */
 int fg_eval_points(const fg_plan*, const double* z, uint64_t n, int32_t mode, void* stream, double* I,
                    double* I_double, double* err, uint8_t* flags);
 /* fg_sample_eval_dump: what the integrator computes per sample, for samples first..first+n-1:

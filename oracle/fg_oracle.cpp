@@ -1072,7 +1072,7 @@ void* fgo_create(int n, int x, const int* photons, int merge, const double* C, d
   if (C) for (int k = 0; k < 4; ++k) o->C[k] = C[k];
   o->D = D;
   o->build_structure();
-  if (!structure_only) o->build_density(deg_override);
+  if (structure_only != 1) o->build_density(deg_override);      // 2: geometries + density (sampler), no Dirac tables
   return o;
 }
 void fgo_destroy(void* h) { delete (Oracle*)h; }
@@ -1177,6 +1177,18 @@ void fgo_eval(void* h, const double* z, long n, double rel_tol, double abs_tol, 
   }
 }
 
+// Diagnostic: "sum of the absolute values of everything that is added" for the same evaluation order, obtained by running
+// eval_point on a number type whose + and - both add magnitudes.  The geometry (Kirchhoff sums, A = 1 - s) is taken at
+// face value through AbsNum as well, so the figure is an upper bound of sum|terms| of the numerator and forest sums.
+struct AbsNum { double v; AbsNum() : v(0) {} AbsNum(double x) : v(std::fabs(x)) {} explicit operator double() const { return v; } };
+static AbsNum operator+(AbsNum a, AbsNum b) { return AbsNum(a.v + b.v); }
+static AbsNum operator-(AbsNum a, AbsNum b) { return AbsNum(a.v + b.v); }
+static AbsNum operator*(AbsNum a, AbsNum b) { return AbsNum(a.v * b.v); }
+static AbsNum operator/(AbsNum a, AbsNum b) { return AbsNum(a.v / b.v); }
+static AbsNum& operator+=(AbsNum& a, AbsNum b) { a.v += b.v; return a; }
+static AbsNum& operator-=(AbsNum& a, AbsNum b) { a.v += b.v; return a; }
+static AbsNum& operator*=(AbsNum& a, AbsNum b) { a.v *= b.v; return a; }
+
 // Third evaluation (O11): the integrand in 256-bit arithmetic, rounded to double, and the relative distance of the
 // __float128 value from it, |I_q - I_w| / |I_w| (computed in 256 bits).  A point is "hard for the oracle's __float128"
 // when that distance exceeds the tolerance of a comparison; the 256-bit value is the reference there.
@@ -1197,6 +1209,12 @@ void fgo_eval_wide(void* h, const double* z, long n, double* I_w, double* I_q, d
     if (I_q) I_q[i] = (double)q;
     if (dist_q) dist_q[i] = aw.sign ? (double)(diff / aw) : (diff.sign ? INFINITY : 0.0);
   }
+}
+
+void fgo_eval_abs(void* h, const double* z, long n, double* Iabs) {
+  Oracle* o = (Oracle*)h; int M = o->M;
+  #pragma omp parallel for schedule(dynamic, 16)
+  for (long i = 0; i < n; ++i) { AbsNum za[16]; for (int v = 0; v < M; ++v) za[v] = AbsNum(z[i * M + v]); Iabs[i] = (double)o->eval_point<AbsNum>(za, nullptr); }
 }
 
 // BF arithmetic pin: out = a op b with a = a0 + a1 + a2, b = b0 + b1 + b2 (exact sums of doubles), returned as three

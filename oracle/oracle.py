@@ -43,6 +43,7 @@ def lib():
                                     C.c_void_p]
         L.fgo_eval_wide.argtypes = [C.c_void_p, C.c_void_p, C.c_long, C.c_void_p, C.c_void_p, C.c_void_p]
         L.fgo_bf_op.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.fgo_eval_abs.argtypes = [C.c_void_p, C.c_void_p, C.c_long, C.c_void_p]
         L.fgo_geom_eval.restype = C.c_int
         L.fgo_geom_eval.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 10
         L.fgo_dirac_selfcheck.restype = C.c_double
@@ -152,6 +153,12 @@ class Oracle:
         Iw = np.zeros(n); Iq = np.zeros(n); dist = np.zeros(n)
         lib().fgo_eval_wide(self.h, _p(z), n, _p(Iw), _p(Iq), _p(dist))
         return Iw, Iq, dist
+
+    def eval_abs(self, z):
+        """Upper bound of the sum of |terms| of the oracle's own evaluation (diagnostic of cancellation)."""
+        z = np.ascontiguousarray(z, dtype=np.float64).reshape(-1, self.M); out = np.zeros(len(z))
+        lib().fgo_eval_abs(self.h, _p(z), len(z), _p(out))
+        return out
 
     def sample(self, seed, first, n):
         M = self.M

@@ -9,8 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfg.so")
-SOURCES = ["fg_kernels.cu", "fg_plan.cpp"]
-DEPS = SOURCES + ["fg_core.cuh", "fg_dd.cuh", "fg_tables.h", "fg_plan.hpp", os.path.join("..", "..", "include", "fg.h")]
+SOURCES = ["fg_kernels.cu", "fg_plan.cpp", "fg_batch.cpp"]
+DEPS = SOURCES + ["fg_core.cuh", "fg_stream.cuh", "fg_dd.cuh", "fg_qd.cuh", "fg_tables.h", "fg_plan.hpp", os.path.join("..", "..", "include", "fg.h")]
 
 
 def _nvcc():

@@ -11,6 +11,7 @@
 #include <stdint.h>
 
 #include "fg_dd.cuh"
+#include "fg_qd.cuh"
 #include "fg_tables.h"
 
 namespace fg {
@@ -112,74 +113,83 @@ FG_HD void draw_sample(const FgPlanDev& P, const double* __restrict__ Z1, const 
 // a5  geometry of one element at one point.  Loop a = own photon a plus the own electron lines between its ends:
 //   B_ab = sum_j z_j eta_ja eta_jb + delta_ab z_gamma_a,  U = det B,  C_a = sum_j z_j eta_ja,  W = C^T B^-1 C,
 //   A_j = 1 - eta_j^T B^-1 C,  beta_ij = eta_i^T B^-1 eta_j,  A^q_j = xi^q_j - eta_j^T B^-1 C^q.
-// B = L D L^T (no square roots).  This step is always carried out in double-double, whatever the precision of the
-// numerator pass: it is a few per cent of the work at 5 loops and it removes the cancellations of the pivots,
+// B = L D L^T (no square roots).  This step is carried out in double-double for the double and the double-double rung
+// (quad-double for the quad-double rung), whatever the precision of the numerator pass: it is a few per cent of the work at 5 loops and it removes the cancellations of the pivots,
 // of 1 - sum and of the beta dot products from the double-precision pass.
 // V receives beta (upper triangle, row-major), then A, then A^q, element idx at V[idx * vs]; amax = max(1,|A|,|A^q|);
 // amp = conditioning of this step: product of the pivot ratios B_aa/d_a times the worst ratio sum|terms|/|value| of the
 // final sums of A, A^q and beta (relative error of the entries of V is about amp * 2^-104).
 // ------------------------------------------------------------------------------------------------
-template <class T> FG_HD T from_dd(dd a);
-template <> FG_HD double from_dd<double>(dd a) { return a.hi + a.lo; }
-template <> FG_HD dd from_dd<dd>(dd a) { return a; }
+// G = arithmetic of the geometry step: double-double for the double and double-double rungs, quad-double for the last one
+template <class T> struct geom_prec { typedef dd type; };
+template <> struct geom_prec<qd> { typedef qd type; };
+template <class T, class G> FG_HD T from_geom(const G& a);
+template <> FG_HD double from_geom<double, dd>(const dd& a) { return a.hi + a.lo; }
+template <> FG_HD dd from_geom<dd, dd>(const dd& a) { return a; }
+template <> FG_HD qd from_geom<qd, qd>(const qd& a) { return a; }
+FG_HD double g_hi(const dd& a) { return a.hi; }
+FG_HD double g_hi(const qd& a) { return a.x[0]; }
+FG_HD dd g_add_d(const dd& a, double b) { return dd_add_d(a, b); }
+FG_HD qd g_add_d(const qd& a, double b) { return a + qd(b); }
 
 template <class T>
 FG_HD void geom_eval(const FgGeomDev& E, const double* zl, T* V, int vs, T& U, T& W, double& amax, double& amp) {
+  typedef typename geom_prec<T>::type G;
   const int l = E.l, ne = E.ne;
-  dd B[FG_MAXL][FG_MAXL], C[FG_MAXL], Cq[FG_MAXL], invd[FG_MAXL];
-  for (int a = 0; a < l; ++a) { C[a] = dd(0.0); Cq[a] = dd(0.0); for (int b = 0; b < l; ++b) B[a][b] = dd(0.0); }
+  G B[FG_MAXL][FG_MAXL], C[FG_MAXL], Cq[FG_MAXL], invd[FG_MAXL];
+  for (int a = 0; a < l; ++a) { C[a] = G(0.0); Cq[a] = G(0.0); for (int b = 0; b < l; ++b) B[a][b] = G(0.0); }
   for (int q = 0; q < ne; ++q) {
     const double z = zl[E.line_e[q]]; const unsigned m = E.eta[q]; const int xq = E.xiq[q];
     const double zh = xq > 0 ? 0.5 * z : -0.5 * z;
     for (int a = 0; a < l; ++a) if ((m >> a) & 1u) {
-      C[a] = dd_add_d(C[a], z);
-      if (xq != 0) Cq[a] = dd_add_d(Cq[a], zh);
-      for (int b = 0; b <= a; ++b) if ((m >> b) & 1u) B[a][b] = dd_add_d(B[a][b], z);
+      C[a] = g_add_d(C[a], z);
+      if (xq != 0) Cq[a] = g_add_d(Cq[a], zh);
+      for (int b = 0; b <= a; ++b) if ((m >> b) & 1u) B[a][b] = g_add_d(B[a][b], z);
     }
   }
-  for (int a = 0; a < l; ++a) B[a][a] = dd_add_d(B[a][a], zl[E.line_ph[a]]);
-  dd u(1.0); double growth = 1.0;
+  for (int a = 0; a < l; ++a) B[a][a] = g_add_d(B[a][a], zl[E.line_ph[a]]);
+  G u(1.0); double growth = 1.0;
   for (int a = 0; a < l; ++a) {
-    dd d = B[a][a]; const double baa = d.hi;
+    G d = B[a][a]; const double baa = g_hi(d);
     for (int b = 0; b < a; ++b) d = d - B[a][b] * B[a][b] * B[b][b];     // B[b][b] holds d_b, B[a][b] holds L_ab
-    invd[a] = dd(1.0) / d; u = u * d; growth *= fmax(1.0, baa / d.hi);
+    invd[a] = G(1.0) / d; u = u * d; growth *= fmax(1.0, baa / g_hi(d));
     for (int c = a + 1; c < l; ++c) {
-      dd t = B[c][a];
+      G t = B[c][a];
       for (int b = 0; b < a; ++b) t = t - B[c][b] * B[a][b] * B[b][b];
       B[c][a] = t * invd[a];
     }
     B[a][a] = d;
   }
-  U = from_dd<T>(u);
+  U = from_geom<T, G>(u);
   for (int a = 0; a < l; ++a) for (int b = 0; b < a; ++b) { C[a] = C[a] - B[a][b] * C[b]; Cq[a] = Cq[a] - B[a][b] * Cq[b]; }   // L^-1 C, L^-1 C^q
-  dd w(0.0); for (int a = 0; a < l; ++a) { w = w + C[a] * C[a] * invd[a]; C[a] = C[a] * invd[a]; Cq[a] = Cq[a] * invd[a]; }
-  W = from_dd<T>(w);
-  dd Y[FG_MAXNE][FG_MAXL]; int first[FG_MAXNE];
+  G w(0.0); for (int a = 0; a < l; ++a) { w = w + C[a] * C[a] * invd[a]; C[a] = C[a] * invd[a]; Cq[a] = Cq[a] * invd[a]; }
+  W = from_geom<T, G>(w);
+  G Y[FG_MAXNE][FG_MAXL]; int first[FG_MAXNE];
   const int nb = ne * (ne + 1) / 2; double am = 1.0, cond = 1.0;
   for (int q = 0; q < ne; ++q) {
     const unsigned m = E.eta[q];
     // y = L^-1 eta_q vanishes below the first loop of the line: structural zeros (block-uniform) are skipped everywhere
     int fq = 0; while (fq < l && !((m >> fq) & 1u)) ++fq;
     first[q] = fq;
-    for (int a = 0; a < fq; ++a) Y[q][a] = dd(0.0);
-    for (int a = fq; a < l; ++a) { dd y = ((m >> a) & 1u) ? dd(1.0) : dd(0.0); for (int b = fq; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
-    dd sa(0.0), sq(0.0); double ta = 1.0, tq = 0.5;
-    for (int a = fq; a < l; ++a) { const dd t1 = Y[q][a] * C[a], t2 = Y[q][a] * Cq[a]; sa = sa + t1; sq = sq + t2; ta += fabs(t1.hi); tq += fabs(t2.hi); }
-    const dd A = dd(1.0) - sa, Aq = dd(0.5 * (double)E.xiq[q]) - sq;
-    V[(nb + q) * vs] = from_dd<T>(A); V[(nb + ne + q) * vs] = from_dd<T>(Aq);
-    am = fmax(am, fmax(fabs(A.hi), fabs(Aq.hi)));
-    if (A.hi != 0.0) cond = fmax(cond, ta / fabs(A.hi));
-    if (E.xiq[q] != 0 && Aq.hi != 0.0) cond = fmax(cond, tq / fabs(Aq.hi));
+    for (int a = 0; a < fq; ++a) Y[q][a] = G(0.0);
+    for (int a = fq; a < l; ++a) { G y = ((m >> a) & 1u) ? G(1.0) : G(0.0); for (int b = fq; b < a; ++b) y = y - B[a][b] * Y[q][b]; Y[q][a] = y; }
+    G sa(0.0), sq(0.0); double ta = 1.0, tq = 0.5;
+    for (int a = fq; a < l; ++a) { const G t1 = Y[q][a] * C[a], t2 = Y[q][a] * Cq[a]; sa = sa + t1; sq = sq + t2; ta += fabs(g_hi(t1)); tq += fabs(g_hi(t2)); }
+    const G A = G(1.0) - sa, Aq = G(0.5 * (double)E.xiq[q]) - sq;
+    V[(nb + q) * vs] = from_geom<T, G>(A); V[(nb + ne + q) * vs] = from_geom<T, G>(Aq);
+    am = fmax(am, fmax(fabs(g_hi(A)), fabs(g_hi(Aq))));
+    if (g_hi(A) != 0.0) cond = fmax(cond, ta / fabs(g_hi(A)));
+    if (E.xiq[q] != 0 && g_hi(Aq) != 0.0) cond = fmax(cond, tq / fabs(g_hi(Aq)));
   }
   amax = am;
   int idx = 0;
   for (int i = 0; i < ne; ++i) {
-    dd yd[FG_MAXL]; for (int a = first[i]; a < l; ++a) yd[a] = Y[i][a] * invd[a];
+    G yd[FG_MAXL]; for (int a = first[i]; a < l; ++a) yd[a] = Y[i][a] * invd[a];
     for (int j = i; j < ne; ++j) {
       const int f2 = first[i] > first[j] ? first[i] : first[j];
-      dd b(0.0); double tb = 0.0; for (int a = f2; a < l; ++a) { const dd t1 = yd[a] * Y[j][a]; b = b + t1; tb += fabs(t1.hi); }
-      if (b.hi != 0.0) cond = fmax(cond, tb / fabs(b.hi));
-      V[idx * vs] = from_dd<T>(b); ++idx;
+      G b(0.0); double tb = 0.0; for (int a = f2; a < l; ++a) { const G t1 = yd[a] * Y[j][a]; b = b + t1; tb += fabs(g_hi(t1)); }
+      if (g_hi(b) != 0.0) cond = fmax(cond, tb / fabs(g_hi(b)));
+      V[idx * vs] = from_geom<T, G>(b); ++idx;
     }
   }
   amp = growth * cond;
@@ -350,6 +360,10 @@ FG_HD int fg_lane() {
 #if defined(__CUDACC__)
 __device__ __forceinline__ double warp_sum(double v, int w) { for (int o = w >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o); return v; }
 __device__ __forceinline__ dd warp_sum(dd v, int w) { for (int o = w >> 1; o > 0; o >>= 1) v = v + dd(__shfl_xor_sync(0xffffffffu, v.hi, o), __shfl_xor_sync(0xffffffffu, v.lo, o)); return v; }
+__device__ __forceinline__ qd warp_sum(qd v, int w) {
+  for (int o = w >> 1; o > 0; o >>= 1) v = v + qd(__shfl_xor_sync(0xffffffffu, v.x[0], o), __shfl_xor_sync(0xffffffffu, v.x[1], o), __shfl_xor_sync(0xffffffffu, v.x[2], o), __shfl_xor_sync(0xffffffffu, v.x[3], o));
+  return v;
+}
 #endif
 // split mode (st.split = w = 2..32 lanes per point): add the partial sums of the w lanes of a point (each of them ends up
 // with the same totals)
@@ -512,7 +526,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
       for (int s = 0; s < S; ++s) { st.acc[0][s] = T(0.0); st.acc[1][s] = T(0.0); st.aab[0][s] = 0.0; st.aab[1][s] = 0.0; }
     }
     bool done = false;
-    if constexpr (!is_dd<T>::value && ABS != 2) {      // (host harness; the device's double pass has its own chunk loop, fg_stream.cuh)
+    if constexpr (!is_ext<T>::value && ABS != 2) {      // (host harness; the device's double pass has its own chunk loop, fg_stream.cuh)
       if (!(flags & (FG_REC_WIDE | FG_REC_TWO | FG_REC_MMA))) {
         done = true;
         const bool qx = (flags & FG_REC_QEXT) != 0;

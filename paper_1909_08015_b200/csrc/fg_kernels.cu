@@ -33,7 +33,7 @@ struct RunArgs {
   const uint32_t* idlist; const unsigned long long* idcount;   // work list (ordinals relative to first) or NULL
   const double* zin;                                           // points instead of samples, or NULL
   double *outI, *outId, *outY, *outErr; uint8_t* outFlags;     // optional per-sample dumps, indexed by ordinal
-  uint32_t* flag_list; unsigned long long* flag_count;         // queue for the next rung
+  uint32_t* flag_bits;                                         // one bit per ordinal: queued for the next rung (compacted in id order afterwards)
   int do_flag;
   double* partials;                                            // [gridDim.x][8]
   void* scratch;
@@ -110,6 +110,36 @@ __device__ void run_program(const FgPlanDev& P, const FgNumDev& N, const Scratch
 #endif
 }
 
+// Precision rungs (PAPER.md:294-298).  unit: round-off unit of the running error estimate K * u * sum|terms|;
+// geom_unit: relative error of the geometry step per unit of its conditioning `amp`.
+template <class T> struct prec;
+template <> struct prec<double> { static const int rung = 0; static __device__ double unit(double e, double af) { return e * af; } static __device__ double geom_unit() { return 0x1p-109; } };
+template <> struct prec<dd> { static const int rung = 1; static __device__ double unit(double e, double) { return e * 0x1p-51; } static __device__ double geom_unit() { return 0x1p-109; } };
+template <> struct prec<qd> { static const int rung = 2; static __device__ double unit(double e, double) { return e * 0x1p-147; } static __device__ double geom_unit() { return 0x1p-205; } };
+
+// Extended rungs: the conditioning of the geometry step is MEASURED instead of bounded.  The product of pivot ratios that
+// the double rung uses as `amp` is a worst-case bound: up to 2^130 in corners of the simplex where all photon loops share
+// the dominant electron lines (B nearly of rank one), although the true amplification is far smaller; with that bound the
+// last rung would reject samples whose value is correct to every digit.  Here the elimination is run a second time with
+// the loops in REVERSE order.  The loop matrix B is a sum of at most ten doubles per entry, exact in double-double and
+// beyond, so all the error of the step comes from the elimination, and the two orders round independently: delta = the
+// largest relative difference between the two tables measures it.  Returned in units of geom_unit, with a factor 4; if the
+// two runs share fewer than 30 bits the worst-case bound stays.
+template <class T>
+__device__ __noinline__ double measured_conditioning(const FgGeomDev& E, const double* zl, const T* V, int vs, const T& U, const T& W, double bound) {
+  FgGeomDev R = E;
+  for (int a = 0; a < E.l; ++a) R.line_ph[a] = E.line_ph[E.l - 1 - a];
+  for (int q = 0; q < E.ne; ++q) { unsigned m = 0; for (int a = 0; a < E.l; ++a) if ((E.eta[q] >> a) & 1u) m |= 1u << (E.l - 1 - a); R.eta[q] = (uint8_t)m; }
+  T V2[FG_VMAX], U2, W2; double am, cp;
+  geom_eval<T>(R, zl, V2, 1, U2, W2, am, cp);
+  const int nv = E.ne * (E.ne + 1) / 2 + 2 * E.ne;
+  auto rel = [](const T& a, const T& b) { const double d = to_double(a - b), s = t_abs_d(a); return s != 0.0 ? fabs(d) / s : (d != 0.0 ? 1.0 : 0.0); };
+  double delta = fmax(rel(U, U2), rel(W, W2));
+  for (int i = 0; i < nv; ++i) delta = fmax(delta, rel(V[i * vs], V2[i]));
+  if (!(delta <= 0x1p-30)) return bound;
+  return 4.0 * fmax(delta / prec<T>::geom_unit(), 1.0);
+}
+
 // a5-a7 for the S points of this thread
 template <class T, int S, int ABS>
 __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*z)[FG_MAXM], T* Vt, int vs, T* Sc, int ss, T* I, double* Iabs, double* amx, double* amp, int split) {
@@ -129,6 +159,7 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
     for (int s = 0; s < S; ++s) {
       T U, W; double am, cp;
       geom_eval<T>(E, zl[s], Vt + s, vs, U, W, am, cp);
+      if constexpr (prec<T>::rung >= 1) cp = measured_conditioning<T>(E, zl[s], Vt + s, vs, U, W, cp);
       Sc[(2 * g) * ss + s] = U; Sc[(2 * g + 1) * ss + s] = W;
       if (am > amx[s] || !(am == am)) amx[s] = am;
       if (cp > amp[s] || !(cp == cp)) amp[s] = cp;
@@ -153,12 +184,6 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
 }
 
 
-// Precision rungs (PAPER.md:294-298).  unit: round-off unit of the running error estimate K * u * sum|terms|;
-// geom_unit: relative error of the geometry step per unit of its conditioning `amp`.
-template <class T> struct prec;
-template <> struct prec<double> { static const int rung = 0; static __device__ double unit(double e, double af) { return e * af; } static __device__ double geom_unit() { return 0x1p-109; } };
-template <> struct prec<dd> { static const int rung = 1; static __device__ double unit(double e, double) { return e * 0x1p-51; } static __device__ double geom_unit() { return 0x1p-109; } };
-
 // a8-a9 for one sample: round-off estimate against the tolerance, queueing / rejection, y = I/g, compensated sums
 struct TailAcc { dd sy, sy2; unsigned long long nflag, nrej, nbig; };
 template <class T>
@@ -176,7 +201,7 @@ __device__ __forceinline__ void sample_tail(const FgPlanDev& P, const RunArgs& A
     const bool over = !(err <= tol);
     if (over && A.do_flag) {
       fl = prec<T>::rung == 0 ? 1 : 8; ++ta.nflag;          // queued for the next rung
-      if (A.flag_list) { const unsigned long long pos = atomicAdd(A.flag_count, 1ull); A.flag_list[pos] = (uint32_t)oid; }
+      if (A.flag_bits) atomicOr(&A.flag_bits[oid >> 5], 1u << (oid & 31u));
     } else if (over && prec<T>::rung > 0) {
       fl = 4; ++ta.nrej;     // not resolved by the last rung: contributes 0 and is counted
     } else {
@@ -230,7 +255,7 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
   // then takes about 0.115 + 0.885 / w of a round with one point per thread (measured at w = 32: ~7x shorter) and
   // holds 1/w of the points; w minimises rounds x time per round (the same choice in every block)
   int split = 0;
-  if (is_dd<T>::value && S == 1 && nwork > 0) {
+  if (is_ext<T>::value && S == 1 && nwork > 0) {
     const double cap = (double)gridDim.x * NT; double best = ceil((double)nwork / cap);
     for (int w = 2; w <= 32; w <<= 1) { const double c = ceil((double)nwork * w / cap) * (0.115 + 0.885 / w); if (c < best) { best = c; split = w; } }
   }
@@ -256,7 +281,7 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
     }
     FG_MARK(ring, 0);
     T I[S]; double Iabs[S], growth[S], amp[S];
-    eval_points<T, S, is_dd<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp, split);
+    eval_points<T, S, is_ext<T>::value ? 2 : 1>(P, ring, z, Vt, vs, Sc, ss, I, Iabs, growth, amp, split);
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       if (!valid[s] || (split && (tid & (split - 1)) != 0)) continue;
@@ -413,6 +438,26 @@ __global__ void __launch_bounds__(FG_ST_THREADS, 1) fg_stream_kernel(const FgPla
   block_reduce_tail(ta, (double*)smem /* the ring is idle now */, A.partials + (size_t)blockIdx.x * 8, 4);
 }
 
+// Queue of the next rung: the set bits of `bits` as a list of ordinals in ascending order (one block; deterministic, so
+// the extended-precision passes add their samples in the same order on every run).
+__global__ void __launch_bounds__(1024) fg_compact_kernel(const uint32_t* __restrict__ bits, uint32_t nwords, uint32_t* __restrict__ list, unsigned long long* __restrict__ count) {
+  __shared__ uint32_t part[1024];
+  const uint32_t t = threadIdx.x, per = (nwords + 1023u) / 1024u, w0 = t * per, w1 = min(nwords, w0 + per);
+  uint32_t c = 0;
+  for (uint32_t w = w0; w < w1; ++w) c += __popc(bits[w]);
+  part[t] = c;
+  __syncthreads();
+  for (uint32_t off = 1; off < 1024; off <<= 1) {          // inclusive scan
+    const uint32_t v = t >= off ? part[t - off] : 0u;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  uint32_t pos = part[t] - c;
+  for (uint32_t w = w0; w < w1; ++w) { uint32_t m = bits[w]; while (m) { const int b = __ffs(m) - 1; list[pos++] = w * 32u + (uint32_t)b; m &= m - 1u; } }
+  if (t == 1023) *count = (unsigned long long)part[1023];
+}
+
 __global__ void fg_reduce_kernel(const double* partials, int nparts, Accum* acc, unsigned long long n_add, int finalize, fg_result* out) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   dd a(acc->sy[0], acc->sy[1]), b(acc->sy2[0], acc->sy2[1]);
@@ -475,12 +520,14 @@ __global__ void fg_dmma_kernel(double* out, int iters, double a, double b) {
 using namespace fg;
 
 static thread_local std::string g_err;
-static int fail(int code, const std::string& m) { g_err = m; return code; }
+int fg_internal_fail(int code, const std::string& m) { g_err = m; return code; }     // shared with fg_batch.cpp
+static int fail(int code, const std::string& m) { return fg_internal_fail(code, m); }
 #define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail(FG_E_CUDA, std::string(#x) + ": " + cudaGetErrorString(e_)); } while (0)
 
 struct fg_graph { Graph g; };
 
 static const int NT_Q = 192, S_Q = 1;     // double-double pass: max threads per block (launch bound), samples per thread
+static const int NT_QD = 64;              // quad-double pass
 static const uint64_t SLAB = 1ull << 24;  // samples per slab (bounds the re-evaluation queue)
 static const size_t WAVE_BYTES = (size_t)3 << 30;   // budget of the operand tables one wave of the double pass keeps in HBM
 
@@ -489,10 +536,15 @@ struct fg_plan {
   std::vector<void*> allocs;
   void* scratch = nullptr; double* partials = nullptr; Accum* accum = nullptr; fg_result* result_dev = nullptr;
   uint32_t* flag_list = nullptr; unsigned long long* flag_count = nullptr; unsigned long long* phase_cycles = nullptr;
+  uint32_t* flag_list2 = nullptr; unsigned long long* flag_count2 = nullptr;      // queue of the quad-double rung
+  uint32_t *flag_bits = nullptr, *flag_bits2 = nullptr;                           // one bit per sample of the slab, per queue
+  int grid_qd = 0, nt_qd = 0; size_t smem_qd = 0;
   int grid_d = 0, grid_q = 0, nt_q = 0; size_t smem_d = 0, smem_q = 0; int vmax = 0;
   int wave_nb = 0; double *gV = nullptr, *gUW = nullptr, *gMisc = nullptr;   // wave buffers of the double pass (fg_geom_kernel -> fg_stream_kernel)
   int64_t table_bytes = 0;
-  int profile = 0; cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; double ms[3] = {0, 0, 0}; long long launches = 0, flagged_last = 0;
+  // per-kernel timing: four events per slab, recorded on the launching stream and resolved later (no host synchronisation
+  // inside the timed region); evpool holds the events of the slabs not yet folded into ms[]
+  int profile = 0; std::vector<cudaEvent_t> evpool, evfree; double ms[3] = {0, 0, 0}; long long launches = 0;
   std::mutex mu;
 };
 
@@ -541,7 +593,8 @@ void fg_plan_destroy(fg_plan* p) {
   if (!p) return;
   cudaSetDevice(p->device);
   for (void* a : p->allocs) cudaFree(a);
-  for (int k = 0; k < 4; ++k) if (p->ev[k]) cudaEventDestroy(p->ev[k]);
+  for (cudaEvent_t e : p->evpool) cudaEventDestroy(e);
+  for (cudaEvent_t e : p->evfree) cudaEventDestroy(e);
   delete p;
 }
 
@@ -556,6 +609,7 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   if (o.deg_rule != 0) return fail(FG_E_OPTS, "deg_rule: only rule 0 is available (the paper's Deg algorithm is in its Refs. [42], [32], PAPER.md:250)");
   PlanOpts po; for (int k = 0; k < 4; ++k) po.C[k] = o.C[k]; po.D = o.D; po.merge = o.merge_ext_lines ? 1 : 0;
   po.rel_tol = o.rel_tol; po.abs_tol = o.abs_tol; po.err_factor = o.err_factor;
+  if (!(po.rel_tol >= 0) || !(po.abs_tol >= 0) || (po.rel_tol == 0 && po.abs_tol == 0)) return fail(FG_E_OPTS, "tolerances: need rel_tol >= 0, abs_tol >= 0, not both 0 (every sample would be rejected)");
   int M = 3 * g->g.n - (po.merge ? 1 : 0);
   if (o.deg_table) po.deg_override.assign(o.deg_table, o.deg_table + ((size_t)1 << M));
   fg_plan* p = new fg_plan(); std::string msg;
@@ -590,21 +644,29 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   p->nt_q = fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd));
   if (p->nt_q < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
   p->smem_q = ring_bytes + (size_t)vmax * (p->nt_q * S_Q + FG_VPAD) * sizeof(dd);
+  p->nt_qd = fit(NT_QD, (size_t)vmax * sizeof(qd));
+  if (p->nt_qd < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
+  p->smem_qd = ring_bytes + (size_t)vmax * (p->nt_qd + FG_VPAD) * sizeof(qd);
   // the attribute is per function, not per plan: always raise it to the device limit
   auto setattr = [&](const void* f) { return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max); };
   e = setattr((const void*)fg_stream_kernel); if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<dd, S_Q, NT_Q>);
+  if (e == cudaSuccess) e = setattr((const void*)fg_eval_kernel<qd, 1, NT_QD>);
   if (e != cudaSuccess) { fg_plan_destroy(p); return fail(FG_E_CUDA, std::string("shared memory: ") + cudaGetErrorString(e)); }
   int bps_q = 1;
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_q, fg_eval_kernel<dd, S_Q, NT_Q>, p->nt_q, p->smem_q);
-  p->grid_d = p->sms; p->grid_q = p->sms * std::max(1, std::min(bps_q, 2));
+  p->grid_d = p->sms; p->grid_q = p->sms * std::max(1, std::min(bps_q, 2)); p->grid_qd = p->sms;
   // a wave = a multiple of the grid in batches, bounded by the HBM budget of its operand tables
   { const size_t per_batch = ((size_t)H.vtot * FG_ST_VS + (size_t)(2 * D.ngeom + FG_GM_ROWS) * FG_ST_SAMPLES) * sizeof(double);
     long rounds = (long)(WAVE_BYTES / (per_batch * (size_t)p->grid_d)); rounds = std::max<long>(1, std::min<long>(rounds, 16));
     p->wave_nb = (int)rounds * p->grid_d; }
-  size_t sc = (size_t)H.scratch_slots * std::max((size_t)FG_ST_SAMPLES * sizeof(double) * p->grid_d, (size_t)p->nt_q * S_Q * sizeof(dd) * p->grid_q);
+  size_t sc = (size_t)H.scratch_slots * std::max(std::max((size_t)FG_ST_SAMPLES * sizeof(double) * p->grid_d, (size_t)p->nt_q * S_Q * sizeof(dd) * p->grid_q), (size_t)p->nt_qd * sizeof(qd) * p->grid_qd);
   auto dmalloc = [&](void** d, size_t bytes) { cudaError_t e2 = cudaMalloc(d, bytes); if (e2 == cudaSuccess) { p->allocs.push_back(*d); cudaMemset(*d, 0, bytes); } return e2; };
   e = dmalloc(&p->scratch, sc);
-  if (e == cudaSuccess) e = dmalloc((void**)&p->partials, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->partials, (size_t)(p->grid_d + p->grid_q + p->grid_qd) * 8 * sizeof(double));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->flag_list2, SLAB * sizeof(uint32_t));
+  if (e == cudaSuccess) e = dmalloc((void**)&p->flag_bits, SLAB / 8);
+  if (e == cudaSuccess) e = dmalloc((void**)&p->flag_bits2, SLAB / 8);
+  if (e == cudaSuccess) e = dmalloc((void**)&p->flag_count2, sizeof(unsigned long long));
   if (e == cudaSuccess) e = dmalloc((void**)&p->accum, sizeof(Accum));
   if (e == cudaSuccess) e = dmalloc((void**)&p->result_dev, sizeof(fg_result));
   if (e == cudaSuccess) e = dmalloc((void**)&p->flag_list, SLAB * sizeof(uint32_t));
@@ -618,21 +680,35 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
 }
 
 int fg_plan_set_tol(fg_plan* p, double rel_tol, double abs_tol) {
-  if (!p || !(rel_tol >= 0) || !(abs_tol >= 0)) return fail(FG_E_ARG, "bad tolerance");
+  if (!p || !(rel_tol >= 0) || !(abs_tol >= 0) || (rel_tol == 0 && abs_tol == 0)) return fail(FG_E_ARG, "bad tolerance: need rel_tol >= 0, abs_tol >= 0, not both 0 (every sample would be rejected)");
   std::lock_guard<std::mutex> lk(p->mu);
   p->D.rel_tol = rel_tol; p->D.abs_tol = abs_tol; return FG_OK;
+}
+
+// folds the recorded events into ms[] (waits for the last of them)
+static int resolve_events(fg_plan* p) {
+  for (size_t i = 0; i + 3 < p->evpool.size(); i += 4) {
+    CU(cudaEventSynchronize(p->evpool[i + 3]));
+    for (int k = 0; k < 3; ++k) { float t = 0; CU(cudaEventElapsedTime(&t, p->evpool[i + k], p->evpool[i + k + 1])); p->ms[k] += t; }
+  }
+  p->evfree.insert(p->evfree.end(), p->evpool.begin(), p->evpool.end()); p->evpool.clear();
+  return FG_OK;
 }
 
 int fg_plan_profile(fg_plan* p, int32_t enable) {
   if (!p) return fail(FG_E_ARG, "NULL plan");
   std::lock_guard<std::mutex> lk(p->mu);
   CU(cudaSetDevice(p->device));
-  if (enable) for (int k = 0; k < 4; ++k) if (!p->ev[k]) CU(cudaEventCreate(&p->ev[k]));
+  int rc = resolve_events(p); if (rc != FG_OK) return rc;
   p->profile = enable ? 1 : 0; p->ms[0] = p->ms[1] = p->ms[2] = 0; p->launches = 0;
   return FG_OK;
 }
-int fg_plan_timing(const fg_plan* p, double* ms3, int64_t* launches) {
+int fg_plan_timing(const fg_plan* cp, double* ms3, int64_t* launches) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
   if (!p) return fail(FG_E_ARG, "NULL plan");
+  std::lock_guard<std::mutex> lk(p->mu);
+  CU(cudaSetDevice(p->device));
+  int rc = resolve_events(p); if (rc != FG_OK) return rc;
   if (ms3) for (int k = 0; k < 3; ++k) ms3[k] = p->ms[k];
   if (launches) *launches = p->launches;
   return FG_OK;
@@ -691,7 +767,7 @@ int fg_host_plan(const fg_graph* g, const fg_plan_opts* opts, fg_plan_stats* sta
 
 int fg_plan_info(const fg_plan* p, fg_plan_stats* s) {
   if (!p || !s) return fail(FG_E_ARG, "NULL argument");
-  fill_stats(p->H, s); s->table_bytes = p->table_bytes;
+  fill_stats(p->H, s); s->table_bytes = p->table_bytes; s->wave_samples = (int64_t)p->wave_nb * FG_ST_SAMPLES;
   return FG_OK;
 }
 
@@ -729,13 +805,21 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
   RunArgs A; std::memset(&A, 0, sizeof(A));
   A.first = first; A.n = n; A.seed = seed; A.zin = zin; A.outI = dI; A.outId = dId; A.outY = dY; A.outErr = dErr; A.outFlags = dFl;
   A.scratch = p->scratch; A.phase_cycles = p->phase_cycles;
-  int nparts = 0;
-  CU(cudaMemsetAsync(p->partials, 0, (size_t)(p->grid_d + p->grid_q) * 8 * sizeof(double), st));
-  if (mode != 2) {
-    CU(cudaMemsetAsync(p->flag_count, 0, sizeof(unsigned long long), st));
-    A.flag_list = p->flag_list; A.flag_count = p->flag_count; A.do_flag = (mode == 0); A.partials = p->partials;
+  const int nparts = p->grid_d + p->grid_q + p->grid_qd;
+  CU(cudaMemsetAsync(p->partials, 0, (size_t)nparts * 8 * sizeof(double), st));
+  const uint32_t nwords = (uint32_t)((n + 31) / 32);
+  CU(cudaMemsetAsync(p->flag_count, 0, sizeof(unsigned long long), st));
+  CU(cudaMemsetAsync(p->flag_count2, 0, sizeof(unsigned long long), st));
+  CU(cudaMemsetAsync(p->flag_bits, 0, (size_t)nwords * 4, st));
+  CU(cudaMemsetAsync(p->flag_bits2, 0, (size_t)nwords * 4, st));
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  if (p->profile) {
+    for (int k = 0; k < 4; ++k) { if (!p->evfree.empty()) { ev[k] = p->evfree.back(); p->evfree.pop_back(); } else CU(cudaEventCreate(&ev[k])); p->evpool.push_back(ev[k]); }
+    CU(cudaEventRecord(ev[0], st));
+  }
+  if (mode <= 1) {          // first rung: double precision; ill-conditioned samples go to the queue of the double-double rung
+    A.flag_bits = p->flag_bits; A.do_flag = (mode == 0); A.partials = p->partials;
     A.gV = p->gV; A.gUW = p->gUW; A.gMisc = p->gMisc;
-    if (p->profile) CU(cudaEventRecord(p->ev[0], st));
     const uint64_t nbatch = (n + FG_ST_SAMPLES - 1) / FG_ST_SAMPLES;
     for (uint64_t b0 = 0; b0 < nbatch; b0 += (uint64_t)p->wave_nb) {      // waves: geometry of a wave, then its record streams
       A.ord0 = b0 * FG_ST_SAMPLES; A.nb = (int)std::min<uint64_t>((uint64_t)p->wave_nb, nbatch - b0);
@@ -744,30 +828,35 @@ static int run_slab(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, cudaS
       fg_stream_kernel<<<std::min(p->grid_d, A.nb), FG_ST_THREADS, p->smem_d, st>>>(p->D, A);
       CU(cudaGetLastError()); ++p->launches;
     }
-    if (p->profile) CU(cudaEventRecord(p->ev[1], st));
-    nparts = p->grid_d;
   }
-  if (mode == 0 || mode == 2) {
-    RunArgs B = A; B.phase_cycles = nullptr; B.do_flag = 0; B.ord0 = 0; B.nb = 0; B.flag_list = nullptr; B.outId = nullptr; B.outErr = nullptr; B.partials = p->partials + (size_t)p->grid_d * 8;
-    if (mode == 0) { B.idlist = p->flag_list; B.idcount = p->flag_count; }
-    if (p->profile && mode == 2) { CU(cudaEventRecord(p->ev[0], st)); CU(cudaEventRecord(p->ev[1], st)); }
+  if (mode == 0) { fg_compact_kernel<<<1, 1024, 0, st>>>(p->flag_bits, nwords, p->flag_list, p->flag_count); CU(cudaGetLastError()); ++p->launches; }
+  if (p->profile) CU(cudaEventRecord(ev[1], st));
+  RunArgs B = A; B.phase_cycles = nullptr; B.ord0 = 0; B.nb = 0; B.outId = nullptr;
+  if (mode == 0 || mode == 2) {     // second rung: double-double over the queue (mode 2: over every point); its own queue feeds the third
+    B.partials = p->partials + (size_t)p->grid_d * 8;
+    B.idlist = mode == 0 ? p->flag_list : nullptr; B.idcount = mode == 0 ? p->flag_count : nullptr;
+    B.do_flag = 1; B.flag_bits = p->flag_bits2;
+    if (mode == 0) B.outErr = nullptr;
     fg_eval_kernel<dd, S_Q, NT_Q><<<p->grid_q, p->nt_q, p->smem_q, st>>>(p->D, B);
     CU(cudaGetLastError()); ++p->launches;
-    nparts = p->grid_d + p->grid_q;
+    fg_compact_kernel<<<1, 1024, 0, st>>>(p->flag_bits2, nwords, p->flag_list2, p->flag_count2); CU(cudaGetLastError()); ++p->launches;
   }
-  if (p->profile) CU(cudaEventRecord(p->ev[2], st));
+  if (mode == 0 || mode == 2 || mode == 3) {     // third rung: quad-double; what it cannot resolve contributes 0
+    B.partials = p->partials + (size_t)(p->grid_d + p->grid_q) * 8;
+    B.idlist = mode == 3 ? nullptr : p->flag_list2; B.idcount = mode == 3 ? nullptr : p->flag_count2;
+    B.do_flag = 0; B.flag_bits = nullptr;
+    B.outErr = mode == 3 ? A.outErr : nullptr;
+    fg_eval_kernel<qd, 1, NT_QD><<<p->grid_qd, p->nt_qd, p->smem_qd, st>>>(p->D, B);
+    CU(cudaGetLastError()); ++p->launches;
+  }
+  if (p->profile) CU(cudaEventRecord(ev[2], st));
   fg_reduce_kernel<<<1, 32, 0, st>>>(p->partials, nparts, p->accum, (unsigned long long)n, finalize ? 1 : 0, out_dev);
   CU(cudaGetLastError()); ++p->launches;
-  if (p->profile) {
-    CU(cudaEventRecord(p->ev[3], st)); CU(cudaEventSynchronize(p->ev[3]));
-    for (int k = 0; k < 3; ++k) { float t = 0; CU(cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1])); p->ms[k] += t; }
-  }
+  if (p->profile) CU(cudaEventRecord(ev[3], st));
   return FG_OK;
 }
 
-int fg_integrate_async(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, void* out_dev) {
-  fg_plan* p = const_cast<fg_plan*>(cp);
-  if (!p || !out_dev) return fail(FG_E_ARG, "NULL argument");
+static int integrate_locked(fg_plan* p, uint64_t first, uint64_t n, uint64_t seed, void* stream, void* out_dev) {
   if (n == 0) return fail(FG_E_ARG, "n_samples must be > 0");
   cudaStream_t st = (cudaStream_t)stream;
   CU(cudaSetDevice(p->device));
@@ -780,11 +869,18 @@ int fg_integrate_async(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t s
   return FG_OK;
 }
 
+int fg_integrate_async(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, void* out_dev) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
+  if (!p || !out_dev) return fail(FG_E_ARG, "NULL argument");
+  std::lock_guard<std::mutex> lk(p->mu);      // the launches of one call are enqueued atomically; see fg.h for stream rules
+  return integrate_locked(p, first, n, seed, stream, out_dev);
+}
+
 int fg_integrate_range(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t seed, void* stream, fg_result* out) {
   fg_plan* p = const_cast<fg_plan*>(cp);
   if (!p || !out) return fail(FG_E_ARG, "NULL argument");
   std::lock_guard<std::mutex> lk(p->mu);
-  int rc = fg_integrate_async(p, first, n, seed, stream, p->result_dev);
+  int rc = integrate_locked(p, first, n, seed, stream, p->result_dev);
   if (rc != FG_OK) return rc;
   CU(cudaMemcpyAsync(out, p->result_dev, sizeof(fg_result), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   CU(cudaStreamSynchronize((cudaStream_t)stream));
@@ -853,7 +949,7 @@ static int eval_common(fg_plan* p, const double* z_host, uint64_t first, uint64_
 
 int fg_eval_points(const fg_plan* cp, const double* z, uint64_t n, int32_t mode, void* stream, double* I, double* I_double, double* err, uint8_t* flags) {
   if (!cp || (!z && n)) return fail(FG_E_ARG, "NULL argument");
-  if (mode < 0 || mode > 2) return fail(FG_E_ARG, "mode must be 0, 1 or 2");
+  if (mode < 0 || mode > 3) return fail(FG_E_ARG, "mode must be 0, 1, 2 or 3");
   return eval_common(const_cast<fg_plan*>(cp), z, 0, n, 0, mode, (cudaStream_t)stream, I, I_double, nullptr, err, flags);
 }
 

@@ -554,10 +554,10 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       std::vector<int> nk = {gi, op_of[m]}; int ni; auto it2 = nmap.find(nk);
       if (it2 == nmap.end()) { ni = (int)P.nums.size(); HNum N; N.geom = gi; N.op = op_of[m]; N.ncomp = P.subs[m].type == 0 ? 2 : 1; N.nse = (int)P.geoms[gi].se_kids.size(); P.nums.push_back(N); nmap[nk] = ni; } else ni = it2->second;
       HNode nd; nd.num = ni; std::vector<int> key = {ni};
-      const HGeom& E = P.geoms[gi];
-      for (int c : E.se_kids) { int id = go(P, c, kids_of, op_of, geom_of, gmap, nmap, ndmap); nd.se_kid.push_back(id); key.push_back(id); }
+      const std::vector<int> se_kids = P.geoms[gi].se_kids, vc_kids = P.geoms[gi].vc_kids;   // copies: the recursion grows P.geoms
+      for (int c : se_kids) { int id = go(P, c, kids_of, op_of, geom_of, gmap, nmap, ndmap); nd.se_kid.push_back(id); key.push_back(id); }
       key.push_back(-1);
-      for (int c : E.vc_kids) { int id = go(P, c, kids_of, op_of, geom_of, gmap, nmap, ndmap); nd.vc_kid.push_back(id); key.push_back(id); }
+      for (int c : vc_kids) { int id = go(P, c, kids_of, op_of, geom_of, gmap, nmap, ndmap); nd.vc_kid.push_back(id); key.push_back(id); }
       auto it3 = ndmap.find(key); if (it3 != ndmap.end()) return it3->second;
       int id = (int)P.nodes.size(); P.nodes.push_back(nd); ndmap[key] = id; return id;
     } };

@@ -14,7 +14,9 @@ LIB_PATH = os.environ.get("FG_LIB") or os.path.join(_HERE, "libfg.so")     # FG_
 EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_plan_create", "fg_plan_destroy",
            "fg_plan_info", "fg_plan_phase_cycles", "fg_host_plan", "fg_host_dirac_table", "fg_plan_set_tol", "fg_plan_profile", "fg_plan_timing", "fg_plan_structure", "fg_plan_tables", "fg_integrate", "fg_integrate_range",
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
-           "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version"]
+           "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version",
+           "fg_batch_create", "fg_batch_destroy", "fg_batch_pilot", "fg_batch_set_times", "fg_batch_probabilities", "fg_batch_next",
+           "fg_batch_fold", "fg_batch_run", "fg_batch_result", "fg_batch_total"]
 
 
 class FgError(RuntimeError):
@@ -38,7 +40,7 @@ class fg_plan_stats(C.Structure):
                 ("n_terms", C.c_int32), ("n_geoms", C.c_int32), ("n_nums", C.c_int32), ("n_nodes", C.c_int32),
                 ("n_records", C.c_int64), ("n_coefs", C.c_int64), ("n_coefs_nonzero", C.c_int64),
                 ("table_bytes", C.c_int64), ("stream_bytes", C.c_int64), ("flops_per_sample", C.c_double),
-                ("exec_flops_per_sample", C.c_double), ("plan_seconds", C.c_double)]
+                ("exec_flops_per_sample", C.c_double), ("plan_seconds", C.c_double), ("wave_samples", C.c_int64)]
 
 
 class fg_result(C.Structure):
@@ -87,6 +89,16 @@ def lib():
         L.fg_sample_eval_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp] + [vp] * 3
         L.fg_dfma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.fg_dmma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.fg_batch_create.argtypes = [vp, C.c_int32, C.POINTER(vp)]
+        L.fg_batch_destroy.argtypes = [vp]
+        L.fg_batch_pilot.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, C.c_double, vp]
+        L.fg_batch_set_times.argtypes = [vp, vp]
+        L.fg_batch_probabilities.argtypes = [vp, vp]
+        L.fg_batch_next.argtypes = [vp, C.c_uint64, C.c_uint64, C.POINTER(C.c_int32), C.POINTER(C.c_uint64)]
+        L.fg_batch_fold.argtypes = [vp, C.c_int32, C.POINTER(fg_result), C.c_double]
+        L.fg_batch_run.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, vp]
+        L.fg_batch_result.argtypes = [vp, C.c_int32, C.POINTER(fg_result), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.fg_batch_total.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
         for f in ("fg_strerror", "fg_last_error_message", "fg_version"):
             getattr(L, f).restype = C.c_char_p
         L.fg_strerror.argtypes = [C.c_int]
@@ -183,6 +195,10 @@ class Plan:
         c = np.zeros(16, dtype=np.uint64)
         rc = _check(lib().fg_plan_phase_cycles(self.h, _p(c), int(bool(reset))))
         return bool(rc), c
+
+    def wave_samples(self):
+        """Samples of one wave of the double-precision pass (one fg_geom_kernel + one fg_stream_kernel launch)."""
+        return int(self.stats["wave_samples"])
 
     def structure(self):
         ns = self.stats["n_subgraphs"]
