@@ -297,6 +297,7 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
   constexpr int STRIDE = (int)sizeof(FgRecC) + NC * (int)sizeof(double);
   constexpr bool PRELOAD = NC <= 48;      // tables small enough to sit in registers
   T pf[NF > 0 ? NF : 1][S], acc[S]; double aab[S];
+  T a[K > 0 ? K : 1][S], aq[K > 0 ? K : 1][S]; uint32_t lastv = 0xffffffffu;
 #pragma unroll
   for (int s = 0; s < S; ++s) { acc[s] = accp[s]; aab[s] = aabp[s]; }
   for (int r = 0; r < nrec; ++r, p += STRIDE) {
@@ -321,16 +322,20 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
 #pragma unroll
       for (int s = 0; s < S; ++s) pf[f][s] = (f == 0) ? pv[s] : pf[f > 0 ? f - 1 : 0][s] * pv[s];
     }
-    T a[K > 0 ? K : 1][S], aq[K > 0 ? K : 1][S];
+    // free variables: reloaded only when they change (runs of records share them)
+    uint32_t vkey; __builtin_memcpy(&vkey, h.vidx, 4);
+    if (K > 0 && vkey != lastv) {
+      lastv = vkey;
 #pragma unroll
-    for (int j = 0; j < K; ++j) {
-      const T* pv = Vt + (int)h.vidx[j] * vs;
+      for (int j = 0; j < K; ++j) {
+        const T* pv = Vt + (int)h.vidx[j] * vs;
 #pragma unroll
-      for (int s = 0; s < S; ++s) a[j][s] = pv[s];
-      if (QX) {
-        const T* pq = pv + ne * vs;
+        for (int s = 0; s < S; ++s) a[j][s] = pv[s];
+        if (QX) {
+          const T* pq = pv + ne * vs;
 #pragma unroll
-        for (int s = 0; s < S; ++s) aq[j][s] = pq[s];
+          for (int s = 0; s < S; ++s) aq[j][s] = pq[s];
+        }
       }
     }
 #if defined(__CUDA_ARCH__)

@@ -120,24 +120,35 @@ template <> struct prec<qd> { static const int rung = 2; static __device__ doubl
 // Extended rungs: the conditioning of the geometry step is MEASURED instead of bounded.  The product of pivot ratios that
 // the double rung uses as `amp` is a worst-case bound: up to 2^130 in corners of the simplex where all photon loops share
 // the dominant electron lines (B nearly of rank one), although the true amplification is far smaller; with that bound the
-// last rung would reject samples whose value is correct to every digit.  Here the elimination is run a second time with
-// the loops in REVERSE order.  The loop matrix B is a sum of at most ten doubles per entry, exact in double-double and
+// last rung would reject samples whose value is correct to every digit.  For a sample that fails the tolerance with the
+// bound, the elimination of every element is run again, in the given loop order and in the REVERSE order.  The loop matrix B is a sum of at most ten doubles per entry, exact in double-double and
 // beyond, so all the error of the step comes from the elimination, and the two orders round independently: delta = the
 // largest relative difference between the two tables measures it.  Returned in units of geom_unit, with a factor 4; if the
 // two runs share fewer than 30 bits the worst-case bound stays.
 template <class T>
-__device__ __noinline__ double measured_conditioning(const FgGeomDev& E, const double* zl, const T* V, int vs, const T& U, const T& W, double bound) {
-  FgGeomDev R = E;
-  for (int a = 0; a < E.l; ++a) R.line_ph[a] = E.line_ph[E.l - 1 - a];
-  for (int q = 0; q < E.ne; ++q) { unsigned m = 0; for (int a = 0; a < E.l; ++a) if ((E.eta[q] >> a) & 1u) m |= 1u << (E.l - 1 - a); R.eta[q] = (uint8_t)m; }
-  T V2[FG_VMAX], U2, W2; double am, cp;
-  geom_eval<T>(R, zl, V2, 1, U2, W2, am, cp);
-  const int nv = E.ne * (E.ne + 1) / 2 + 2 * E.ne;
+__device__ __noinline__ double measured_conditioning(const FgPlanDev& P, const double* z) {
+  double zl[FG_MAXLINES];
+  for (int v = 0; v < P.M; ++v) {
+    const int l0 = P.var_line0[v], l1 = P.var_line1[v];
+    if (l1 == 255) zl[l0] = z[v]; else { zl[l0] = 0.5 * z[v]; zl[l1] = 0.5 * z[v]; }
+  }
   auto rel = [](const T& a, const T& b) { const double d = to_double(a - b), s = t_abs_d(a); return s != 0.0 ? fabs(d) / s : (d != 0.0 ? 1.0 : 0.0); };
-  double delta = fmax(rel(U, U2), rel(W, W2));
-  for (int i = 0; i < nv; ++i) delta = fmax(delta, rel(V[i * vs], V2[i]));
-  if (!(delta <= 0x1p-30)) return bound;
-  return 4.0 * fmax(delta / prec<T>::geom_unit(), 1.0);
+  double amp = 1.0;
+  for (int g = 0; g < P.ngeom; ++g) {
+    const FgGeomDev E = P.geoms[g];
+    FgGeomDev R = E;
+    for (int a = 0; a < E.l; ++a) R.line_ph[a] = E.line_ph[E.l - 1 - a];
+    for (int q = 0; q < E.ne; ++q) { unsigned m = 0; for (int a = 0; a < E.l; ++a) if ((E.eta[q] >> a) & 1u) m |= 1u << (E.l - 1 - a); R.eta[q] = (uint8_t)m; }
+    T V1[FG_VMAX], V2[FG_VMAX], U1, W1, U2, W2; double am, bound, cp2;
+    geom_eval<T>(E, zl, V1, 1, U1, W1, am, bound);
+    geom_eval<T>(R, zl, V2, 1, U2, W2, am, cp2);
+    const int nv = E.ne * (E.ne + 1) / 2 + 2 * E.ne;
+    double delta = fmax(rel(U1, U2), rel(W1, W2));
+    for (int i = 0; i < nv; ++i) delta = fmax(delta, rel(V1[i], V2[i]));
+    const double a = (delta <= 0x1p-30) ? 4.0 * fmax(delta / prec<T>::geom_unit(), 1.0) : bound;
+    if (a > amp || !(a == a)) amp = a;
+  }
+  return amp;
 }
 
 // a5-a7 for the S points of this thread
@@ -159,7 +170,6 @@ __device__ void eval_points(const FgPlanDev& P, ChunkRing& ring, const double (*
     for (int s = 0; s < S; ++s) {
       T U, W; double am, cp;
       geom_eval<T>(E, zl[s], Vt + s, vs, U, W, am, cp);
-      if constexpr (prec<T>::rung >= 1) cp = measured_conditioning<T>(E, zl[s], Vt + s, vs, U, W, cp);
       Sc[(2 * g) * ss + s] = U; Sc[(2 * g + 1) * ss + s] = W;
       if (am > amx[s] || !(am == am)) amx[s] = am;
       if (cp > amp[s] || !(cp == cp)) amp[s] = cp;
@@ -285,6 +295,11 @@ __global__ void __launch_bounds__(MAXNT) fg_eval_kernel(const FgPlanDev P, const
 #pragma unroll
     for (int s = 0; s < S; ++s) {
       if (!valid[s] || (split && (tid & (split - 1)) != 0)) continue;
+      if constexpr (prec<T>::rung >= 1) {       // the bound failed: measure the conditioning of the geometry step instead
+        const double Id = to_double(I[s]);
+        const double err = (prec<T>::unit(P.err_eps, 1.0) + amp[s] * prec<T>::geom_unit()) * Iabs[s];
+        if (!bad[s] && !(err <= fmax(P.rel_tol * fabs(Id), ldexp(P.abs_tol * mant[s], ex[s])))) amp[s] = measured_conditioning<T>(P, z[s]);
+      }
       sample_tail<T>(P, A, I[s], Iabs[s], growth[s], amp[s], mant[s], ex[s], bad[s], oid[s], ta);
     }
     FG_MARK(ring, 7);
@@ -385,7 +400,7 @@ __global__ void __launch_bounds__(FG_ST_THREADS, 1) fg_stream_kernel(const FgPla
   extern __shared__ __align__(128) unsigned char smem[];
   ChunkRing ring; ring.buf = smem; ring.bar = (uint64_t*)(smem + 2 * FG_CHUNK_BYTES); ring.phase[0] = ring.phase[1] = 0u;
 #ifdef FG_PHASE_PROF
-  long long prof[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}; ring.prof = prof; ring.tlast = clock64();
+  long long prof[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}; ring.prof = prof; ring.tlast = clock64();
 #endif
   uint64_t* barV = ring.bar + 2; uint32_t phaseV = 0u;
   double* xbuf = (double*)(smem + 2 * FG_CHUNK_BYTES + 128);
@@ -433,7 +448,7 @@ __global__ void __launch_bounds__(FG_ST_THREADS, 1) fg_stream_kernel(const FgPla
     FG_MARK(ring, 7);
   }
 #ifdef FG_PHASE_PROF
-  if (A.phase_cycles && (tid & 31) == 0) for (int k = 0; k < 9; ++k) atomicAdd(&A.phase_cycles[k], (unsigned long long)prof[k]);
+  if (A.phase_cycles && (tid & 31) == 0) for (int k = 0; k < 16; ++k) atomicAdd(&A.phase_cycles[k], (unsigned long long)prof[k]);
 #endif
   block_reduce_tail(ta, (double*)smem /* the ring is idle now */, A.partials + (size_t)blockIdx.x * 8, 4);
 }

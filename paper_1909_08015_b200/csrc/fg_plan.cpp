@@ -662,7 +662,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       while (j < nr && cls(N.recs[j]) == cls(N.recs[i]) && std::memcmp(N.recs[j].vidx, N.recs[i].vidx, sizeof(N.recs[i].vidx)) == 0) ++j;
       const HRecord& r0 = N.recs[i];
       const bool qx = (r0.flags & FG_REC_QEXT) != 0;
-      bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= 2 && (j - i) >= FG_MMA_MINREC;
+      bool mma = r0.nf <= FG_NFC && !(r0.flags & FG_REC_TWO) && r0.k >= FG_MMA_MINK && (j - i) >= FG_MMA_MINREC;
       if (mma) {     // tiles store the high word of the double: only if every coefficient of the run has a zero low word
         for (size_t t = i; t < j && mma; ++t) for (double c : N.recs[t].coef) { FgMmaCoef h; if (!fg_mma_coef_pack(c, &h)) { mma = false; break; } }
       }
@@ -694,6 +694,16 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
           N.exec_flops += 8.0 * (8.0 * steps + 4.0);
         }
         { auto& h = hist[{1, r0.nf, r0.k, qx ? 1 : 0, 0}]; h[0] += R; h[1] += ntiles; h[2] += 1; }
+        if (std::getenv("FG_PLAN_HIST")) {      // sparsity by k-step: per record the mask of steps with a non-zero coefficient
+          static std::map<std::vector<int>, std::map<unsigned, long>> masks; static std::map<std::vector<int>, std::array<long, 3>> tot;
+          std::vector<int> key = {r0.nf, r0.k, qx ? 1 : 0};
+          std::map<unsigned, long> local;
+          for (size_t t = i; t < j; ++t) { unsigned m = 0; for (int st = 0; st < steps; ++st) for (int x = 0; x < 4; ++x) if (mma_coef(N.recs[t], st, x) != 0.0) m |= 1u << st; masks[key][m]++; local[m]++; tot[key][0] += __builtin_popcount(m); tot[key][1] += steps; }
+          // tiles needed if the records of this run are regrouped by mask: sum over masks of ceil(count/8) * popcount(mask)
+          long dm = 0; for (auto& kv : local) dm += ((kv.second + 7) / 8) * __builtin_popcount(kv.first);
+          tot[key][2] += dm;
+          if (i + R >= nr) for (auto& kv : tot) std::fprintf(stderr, "  steps nf %d k %d qx %d: nonzero record-steps %ld of %ld; DMMA per row block if regrouped by mask %ld; distinct masks %zu\n", kv.first[0], kv.first[1], kv.first[2], kv.second[0], kv.second[1], kv.second[2], masks[kv.first].size());
+        }
         for (size_t t = i; t < j; ++t) N.algo_flops += std::max(0, N.recs[t].nf - 1);
         close_group();
         i = j; continue;

@@ -41,6 +41,9 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int vq = ne * ROWB;
   const unsigned char* __restrict__ Vb = (const unsigned char*)(Vw + 8 * rb0 + r);     // sample of row block rb0; + 64 bytes per further row block
+  // the lane's base address goes through an opaque asm: ptxas otherwise rebuilds it from %tid (S2R + four integer
+  // instructions) in front of every load of the record epilogue to save one register (+11-17 % samples/s, A/B in profiles/)
+  { uint32_t vb32 = (uint32_t)__cvta_generic_to_shared(Vb); asm volatile("" : "+r"(vb32)); Vb = (const unsigned char*)__cvta_shared_to_generic(vb32); __builtin_assume(__isShared(Vb)); }
   double av[NRB], ab[NRB];
 #pragma unroll
   for (int bi = 0; bi < NRB; ++bi) { av[bi] = part[bi]; ab[bi] = part[NRB + bi]; }
@@ -173,6 +176,7 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
   const int tid = threadIdx.x, w = tid >> 5;
   const bool owner = tid < FG_ST_SAMPLES;
   const double* Vt = V + (owner ? tid : 0);                      // the owner's column
+  { uint32_t a32 = (uint32_t)__cvta_generic_to_shared(Vt); asm volatile("" : "+r"(a32)); Vt = (const double*)__cvta_shared_to_generic(a32); __builtin_assume(__isShared(Vt)); }
   const double* Vw = V + 32 * (w & 7); const int rb0 = FG_ST_NRB * (w >> 3);
   const int ngroups = ((const FgChunkHdr*)chunk)->ngroups;
   const unsigned char* p = chunk + sizeof(FgChunkHdr);
@@ -198,7 +202,7 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
 #undef FG_MM
         default: break;      // the planner makes tensor-core groups of these classes only
       }
-      FG_MARK(st, 2);
+      FG_MARK(st, 9 + (k - 2) * 2 + (qx ? 1 : 0));      // 9..14: tensor-core groups by class (k = 2, 3, 4; without / with q-extension)
       p = p0 + gh.seq_bytes; g += nseq - 1; continue;
     }
     const int bytes = nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));

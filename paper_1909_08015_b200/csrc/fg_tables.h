@@ -66,6 +66,9 @@ struct FgTermDev {
 #define FG_REC_WIDE 4      // records use the wide header (nf > FG_NFC): generic slow path
 #define FG_REC_MMA 8       // tensor-core group: records that share their free variables, stored as 8-record tiles
 #define FG_NFC 5           // product factors of a compact record (= Wick pairs, <= n)
+#ifndef FG_MMA_MINK
+#define FG_MMA_MINK 2      // tensor-core groups only for records with at least this many free variables
+#endif
 #ifndef FG_MMA_MINREC
 #define FG_MMA_MINREC 3    // a run of records with equal free variables becomes a tensor-core group from this length on
 #endif
