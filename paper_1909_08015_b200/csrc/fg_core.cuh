@@ -288,7 +288,7 @@ template <int N> struct PreLoad<N, N> { static __device__ __forceinline__ void r
 #define FG_NOINLINE inline
 #endif
 template <class T, int S, int ABS, int NF, int K, bool QX>
-FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* __restrict__ accp, double* __restrict__ aabp) {
+FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* __restrict__ accp, double* __restrict__ aabp, int r0 = 0) {   // records r0 .. nrec-1 (r0 > 0: a second thread set takes the rest; its first record rebuilds the whole prefix)
 #if defined(__CUDA_ARCH__)
   __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vt));
 #endif
@@ -300,7 +300,8 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
   T a[K > 0 ? K : 1][S], aq[K > 0 ? K : 1][S]; uint32_t lastv = 0xffffffffu;
 #pragma unroll
   for (int s = 0; s < S; ++s) { acc[s] = accp[s]; aab[s] = aabp[s]; }
-  for (int r = 0; r < nrec; ++r, p += STRIDE) {
+  p += (size_t)r0 * STRIDE;
+  for (int r = r0; r < nrec; ++r, p += STRIDE) {
     const FgRecC h = *(const FgRecC*)p;
     const double* __restrict__ coef = (const double*)(p + sizeof(FgRecC));
     double cr[PRELOAD ? NC : 2];
@@ -315,7 +316,7 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
 #endif
     }
     const double* __restrict__ cc = PRELOAD ? cr : coef;
-    const int keep = h.keep;
+    const int keep = (r == r0 && r0 > 0) ? 0 : h.keep;
 #pragma unroll
     for (int f = 0; f < NF; ++f) if (f >= keep) {
       const T* pv = Vt + (int)h.fidx[f] * vs;
@@ -338,7 +339,7 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
         }
       }
     }
-#if defined(__CUDA_ARCH__)
+#if defined(__CUDA_ARCH__) && defined(FG_STATIC_SYNCWARP)
     __syncwarp();   // scheduling fence: every load of the record is issued before the first FMA waits on one
 #endif
     T q[S];

@@ -352,8 +352,8 @@ __global__ void __launch_bounds__(FG_ST_SAMPLES) fg_geom_kernel(const FgPlanDev 
 }
 
 // ---- double-precision pass, second kernel: a6-a10 ------------------------------------------------------------------
-// shared memory: [ring 2 x FG_CHUNK_BYTES][3 mbarriers, 128 B][exchange buffer 2 x FG_ST_SAMPLES doubles][V: vmax rows]
-#define FG_ST_XBUF_BYTES (2 * FG_ST_SAMPLES * 8)
+// shared memory: [ring 2 x FG_CHUNK_BYTES][3 mbarriers, 128 B][exchange buffer 4 x FG_ST_SAMPLES doubles][V: vmax rows]
+#define FG_ST_XBUF_BYTES (4 * FG_ST_SAMPLES * 8)
 #define FG_ST_SMEM(vmax) (2 * FG_CHUNK_BYTES + 128 + FG_ST_XBUF_BYTES + (size_t)(vmax) * FG_ST_VS * 8)
 
 __device__ void run_program_s(const FgPlanDev& P, const FgNumDev& N, const ScratchMap& sm, ChunkRing& ring, const double* V, int ne, double* Sc, double* xbuf) {
@@ -368,7 +368,7 @@ __device__ void run_program_s(const FgPlanDev& P, const FgNumDev& N, const Scrat
     mbar_expect_tx(&ring.bar[0], used[0]); bulk_g2s(ring.buf, g0, used[0], &ring.bar[0]);
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
   }
-  StreamState st; st.cur = -1; st.has_part = 0; st.acc[0] = st.acc[1] = st.aab[0] = st.aab[1] = 0.0;
+  StreamState st; st.cur = -1; st.has_part = 0; st.has_half = 0; st.has_two = 0; st.acc[0] = st.acc[1] = st.aab[0] = st.aab[1] = 0.0;
 #pragma unroll
   for (int i = 0; i < 2 * FG_ST_NRB; ++i) st.part[i] = 0.0;
 #ifdef FG_PHASE_PROF

@@ -143,30 +143,46 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
 // Running state of one program in the stream kernel.  acc/aab: accumulators of the current destination (owner threads:
 // thread t < FG_ST_SAMPLES owns sample t of the batch); part: per-lane tensor-core partial sums (all threads).
 struct StreamState {
-  double acc[2], aab[2], part[2 * FG_ST_NRB]; int cur, has_part;
+  double acc[2], aab[2], part[2 * FG_ST_NRB]; int cur, has_part, has_half, has_two;
 #ifdef FG_PHASE_PROF
   long long* prof; long long tlast;
 #endif
 };
 
-// Hand the tensor-core partial sums to the owner threads: quad-reduce, lane c == 0 of quad r posts the sums of sample
-// 32*sg + 8*b + r in the exchange buffer, the owner adds them.  Block-uniform (every warp walks the same stream), two
-// block barriers; called when the destination changes and at the end of a program.
+// Hand the partial sums to the owner threads.  Tensor-core groups: quad-reduce, lane c == 0 of quad r posts the sums of sample
+// 32*sg + 8*b + r.  Scalar groups: the helper thread t + 256 (which ran the second half of the records of every scalar group
+// on the operands of sample t) posts its accumulators.  The owner adds both.  Block-uniform (every warp walks the same
+// stream), two block barriers (four if two-component records were met); called when the destination changes and at the
+// end of a program.  xbuf: [0, 512) tensor-core pairs, [512, 1024) helper pairs.
 __device__ __forceinline__ void fold_parts(StreamState& st, double* __restrict__ xbuf) {
-  if (!st.has_part) return;
+  if (!st.has_part && !st.has_half) return;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, sg = w & 7, rb0 = FG_ST_NRB * (w >> 3);
+  const bool owner = tid < FG_ST_SAMPLES;
+  if (st.has_part) {
 #pragma unroll
-  for (int bi = 0; bi < FG_ST_NRB; ++bi) {
-    double v = st.part[bi], a = st.part[FG_ST_NRB + bi];
-    v += __shfl_xor_sync(0xffffffffu, v, 1); a += __shfl_xor_sync(0xffffffffu, a, 1);
-    v += __shfl_xor_sync(0xffffffffu, v, 2); a += __shfl_xor_sync(0xffffffffu, a, 2);
-    if ((lane & 3) == 0) { const int smp = 32 * sg + 8 * (rb0 + bi) + (lane >> 2); xbuf[2 * smp] = v; xbuf[2 * smp + 1] = a; }
-    st.part[bi] = 0.0; st.part[FG_ST_NRB + bi] = 0.0;
+    for (int bi = 0; bi < FG_ST_NRB; ++bi) {
+      double v = st.part[bi], a = st.part[FG_ST_NRB + bi];
+      v += __shfl_xor_sync(0xffffffffu, v, 1); a += __shfl_xor_sync(0xffffffffu, a, 1);
+      v += __shfl_xor_sync(0xffffffffu, v, 2); a += __shfl_xor_sync(0xffffffffu, a, 2);
+      if ((lane & 3) == 0) { const int smp = 32 * sg + 8 * (rb0 + bi) + (lane >> 2); xbuf[2 * smp] = v; xbuf[2 * smp + 1] = a; }
+      st.part[bi] = 0.0; st.part[FG_ST_NRB + bi] = 0.0;
+    }
+  }
+  if (st.has_half && !owner) { xbuf[2 * FG_ST_SAMPLES + 2 * (tid - FG_ST_SAMPLES)] = st.acc[0]; xbuf[2 * FG_ST_SAMPLES + 2 * (tid - FG_ST_SAMPLES) + 1] = st.aab[0]; }
+  __syncthreads();
+  if (owner) {
+    if (st.has_part) { st.acc[0] += xbuf[2 * tid]; st.aab[0] += xbuf[2 * tid + 1]; }
+    if (st.has_half) { st.acc[0] += xbuf[2 * FG_ST_SAMPLES + 2 * tid]; st.aab[0] += xbuf[2 * FG_ST_SAMPLES + 2 * tid + 1]; }
   }
   __syncthreads();
-  if (tid < FG_ST_SAMPLES) { st.acc[0] += xbuf[2 * tid]; st.aab[0] += xbuf[2 * tid + 1]; }
-  __syncthreads();
-  st.has_part = 0;
+  if (st.has_two) {        // second component of self-energy elements
+    if (!owner) { xbuf[2 * (tid - FG_ST_SAMPLES)] = st.acc[1]; xbuf[2 * (tid - FG_ST_SAMPLES) + 1] = st.aab[1]; }
+    __syncthreads();
+    if (owner) { st.acc[1] += xbuf[2 * tid]; st.aab[1] += xbuf[2 * tid + 1]; }
+    __syncthreads();
+  }
+  if (!owner) { st.acc[0] = st.acc[1] = 0.0; st.aab[0] = st.aab[1] = 0.0; }
+  st.has_part = 0; st.has_half = 0; st.has_two = 0;
 }
 
 // All groups of one chunk.  V: operand table of the batch (row stride vs); owner threads flush finished destinations.
@@ -175,7 +191,7 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
   __builtin_assume(__isShared(chunk)); __builtin_assume(__isShared(V));
   const int tid = threadIdx.x, w = tid >> 5;
   const bool owner = tid < FG_ST_SAMPLES;
-  const double* Vt = V + (owner ? tid : 0);                      // the owner's column
+  const double* Vt = V + (tid & (FG_ST_SAMPLES - 1));            // the owner's column; a helper thread mirrors sample tid - 256
   { uint32_t a32 = (uint32_t)__cvta_generic_to_shared(Vt); asm volatile("" : "+r"(a32)); Vt = (const double*)__cvta_shared_to_generic(a32); __builtin_assume(__isShared(Vt)); }
   const double* Vw = V + 32 * (w & 7); const int rb0 = FG_ST_NRB * (w >> 3);
   const int ngroups = ((const FgChunkHdr*)chunk)->ngroups;
@@ -187,7 +203,7 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
     if ((int)gh.dst != st.cur) {
       fold_parts(st, xbuf);
       if (st.cur >= 0 && owner) flush(st.cur, st.acc, st.aab);
-      st.cur = gh.dst; st.acc[0] = st.acc[1] = 0.0; st.aab[0] = st.aab[1] = 0.0;
+      st.cur = gh.dst; st.acc[0] = st.acc[1] = 0.0; st.aab[0] = st.aab[1] = 0.0;      // (helpers: zeroed by fold_parts already)
     }
     const bool qx = (flags & FG_REC_QEXT) != 0;
     if (flags & FG_REC_MMA) {
@@ -206,13 +222,16 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
       p = p0 + gh.seq_bytes; g += nseq - 1; continue;
     }
     const int bytes = nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));
-    if (owner) {
+    // scalar groups: the owner threads take records [0, half), the helper threads [half, nrec) on the same operands
+    const int half = (nrec + 1) >> 1, r0 = owner ? 0 : half, r1 = owner ? half : nrec;
+    st.has_half = 1; if (flags & FG_REC_TWO) st.has_two = 1;
+    if (r0 < r1) {
       bool done = false;
       if (!(flags & (FG_REC_WIDE | FG_REC_TWO))) {
         done = true;
         switch (nf * 8 + k) {
-#define FG_CLS(NF, K) case NF * 8 + K: if (qx) run_group_static<double, 1, 1, NF, K, true>(p, nrec, Vt, vs, ne, &st.acc[0], &st.aab[0]); \
-                                        else run_group_static<double, 1, 1, NF, K, false>(p, nrec, Vt, vs, ne, &st.acc[0], &st.aab[0]); break;
+#define FG_CLS(NF, K) case NF * 8 + K: if (qx) run_group_static<double, 1, 1, NF, K, true>(p, r1, Vt, vs, ne, &st.acc[0], &st.aab[0], r0); \
+                                        else run_group_static<double, 1, 1, NF, K, false>(p, r1, Vt, vs, ne, &st.acc[0], &st.aab[0], r0); break;
           FG_CLS(0, 0) FG_CLS(0, 1) FG_CLS(0, 2) FG_CLS(0, 3) FG_CLS(0, 4)
           FG_CLS(1, 0) FG_CLS(1, 1) FG_CLS(1, 2) FG_CLS(1, 3) FG_CLS(1, 4)
           FG_CLS(2, 0) FG_CLS(2, 1) FG_CLS(2, 2) FG_CLS(2, 3) FG_CLS(2, 4)
@@ -225,8 +244,9 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
       }
       if (done) FG_MARK(st, 3);
       else {
+        const int stride = ((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double);
         RecState<double, 1> rs; rs.acc[0][0] = st.acc[0]; rs.acc[1][0] = st.acc[1]; rs.aab[0][0] = st.aab[0]; rs.aab[1][0] = st.aab[1]; rs.cur = st.cur; rs.split = 0; rs.rr = 0;
-        run_group_dyn<double, 1, 1>(p, nrec, nf, k, flags, Vt, vs, ne, rs);
+        run_group_dyn<double, 1, 1>(p + (size_t)r0 * stride, r1 - r0, nf, k, flags, Vt, vs, ne, rs);
         st.acc[0] = rs.acc[0][0]; st.acc[1] = rs.acc[1][0]; st.aab[0] = rs.aab[0][0]; st.aab[1] = rs.aab[1][0];
         FG_MARK(st, 4);
       }

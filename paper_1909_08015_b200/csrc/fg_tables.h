@@ -13,7 +13,9 @@
 #ifndef FG_CHUNK_BYTES
 #define FG_CHUNK_BYTES 32768  // numerator stream is cut into chunks of this size (records and tiles never straddle)
 #endif
+#ifndef FG_VPAD
 #define FG_VPAD 8          // padding (elements) of the row stride of the per-sample operand table V in shared memory
+#endif
 #define FG_MAXSE 4         // self-energy children of one element
 #define FG_MAXVC 5         // vertexlike children of one element
 #define FG_MAXMEM 8        // members of one forest
