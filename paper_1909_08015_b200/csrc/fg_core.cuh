@@ -317,11 +317,13 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
     }
     const double* __restrict__ cc = PRELOAD ? cr : coef;
     const int keep = (r == r0 && r0 > 0) ? 0 : h.keep;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) if (f >= keep) {
-      const T* pv = Vt + (int)h.fidx[f] * vs;
-#pragma unroll
-      for (int s = 0; s < S; ++s) pf[f][s] = (f == 0) ? pv[s] : pf[f > 0 ? f - 1 : 0][s] * pv[s];
+    // levels keep .. NF-1 of the prefix stack are rebuilt.  keep is the same in every lane (all lanes run the same record):
+    // a uniform switch with fall-through, so that every level is defined unconditionally inside its case
+    switch (keep) {
+#define FG_LVL(F) case F: if (F < NF) { const T* pv = Vt + (int)h.fidx[F < NF ? F : 0] * vs; _Pragma("unroll") for (int s = 0; s < S; ++s) pf[F < NF ? F : 0][s] = (F == 0) ? pv[s] : pf[(F > 0 && F < NF) ? F - 1 : 0][s] * pv[s]; }
+      FG_LVL(0) FG_LVL(1) FG_LVL(2) FG_LVL(3) FG_LVL(4) FG_LVL(5)
+#undef FG_LVL
+      default: break;
     }
     // free variables: reloaded only when they change (runs of records share them)
     uint32_t vkey; __builtin_memcpy(&vkey, h.vidx, 4);
