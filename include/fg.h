@@ -208,6 +208,24 @@ int fg_eval_points(const fg_plan*, const double* z, uint64_t n, int32_t mode, vo
  * I (final), y = I/g, flags as above. */
 int fg_sample_eval_dump(const fg_plan*, uint64_t first, uint64_t n, uint64_t seed, void* stream, double* I, double* y,
                         uint8_t* flags);
+/* ---- no-allocation entry point ---------------------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it).
+ * fg_eval_points_dd_noalloc: the integrand at n points in double-double (the second rung for EVERY point, no further rung), like
+ * fg_eval_points(mode 2) without its quad-double follow-up.  ALL pointers are DEVICE pointers owned by the caller:
+ * z_dev n*M doubles (points on the simplex), I_dev n doubles, err_dev n doubles or NULL (error estimate), flags_dev n bytes
+ * (bit1 = non-finite / degenerate, bit2 = not resolved by double-double at the plan's tolerance).  The call allocates nothing:
+ * the per-block scratch of the kernel lives in a static device array of 32 MiB (held by every GPU that loads the library until
+ * exit); plan tables and the plan's partial-sum buffer come from fg_plan_create.  Limits (fg_noalloc_limits): n <= 2^20, and the
+ * plan's per-block scratch must fit the array (FG_E_LIMIT otherwise).  Asynchronous on `stream`; no host synchronisation.
+ * Every call shares the array and the plan's buffers: calls (of this or of any other integration on the same plan, or of this
+ * entry point on ANY plan of the same device) that overlap on the GPU race; enqueue them on one stream or synchronise between them.
+ * fg_noalloc_setup(device) resolves the array's device address (cudaGetSymbolAddress, once per device); call it before a graph
+ * capture; fg_eval_points_dd_noalloc does it itself on its first call for a device otherwise. */
+int fg_noalloc_setup(int32_t device);
+int fg_noalloc_limits(uint64_t* scratch_bytes, uint64_t* max_points);
+int fg_eval_points_dd_noalloc(const fg_plan*, const double* z_dev, uint64_t n, void* stream, double* I_dev, double* err_dev,
+                              uint8_t* flags_dev);
+
 /* fg_dfma_peak: FP64-FMA micro-benchmark on the plan-independent device (the roofline denominator):
  * returns achieved TFLOP/s (FMA = 2) over `iters` dependent-chain steps x 8 chains per thread on all SMs. */
 int fg_dfma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms);

@@ -973,6 +973,70 @@ int fg_sample_eval_dump(const fg_plan* cp, uint64_t first, uint64_t n, uint64_t 
   return eval_common(const_cast<fg_plan*>(cp), nullptr, first, n, seed, 0, (cudaStream_t)stream, I, nullptr, y, nullptr, flags);
 }
 
+// ---- no-allocation entry point -----------------------------------------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+// the double-double evaluation of given points with the per-block scratch of fg_eval_kernel<dd> in a file-scope device
+// array instead of the plan's cudaMalloc'ed scratch.  Every GPU that loads the library holds the array until exit.
+#define FG_NOALLOC_SCRATCH_BYTES (32u << 20)        // 32 MiB
+#define FG_NOALLOC_MAX_POINTS (1u << 20)
+static __device__ __align__(256) unsigned char fg_noalloc_scratch[FG_NOALLOC_SCRATCH_BYTES];
+// In host code `fg_noalloc_scratch` is a host-side stand-in, not a device address: the address the kernel gets comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static std::mutex g_noalloc_mu;
+static void* g_noalloc_ptr[64] = {nullptr};
+
+static int noalloc_setup_locked(int device) {
+  if (device < 0 || device >= 64) return fail(FG_E_ARG, "device out of range");
+  if (g_noalloc_ptr[device]) return FG_OK;
+  CU(cudaSetDevice(device));
+  void* ptr = nullptr;
+  cudaError_t e = cudaGetSymbolAddress((void**)&ptr, fg_noalloc_scratch);
+  if (e != cudaSuccess || !ptr) return fail(FG_E_CUDA, std::string("cudaGetSymbolAddress(fg_noalloc_scratch): ") + cudaGetErrorString(e));
+  g_noalloc_ptr[device] = ptr;
+  return FG_OK;
+}
+
+int fg_noalloc_setup(int32_t device) {
+  int ndev = 0; if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(FG_E_CUDA, "no CUDA device");
+  if (device < 0 || device >= ndev) return fail(FG_E_ARG, "device out of range");
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  return noalloc_setup_locked(device);
+}
+
+int fg_noalloc_limits(uint64_t* scratch_bytes, uint64_t* max_points) {
+  if (scratch_bytes) *scratch_bytes = FG_NOALLOC_SCRATCH_BYTES;
+  if (max_points) *max_points = FG_NOALLOC_MAX_POINTS;
+  return FG_OK;
+}
+
+int fg_eval_points_dd_noalloc(const fg_plan* cp, const double* z_dev, uint64_t n, void* stream, double* I_dev, double* err_dev, uint8_t* flags_dev) {
+  fg_plan* p = const_cast<fg_plan*>(cp);
+  if (!p || !z_dev || !I_dev || !flags_dev) return fail(FG_E_ARG, "NULL argument");
+  if (n == 0) return FG_OK;
+  if (n > FG_NOALLOC_MAX_POINTS) return fail(FG_E_LIMIT, "fg_eval_points_dd_noalloc: at most 2^20 points per call");
+  const size_t per_block = (size_t)p->D.scratch_slots * (size_t)p->nt_q * S_Q * sizeof(dd);
+  if (per_block > FG_NOALLOC_SCRATCH_BYTES)
+    return fail(FG_E_LIMIT, "fg_eval_points_dd_noalloc: the per-block scratch of this plan (" + std::to_string(per_block) + " bytes) exceeds the static array (" + std::to_string((size_t)FG_NOALLOC_SCRATCH_BYTES) + " bytes)");
+  { std::lock_guard<std::mutex> lk(g_noalloc_mu); int rc = noalloc_setup_locked(p->device); if (rc != FG_OK) return rc; }
+  std::lock_guard<std::mutex> lk(p->mu);
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaSetDevice(p->device));
+  const int grid = (int)std::min<size_t>((size_t)p->grid_q, FG_NOALLOC_SCRATCH_BYTES / per_block);
+  RunArgs B; std::memset(&B, 0, sizeof(B));
+  B.n = n; B.zin = z_dev; B.outI = I_dev; B.outErr = err_dev; B.outFlags = flags_dev;
+  B.scratch = g_noalloc_ptr[p->device];
+  B.partials = p->partials + (size_t)p->grid_d * 8;           // plan-owned (allocated by fg_plan_create); the sums are not returned
+  B.do_flag = 0;                                               // last rung of this call: unresolved points get flag bit 2
+  // the array keeps the last call's contents: the kernel writes every scratch slot before it reads it, but the part this
+  // launch uses is cleared all the same, and so are the flags (the kernel ORs into them) and the partial sums it adds to
+  CU(cudaMemsetAsync(B.scratch, 0, (size_t)grid * per_block, st));
+  CU(cudaMemsetAsync(flags_dev, 0, n, st));
+  CU(cudaMemsetAsync(B.partials, 0, (size_t)p->grid_q * 8 * sizeof(double), st));
+  fg_eval_kernel<dd, S_Q, NT_Q><<<grid, p->nt_q, p->smem_q, st>>>(p->D, B);
+  CU(cudaGetLastError()); ++p->launches;
+  return FG_OK;
+}
+
 int fg_dfma_peak(int32_t device, int32_t iters, void* stream, double* tflops, double* ms_out) {
   if (!tflops || iters <= 0) return fail(FG_E_ARG, "bad argument");
   int ndev = 0; if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(FG_E_CUDA, "no CUDA device");

@@ -16,7 +16,8 @@ EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_pl
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
            "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version",
            "fg_batch_create", "fg_batch_destroy", "fg_batch_pilot", "fg_batch_set_times", "fg_batch_probabilities", "fg_batch_next",
-           "fg_batch_fold", "fg_batch_run", "fg_batch_result", "fg_batch_total"]
+           "fg_batch_fold", "fg_batch_run", "fg_batch_result", "fg_batch_total",
+           "fg_noalloc_setup", "fg_noalloc_limits", "fg_eval_points_dd_noalloc"]
 
 
 class FgError(RuntimeError):
@@ -99,6 +100,9 @@ def lib():
         L.fg_batch_run.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, vp]
         L.fg_batch_result.argtypes = [vp, C.c_int32, C.POINTER(fg_result), C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.fg_batch_total.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+        L.fg_noalloc_setup.argtypes = [C.c_int32]
+        L.fg_noalloc_limits.argtypes = [C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+        L.fg_eval_points_dd_noalloc.argtypes = [vp, vp, C.c_uint64, vp, vp, vp, vp]
         for f in ("fg_strerror", "fg_last_error_message", "fg_version"):
             getattr(L, f).restype = C.c_char_p
         L.fg_strerror.argtypes = [C.c_int]
@@ -246,6 +250,11 @@ class Plan:
         _check(lib().fg_eval_points(self.h, _p(z), n, int(mode), _stream(stream), _p(I), _p(Id), _p(err), _p(fl)))
         return dict(I=I, I_double=Id, err=err, flags=fl)
 
+    def eval_points_dd_noalloc(self, z_dev_ptr, n, I_dev_ptr, err_dev_ptr, flags_dev_ptr, stream=None):
+        """fg_eval_points_dd_noalloc: every argument is a DEVICE address (int) owned by the caller; allocates nothing."""
+        _check(lib().fg_eval_points_dd_noalloc(self.h, C.c_void_p(int(z_dev_ptr)), int(n), _stream(stream), C.c_void_p(int(I_dev_ptr)),
+                                               C.c_void_p(int(err_dev_ptr)) if err_dev_ptr else None, C.c_void_p(int(flags_dev_ptr))))
+
     def sample_eval_dump(self, first, n, seed, stream=None):
         I = np.zeros(n); y = np.zeros(n); fl = np.zeros(n, dtype=np.uint8)
         _check(lib().fg_sample_eval_dump(self.h, int(first), int(n), int(seed), _stream(stream), _p(I), _p(y), _p(fl)))
@@ -294,6 +303,16 @@ def result_merge(a, b):
     """fg_result_merge on two raw fg_result structs."""
     out = fg_result(); _check(lib().fg_result_merge(C.byref(a), C.byref(b), C.byref(out)))
     return out
+
+
+def noalloc_setup(device=0):
+    _check(lib().fg_noalloc_setup(int(device)))
+
+
+def noalloc_limits():
+    a = C.c_uint64(); b = C.c_uint64()
+    _check(lib().fg_noalloc_limits(C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
 
 
 def dfma_peak(device=0, iters=200000, stream=None):
