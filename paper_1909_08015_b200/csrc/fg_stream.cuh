@@ -8,7 +8,8 @@
 // Work split: warp w serves the 32 samples of sample group sg = w % 8 and the row blocks (8 samples each)
 // rb0 .. rb0 + FG_ST_NRB - 1 with rb0 = FG_ST_NRB * (w / 8); two warps share a sample group, so sixteen warps (four per
 // scheduler) stream the same tiles in step.  For one row block the monomials of a group are built ONCE (A fragments stay in
-// registers for all tiles of the group); per tile the lane loads its B fragment (one conflict-free LDS.32 per k-step: the
+// registers for all tiles of the group; the two row blocks of a warp are interleaved column by column so that one 16-byte
+// load serves both); per tile the lane loads its B fragment (one conflict-free LDS.32 per k-step: the
 // high word of the double), runs the k-steps, and weights its two record values with their products of beta's.
 #pragma once
 #include "fg_core.cuh"
@@ -40,7 +41,10 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
   constexpr int ROWB = FG_ST_VS * 8;                 // bytes of one row of V
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int vq = ne * ROWB;
-  const unsigned char* __restrict__ Vb = (const unsigned char*)(Vw + 8 * rb0 + r);     // sample of row block rb0; + 64 bytes per further row block
+  static_assert(FG_ST_NRB == 2, "the two row blocks of a warp are interleaved column by column");
+  // columns: row r of row block rb0 + bi is column 8 * rb0 + 2 * r + bi of the warp's sample group, so that one 16-byte load
+  // serves both row blocks (the DMMA does not care which sample sits in which row; fold_parts uses the same map)
+  const unsigned char* __restrict__ Vb = (const unsigned char*)(Vw + 8 * rb0 + 2 * r);
   // the lane's base address goes through an opaque asm: ptxas otherwise rebuilds it from %tid (S2R + four integer
   // instructions) in front of every load of the record epilogue to save one register (+11-17 % samples/s, A/B in profiles/)
   { uint32_t vb32 = (uint32_t)__cvta_generic_to_shared(Vb); asm volatile("" : "+r"(vb32)); Vb = (const unsigned char*)__cvta_shared_to_generic(vb32); __builtin_assume(__isShared(Vb)); }
@@ -53,29 +57,34 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
     const int v0 = (int)((gw.y >> 16) & 255u) * ROWB, v1 = (int)(gw.y >> 24) * ROWB, v2 = (int)(gw.z & 255u) * ROWB, v3 = (int)((gw.z >> 8) & 255u) * ROWB;
     // the lane's column of the A fragments of every k-step (monomial order: fg_tables.h, mma_monomials), built once per group
     double mono[NRB][STEPS];
+    {
+      const double2 A0 = *(const double2*)(Vb + v0), A1 = *(const double2*)(Vb + v1);
+      double2 A2 = make_double2(1.0, 1.0), A3 = make_double2(1.0, 1.0), Q0, Q1, Q2, Q3;
+      if (K > 2) A2 = *(const double2*)(Vb + v2);
+      if (K > 3) A3 = *(const double2*)(Vb + v3);
+      if (QX) { Q0 = *(const double2*)(Vb + v0 + vq); Q1 = *(const double2*)(Vb + v1 + vq); if (K > 2) Q2 = *(const double2*)(Vb + v2 + vq); if (K > 3) Q3 = *(const double2*)(Vb + v3 + vq); }
 #pragma unroll
-    for (int bi = 0; bi < NRB; ++bi) {
-      const unsigned char* Vs = Vb + 64 * bi;
-      const double a0 = *(const double*)(Vs + v0), a1 = *(const double*)(Vs + v1);
-      const double a2 = K > 2 ? *(const double*)(Vs + v2) : 1.0, a3 = K > 3 ? *(const double*)(Vs + v3) : 1.0;
-      const double a01 = a0 * a1;
-      const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
-      double hi[NM]; hi[0] = 1.0;
-      if (K > 2) hi[1] = a2;
-      if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
-      mono[bi][0] = mlo;
+      for (int bi = 0; bi < NRB; ++bi) {
+        const double a0 = bi ? A0.y : A0.x, a1 = bi ? A1.y : A1.x, a2 = bi ? A2.y : A2.x, a3 = bi ? A3.y : A3.x;
+        const double a01 = a0 * a1;
+        const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
+        double hi[NM]; hi[0] = 1.0;
+        if (K > 2) hi[1] = a2;
+        if (K > 3) { hi[2] = a3; hi[3] = a2 * a3; }
+        mono[bi][0] = mlo;
 #pragma unroll
-      for (int tt = 1; tt < NM; ++tt) mono[bi][tt] = mlo * hi[tt];
-      if (QX) {
-        const double q0 = *(const double*)(Vs + v0 + vq), q1 = *(const double*)(Vs + v1 + vq);
-        const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
-        mono[bi][NM] = mq;
+        for (int tt = 1; tt < NM; ++tt) mono[bi][tt] = mlo * hi[tt];
+        if (QX) {
+          const double q0 = bi ? Q0.y : Q0.x, q1 = bi ? Q1.y : Q1.x;
+          const double mq = ((c & 2) ? q1 : q0) * ((c & 1) ? ((c & 2) ? a0 : a1) : 1.0);
+          mono[bi][NM] = mq;
 #pragma unroll
-        for (int tt = 1; tt < NM; ++tt) mono[bi][NM + tt] = mq * hi[tt];
-        if (K == 3) mono[bi][2 * NM] = mlo * *(const double*)(Vs + v2 + vq);
-        if (K == 4) {
-          const double m2 = mlo * *(const double*)(Vs + v2 + vq), m3 = mlo * *(const double*)(Vs + v3 + vq);
-          mono[bi][2 * NM] = m2; mono[bi][2 * NM + 1] = m2 * a3; mono[bi][2 * NM + 2] = m3; mono[bi][2 * NM + 3] = m3 * a2;
+          for (int tt = 1; tt < NM; ++tt) mono[bi][NM + tt] = mq * hi[tt];
+          if (K == 3) mono[bi][2 * NM] = mlo * (bi ? Q2.y : Q2.x);
+          if (K == 4) {
+            const double m2 = mlo * (bi ? Q2.y : Q2.x), m3 = mlo * (bi ? Q3.y : Q3.x);
+            mono[bi][2 * NM] = m2; mono[bi][2 * NM + 1] = m2 * a3; mono[bi][2 * NM + 2] = m3; mono[bi][2 * NM + 3] = m3 * a2;
+          }
         }
       }
     }
@@ -119,11 +128,9 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
 #pragma unroll
           for (int i = 0; i < NF; ++i) if (i >= keep) {
             const int off = (int)__byte_perm(i < 4 ? w0 : w1, 0u, 0x4440 + (i & 3)) * ROWB;
-#pragma unroll
-            for (int bi = 0; bi < NRB; ++bi) {
-              const double v = *(const double*)(Vb + 64 * bi + off);
-              pf[bi][i] = (i == 0) ? v : pf[bi][i > 0 ? i - 1 : 0] * v;
-            }
+            const double2 v = *(const double2*)(Vb + off);
+            pf[0][i] = (i == 0) ? v.x : pf[0][i > 0 ? i - 1 : 0] * v.x;
+            pf[1][i] = (i == 0) ? v.y : pf[1][i > 0 ? i - 1 : 0] * v.y;
           }
         }
 #pragma unroll
@@ -164,7 +171,7 @@ __device__ __forceinline__ void fold_parts(StreamState& st, double* __restrict__
       double v = st.part[bi], a = st.part[FG_ST_NRB + bi];
       v += __shfl_xor_sync(0xffffffffu, v, 1); a += __shfl_xor_sync(0xffffffffu, a, 1);
       v += __shfl_xor_sync(0xffffffffu, v, 2); a += __shfl_xor_sync(0xffffffffu, a, 2);
-      if ((lane & 3) == 0) { const int smp = 32 * sg + 8 * (rb0 + bi) + (lane >> 2); xbuf[2 * smp] = v; xbuf[2 * smp + 1] = a; }
+      if ((lane & 3) == 0) { const int smp = 32 * sg + 8 * rb0 + 2 * (lane >> 2) + bi; xbuf[2 * smp] = v; xbuf[2 * smp + 1] = a; }      // column map of run_group_mma_rb
       st.part[bi] = 0.0; st.part[FG_ST_NRB + bi] = 0.0;
     }
   }

@@ -14,7 +14,8 @@
 #define FG_CHUNK_BYTES 32768  // numerator stream is cut into chunks of this size (records and tiles never straddle)
 #endif
 #ifndef FG_VPAD
-#define FG_VPAD 8          // padding (elements) of the row stride of the per-sample operand table V in shared memory
+#define FG_VPAD 4          // padding (elements) of the row stride of the operand table V in shared memory: rows i and j fall
+                           // into the same banks only if i = j mod 4 (32-byte shift per row)
 #endif
 #define FG_MAXSE 4         // self-energy children of one element
 #define FG_MAXVC 5         // vertexlike children of one element
