@@ -35,6 +35,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--graphs", type=int, default=32, help="how many graphs of the 32-graph config-5 batch to time")
+    ap.add_argument("--graph-list", default="", help="comma-separated indices into the 32-graph batch (overrides --graphs), e.g. 0,17 for a profiler capture")
     ap.add_argument("--samples", type=int, default=1 << 22, help="samples per graph per step and per GPU")
     ap.add_argument("--pilot-samples", type=int, default=1 << 16, help="samples of the pilot stage that sets the acceptance tolerance")
     ap.add_argument("--impl", default="fg", choices=["fg", "reference"])
@@ -77,9 +78,11 @@ class ClockSampler:
                 "samples": len(self.rows)}
 
 
-def cfg5_graphs(n_graphs):
+def cfg5_graphs(n_graphs, graph_list=""):
     from paper_1909_08015_b200 import inputs
     cfg = inputs.config(5)
+    if graph_list:
+        return [cfg["graphs"][int(i)] for i in graph_list.split(",")], cfg
     return cfg["graphs"][:n_graphs], cfg
 
 
@@ -139,7 +142,7 @@ def main_fg(args):
         build.build()
     if world > 1:
         dist.barrier()
-    graphs, cfg = cfg5_graphs(args.graphs)
+    graphs, cfg = cfg5_graphs(args.graphs, args.graph_list)
     S = args.samples                 # samples per graph per step PER GPU (weak scaling): a step integrates world * S per graph
     stream = torch.cuda.current_stream()
     # plans; acceptance tolerance (18) for the run length the config names: abs_tol = sigma_down(target)/4 from a pilot stage
@@ -222,7 +225,7 @@ def main_fg(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": "config5: %s of the 32 seeded random 5-loop vertex graphs (14 lines, M=14 after merge), %d samples per graph per step per GPU, graphs one after another, fresh Philox sample ids every step; value = whole-job samples/s per graph (all graphs' samples / device time)" % ("all 32" if len(plans) == 32 else "the first %d" % len(plans), S),
+            "config": {"workload": "config5: %s of the 32 seeded random 5-loop vertex graphs (14 lines, M=14 after merge), %d samples per graph per step per GPU, graphs one after another, fresh Philox sample ids every step; value = whole-job samples/s per graph (all graphs' samples / device time)" % ("all 32" if len(plans) == 32 else ("graphs %s" % args.graph_list if args.graph_list else "the first %d" % len(plans)), S),
                        "l2": "inputs are generated on chip; the 2-9 MB coefficient stream per graph is L2-resident by design (re-read by every block), no flush applies",
                        "tolerance": "rel_tol %.1e, abs_tol = sigma_down(%.0e samples)/4 from a %d-sample pilot stage per graph (PAPER.md:286, (18))" % (args.rel_tol, args.target_samples, args.pilot_samples),
                        "graphs": info, "flagged_fraction": flagged / max(1.0, float(world) * len(plans) * S * e2e_steps), "flagged2": flagged2, "rejected": rejected,
