@@ -287,8 +287,13 @@ template <int N> struct PreLoad<N, N> { static __device__ __forceinline__ void r
 #else
 #define FG_NOINLINE inline
 #endif
+#if defined(__CUDACC__)
+#define FG_FORCEINLINE __device__ __forceinline__
+#else
+#define FG_FORCEINLINE inline
+#endif
 template <class T, int S, int ABS, int NF, int K, bool QX>
-FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* __restrict__ accp, double* __restrict__ aabp, int r0 = 0) {   // records r0 .. nrec-1 (r0 > 0: a second thread set takes the rest; its first record rebuilds the whole prefix)
+FG_FORCEINLINE void run_group_static_body(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* __restrict__ accp, double* __restrict__ aabp, int r0 = 0) {   // records r0 .. nrec-1 (r0 > 0: a second thread set takes the rest; its first record rebuilds the whole prefix)
 #if defined(__CUDA_ARCH__)
   __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vt));
 #endif
@@ -356,6 +361,11 @@ FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec,
   }
 #pragma unroll
   for (int s = 0; s < S; ++s) { accp[s] = acc[s]; aabp[s] = aab[s]; }
+}
+
+template <class T, int S, int ABS, int NF, int K, bool QX>
+FG_NOINLINE void run_group_static(const unsigned char* __restrict__ p, int nrec, const T* __restrict__ Vt, int vs, int ne, T* __restrict__ accp, double* __restrict__ aabp, int r0 = 0) {
+  run_group_static_body<T, S, ABS, NF, K, QX>(p, nrec, Vt, vs, ne, accp, aabp, r0);
 }
 
 FG_HD int fg_lane() {
@@ -457,12 +467,26 @@ FG_HD void run_group_dyn(const unsigned char* __restrict__ p, int nrec, int nf, 
 }
 
 // ---- tensor-core groups (FG_REC_MMA): monomial order shared by the planner, the scalar interpreter and the DMMA path ----
-FG_HD constexpr int mma_steps(int k, bool qx) { return (1 << (k - 2)) + (qx ? (1 << (k - 2)) + (k - 2) * ((1 << k) >> 3) : 0); }
+FG_HD constexpr int mma_steps(int k, bool qx) { return k < 2 ? 1 : (1 << (k - 2)) + (qx ? (1 << (k - 2)) + (k - 2) * ((1 << k) >> 3) : 0); }
 
 // all monomials of one point: mono[4*step + x] (see FgRecM in fg_tables.h)
 template <class T>
-FG_HD void mma_monomials(int k, bool qx, const T* a, const T* aq, T* mono) {
+FG_HD void mma_monomials(int k, bool qx, bool par4, const T* a, const T* aq, T* mono) {      // par4: group flagged FG_REC_PAR_A / FG_REC_PAR_B
+  if (k < 2) { mono[0] = T(1.0); mono[1] = k ? a[0] : T(0.0); mono[2] = (k && qx) ? aq[0] : T(0.0); mono[3] = T(0.0); return; }
   const int nm = 1 << (k - 2);
+  if (k == 4 && par4) {      // parity-homogeneous steps (fg_tables.h): subsets of the four variables, of the other three
+    for (int st = 0; st < 4; ++st) for (int x = 0; x < 4; ++x) {
+      const int sub = FG_MMA4_MAIN_SUBSET(st, x); T m = T(1.0);
+      for (int i = 0; i < 4; ++i) if ((sub >> i) & 1) m = m * a[i];
+      mono[4 * st + x] = m;
+    }
+    if (qx) for (int j = 0; j < 4; ++j) for (int par = 0; par < 2; ++par) for (int x = 0; x < 4; ++x) {
+      const int sub = FG_MMA4_Q_SUBSET(par, x); T m = aq[j]; int bit = 0;
+      for (int i = 0; i < 4; ++i) if (i != j) { if ((sub >> bit) & 1) m = m * a[i]; ++bit; }
+      mono[4 * (4 + 2 * j + par) + x] = m;
+    }
+    return;
+  }
   T mlo[4] = {T(1.0), a[0], a[1], a[0] * a[1]};
   for (int t = 0; t < nm; ++t) {
     T h = T(1.0); for (int i = 0; i + 2 < k; ++i) if ((t >> i) & 1) h = h * a[2 + i];
@@ -491,7 +515,7 @@ FG_HD void run_group_mma_dyn(const unsigned char* __restrict__ p, int ntiles, in
   for (int s = 0; s < S; ++s) {
     T a[FG_KMAX], aq[FG_KMAX];
     for (int j = 0; j < k; ++j) { a[j] = Vt[(int)vidx[j] * vs + s]; aq[j] = qx ? Vt[((int)vidx[j] + ne) * vs + s] : T(0.0); }
-    mma_monomials<T>(k, qx, a, aq, mono[s]);
+    mma_monomials<T>(k, qx, (flags & (FG_REC_PAR_A | FG_REC_PAR_B)) != 0, a, aq, mono[s]);
     if (ABS == 2) for (int J = 0; J < 4 * steps; ++J) monoa[s][J] = t_abs_d(mono[s][J]);
   }
   const int tile_bytes = FG_TILE_BYTES(steps);
@@ -555,7 +579,7 @@ FG_HD void run_chunk(const unsigned char* __restrict__ chunk, const T* __restric
     if (flags & FG_REC_MMA) {
       if (!done) run_group_mma_dyn<T, S, ABS>(p, nrec, nf, k, flags, gh.vidx, Vt, vs, ne, st);
       FG_MARK(st, 4);
-      p += nrec * FG_TILE_BYTES(mma_steps(k, (flags & FG_REC_QEXT) != 0));
+      p += (size_t)gh.grp_units * 16;
       continue;
     }
     if (!done) { run_group_dyn<T, S, ABS>(p, nrec, nf, k, flags, Vt, vs, ne, st); FG_MARK(st, 4); } else FG_MARK(st, 3);

@@ -60,7 +60,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t phase[2];
+struct ChunkRing { unsigned char* buf; uint64_t* bar; uint32_t* cnt; uint32_t phase[2];      // cnt: warps that have left each buffer (stream kernel)
 #ifdef FG_PHASE_PROF
   long long* prof; long long tlast;
 #endif
@@ -364,13 +364,16 @@ __device__ void run_program_s(const FgPlanDev& P, const FgNumDev& N, const Scrat
   if (nch == 0) return;
   const unsigned char* g0 = P.chunks + (size_t)N.chunk_begin * FG_CHUNK_BYTES;
   const uint32_t* used = P.chunk_used + N.chunk_begin;
+#if FG_DECOUPLE
+  __syncthreads();      // every warp has left the ring buffers of the previous program
+#endif
   if (tid == 0) {
     mbar_expect_tx(&ring.bar[0], used[0]); bulk_g2s(ring.buf, g0, used[0], &ring.bar[0]);
     if (nch > 1) { mbar_expect_tx(&ring.bar[1], used[1]); bulk_g2s(ring.buf + FG_CHUNK_BYTES, g0 + FG_CHUNK_BYTES, used[1], &ring.bar[1]); }
   }
   StreamState st; st.cur = -1; st.has_part = 0; st.has_half = 0; st.has_two = 0; st.acc[0] = st.acc[1] = st.aab[0] = st.aab[1] = 0.0;
 #pragma unroll
-  for (int i = 0; i < 2 * FG_ST_NRB; ++i) st.part[i] = 0.0;
+  for (int i = 0; i < 2 * FG_ST_NRB; ++i) st.part.v[i] = 0.0;
 #ifdef FG_PHASE_PROF
   st.prof = ring.prof; st.tlast = ring.tlast;
 #endif
@@ -384,9 +387,24 @@ __device__ void run_program_s(const FgPlanDev& P, const FgNumDev& N, const Scrat
     FG_MARK(st, 5);
     run_chunk_s(ring.buf + b * FG_CHUNK_BYTES, V, FG_ST_VS, ne, st, xbuf, flush);
     FG_MARK(st, 8);
+#if FG_DECOUPLE
+    // buffer b is released warp by warp: the last of the 16 warps to leave it starts the copy of chunk ch + 2 (the counter
+    // only grows; 16 divides 2^32).  No warp waits here; a fast pair runs at most one chunk ahead of the slowest.
+    __syncwarp();
+    if ((tid & 31) == 0) {
+      const uint32_t old = atomicAdd(&ring.cnt[b], 1u);
+      if ((old + 1u) % (FG_ST_THREADS / 32) == 0u && ch + 2 < nch) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const uint32_t ub = used[ch + 2];
+        mbar_expect_tx(&ring.bar[b], ub); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, ub, &ring.bar[b]);
+      }
+    }
+    FG_MARK(st, 5);
+#else
     __syncthreads();   // every thread is done with buffer b
     FG_MARK(st, 5);
     if (tid == 0 && ch + 2 < nch) { mbar_expect_tx(&ring.bar[b], used[ch + 2]); bulk_g2s(ring.buf + b * FG_CHUNK_BYTES, g0 + (size_t)(ch + 2) * FG_CHUNK_BYTES, used[ch + 2], &ring.bar[b]); }
+#endif
   }
   fold_parts(st, xbuf);
   if (st.cur >= 0 && owner) flush(st.cur, st.acc, st.aab);
@@ -403,6 +421,8 @@ __global__ void __launch_bounds__(FG_ST_THREADS, 1) fg_stream_kernel(const FgPla
   long long prof[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}; ring.prof = prof; ring.tlast = clock64();
 #endif
   uint64_t* barV = ring.bar + 2; uint32_t phaseV = 0u;
+  ring.cnt = (uint32_t*)(smem + 2 * FG_CHUNK_BYTES + 64);
+  if (threadIdx.x == 0) { ring.cnt[0] = 0u; ring.cnt[1] = 0u; }
   double* xbuf = (double*)(smem + 2 * FG_CHUNK_BYTES + 128);
   double* V = (double*)(smem + 2 * FG_CHUNK_BYTES + 128 + FG_ST_XBUF_BYTES);
   const int tid = threadIdx.x, ss = FG_ST_SAMPLES; const bool owner = tid < FG_ST_SAMPLES;
@@ -450,7 +470,7 @@ __global__ void __launch_bounds__(FG_ST_THREADS, 1) fg_stream_kernel(const FgPla
 #ifdef FG_PHASE_PROF
   if (A.phase_cycles && (tid & 31) == 0) for (int k = 0; k < 16; ++k) atomicAdd(&A.phase_cycles[k], (unsigned long long)prof[k]);
 #endif
-  block_reduce_tail(ta, (double*)smem /* the ring is idle now */, A.partials + (size_t)blockIdx.x * 8, 4);
+  block_reduce_tail(ta, (double*)smem /* the ring is idle after the block barrier in there */, A.partials + (size_t)blockIdx.x * 8, 4);
 }
 
 // Queue of the next rung: the set bits of `bits` as a list of ordinals in ascending order (one block; deterministic, so

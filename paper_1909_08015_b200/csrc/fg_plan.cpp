@@ -616,7 +616,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
     // pack records into chunks of class-uniform groups; keep = leading product factors shared with the previous record.
     // Runs of records with the same class and the same free variables become tensor-core (DMMA) tile groups.
     size_t cur = 0, base = 0, ghdr = 0; bool open = false, gopen = false; int ngroups = 0, gn = 0; const HRecord* prev = nullptr;
-    auto mma_steps = [](int k, bool qx) { int nm = 1 << (k - 2); return nm + (qx ? nm + (k - 2) * ((1 << k) >> 3) : 0); };
+    auto mma_steps = [](int k, bool qx) { if (k < 2) return 1; int nm = 1 << (k - 2); return nm + (qx ? nm + (k - 2) * ((1 << k) >> 3) : 0); };
     auto rec_ncoef_host = [](int k, int flags) { int n = (flags & FG_REC_QEXT) ? (1 << k) + k * ((1 << k) >> 1) : ((flags & FG_REC_TWO) ? 2 : 1) << k; return (n + 1) & ~1; };
     auto cls = [](const HRecord& r) { int fl = r.flags & (FG_REC_TWO | FG_REC_QEXT); if (r.nf > FG_NFC) fl |= FG_REC_WIDE; return (r.dst << 16) | (r.nf << 12) | (r.k << 8) | fl; };
     auto close_group = [&]() { if (gopen) { FgGroupHdr g; std::memcpy(&g, &P.d_chunks[ghdr], sizeof(g)); g.nrec = (uint16_t)gn; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); gopen = false; } };
@@ -632,6 +632,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
         const bool qx = (g.flags & FG_REC_QEXT) != 0;
         size_t body = (g.flags & FG_REC_MMA) ? (size_t)g.nrec * (size_t)FG_TILE_BYTES(mma_steps(g.k, qx))
                                              : (size_t)g.nrec * (((g.flags & FG_REC_WIDE) ? sizeof(FgRecW) : sizeof(FgRecC)) + (size_t)rec_ncoef_host(g.k, g.flags) * sizeof(double));
+        if (g.flags & FG_REC_MMA) { g.grp_units = (uint16_t)(body / 16); std::memcpy(&P.d_chunks[o], &g, sizeof(g)); }
         offs.push_back(o); sizes.push_back(sizeof(FgGroupHdr) + body); o += sizeof(FgGroupHdr) + body;
       }
       for (int gi = 0; gi < ngroups; ++gi) {
@@ -639,7 +640,7 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
         if (!(g.flags & FG_REC_MMA)) continue;
         int n = 1; size_t bytes = sizes[gi];
         for (int gj = gi + 1; gj < ngroups; ++gj) { FgGroupHdr g2; std::memcpy(&g2, &P.d_chunks[offs[gj]], sizeof(g2)); if (g2.nf != g.nf || g2.k != g.k || g2.flags != g.flags || g2.dst != g.dst) break; ++n; bytes += sizes[gj]; }
-        g.nseq = (uint16_t)n; g.seq_bytes = (uint32_t)bytes; std::memcpy(&P.d_chunks[offs[gi]], &g, sizeof(g));
+        g.nseq = (uint16_t)n; g.seq_units = (uint16_t)(bytes / 16); std::memcpy(&P.d_chunks[offs[gi]], &g, sizeof(g));
       }
     };
     auto new_chunk = [&]() { close_chunk(); base = P.d_chunks.size(); P.d_chunks.resize(base + FG_CHUNK_BYTES, 0); cur = sizeof(FgChunkHdr); ngroups = 0; open = true; };
@@ -650,8 +651,14 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
       std::memcpy(g.vidx, r.vidx, sizeof(g.vidx));
       ghdr = base + cur; std::memcpy(&P.d_chunks[ghdr], &g, sizeof(g)); cur += sizeof(g); gopen = true; gn = 0; ++ngroups; prev = nullptr;
     };
-    auto mma_coef = [](const HRecord& r, int step, int x) -> double {
-      const int k = r.k, nm = 1 << (k - 2); const double* mainT = r.coef.data(); const double* qT = mainT + (1 << k); const int qs = (1 << k) >> 1;
+    auto mma_coef = [](const HRecord& r, int step, int x, bool par4 = false) -> double {      // par4: the parity-homogeneous step order of flagged k = 4 groups
+      const int k = r.k; const double* mainT = r.coef.data(); const double* qT = mainT + (1 << k); const int qs = (1 << k) >> 1;
+      if (k < 2) return x == 0 ? mainT[0] : (x == 1 && k == 1) ? mainT[1] : (x == 2 && k == 1 && (r.flags & FG_REC_QEXT)) ? qT[0] : 0.0;      // {1, a0, aq0, 0}
+      if (k == 4 && par4) {      // parity-homogeneous steps (fg_tables.h)
+        if (step < 4) return mainT[FG_MMA4_MAIN_SUBSET(step, x)];
+        const int j = (step - 4) >> 1, par = (step - 4) & 1; return qT[j * qs + FG_MMA4_Q_SUBSET(par, x)];
+      }
+      const int nm = 1 << (k - 2);
       if (step < nm) return mainT[x | (step << 2)];
       if (step < 2 * nm) { int t = step - nm, j = x >> 1; return qT[j * qs + ((x & 1) | (t << 1))]; }
       int s2 = step - 2 * nm, nh = (1 << k) >> 3, j = 2 + s2 / nh, t2 = s2 % nh; return qT[j * qs + (x | (t2 << 2))];
@@ -671,10 +678,19 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
         const int R = (int)(j - i), ntiles = (R + 7) / 8;
         // record shown to lane c (of every quad) in tile t, slot e: depth-first index c*2*ntiles + 2t + e
         auto rec_at = [&](int t, int n) -> const HRecord* { int d = (n >> 1) * 2 * ntiles + 2 * t + (n & 1); return d < R ? &N.recs[i + d] : nullptr; };
+        // k = 4: steps in which a record of the run has a non-zero coefficient; inside set A or set B the group is flagged
+        // and the kernel leaves the other steps out
+        int par_flag = 0, steps_run = steps;
+        if (r0.k == 4 && FG_MMA_PARITY) {
+          uint32_t gm = 0;
+          for (size_t t = i; t < j; ++t) for (int st = 0; st < steps; ++st) for (int x = 0; x < 4; ++x) if (mma_coef(N.recs[t], st, x, true) != 0.0) gm |= 1u << st;
+          if ((gm & ~FG_MMA_PAR_MASK_A(qx)) == 0) { par_flag = FG_REC_PAR_A; steps_run = __builtin_popcount(FG_MMA_PAR_MASK_A(qx)); }
+          else if ((gm & ~FG_MMA_PAR_MASK_B(qx)) == 0) { par_flag = FG_REC_PAR_B; steps_run = __builtin_popcount(FG_MMA_PAR_MASK_B(qx)); }
+        }
         for (int t = 0; t < ntiles; ++t) {
           bool need_group = !gopen || prev != nullptr;      // prev != nullptr: a regular group is open
           if (!open || cur + tile_bytes + (need_group ? sizeof(FgGroupHdr) : 0) > FG_CHUNK_BYTES) { new_chunk(); need_group = true; }
-          if (need_group) open_group(r0, FG_REC_MMA);
+          if (need_group) open_group(r0, FG_REC_MMA | par_flag);
           for (int n = 0; n < 8; ++n) {
             FgRecM h; std::memset(&h, 0, sizeof(h)); h.keep = (uint8_t)r0.nf;
             if (const HRecord* r = rec_at(t, n)) {
@@ -688,10 +704,10 @@ int build_plan(const Graph& g, const PlanOpts& opts, HostPlan& P, std::string& m
           }
           FgMmaCoef* fr = (FgMmaCoef*)&P.d_chunks[base + cur + 8 * sizeof(FgRecM)];
           for (int st = 0; st < steps; ++st) for (int n = 0; n < 8; ++n) for (int x = 0; x < 4; ++x) {
-            const HRecord* r = rec_at(t, n); FgMmaCoef h = 0; if (r) fg_mma_coef_pack(mma_coef(*r, st, x), &h); fr[st * 32 + n * 4 + x] = h;
+            const HRecord* r = rec_at(t, n); FgMmaCoef h = 0; if (r) fg_mma_coef_pack(mma_coef(*r, st, x, par_flag != 0), &h); fr[st * 32 + n * 4 + x] = h;
           }
           cur += tile_bytes; ++gn;
-          N.exec_flops += 8.0 * (8.0 * steps + 4.0);
+          N.exec_flops += 8.0 * (8.0 * steps_run + 4.0);
         }
         { auto& h = hist[{1, r0.nf, r0.k, qx ? 1 : 0, 0}]; h[0] += R; h[1] += ntiles; h[2] += 1; }
         if (std::getenv("FG_PLAN_HIST")) {      // sparsity by k-step: per record the mask of steps with a non-zero coefficient

@@ -34,10 +34,23 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 // The FG_ST_NRB row blocks of the warp go through a tile together: one B fragment and one decoded record header serve
 // them all (shared-memory wavefronts, not the FP64 pipe, are what this loop has to economise: ncu, profiles/).
 // part[bi] += value partial, part[FG_ST_NRB + bi] += |.| partial of row block rb0 + bi (reduced over the quad by fold_parts).
+// partial sums travel by value (registers): a pointer into the caller's state would pin that state to local memory
+struct MmaPart { double v[2 * FG_ST_NRB]; };
+struct AccPair { double acc, aab; };
 template <int NF, int K, bool QX>
-__device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int ne, int rb0, double* __restrict__ part) {
+__device__ __noinline__ AccPair run_group_static_v(const unsigned char* __restrict__ p, int nrec, const double* __restrict__ Vt, int vs, int ne, AccPair in, int r0) {
+  double a = in.acc, b = in.aab;
+  run_group_static_body<double, 1, 1, NF, K, QX>(p, nrec, Vt, vs, ne, &a, &b, r0);
+  AccPair out; out.acc = a; out.aab = b; return out;
+}
+
+// VAR (k = 4 only): 0 every step, 1 / 2 the steps of set A / B of a group flagged FG_REC_PAR_A / FG_REC_PAR_B
+template <int NF, int K, bool QX, int VAR = 0>
+__device__ __noinline__ MmaPart run_group_mma_rb(const unsigned char* __restrict__ p, int nseq, const double* __restrict__ Vw, int ne, int rb0, MmaPart part) {
   __builtin_assume(__isShared(p)); __builtin_assume(__isShared(Vw));
-  constexpr int NM = 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS), NRB = FG_ST_NRB;
+  constexpr int NM = K < 2 ? 1 : 1 << (K - 2), STEPS = mma_steps(K, QX), TILE = FG_TILE_BYTES(STEPS), NRB = FG_ST_NRB;
+  constexpr bool PAR4 = K == 4 && VAR != 0;           // flagged groups: parity-homogeneous step order (fg_tables.h)
+  constexpr unsigned SMASK = VAR == 1 ? FG_MMA_PAR_MASK_A(QX) : VAR == 2 ? FG_MMA_PAR_MASK_B(QX) : (1u << STEPS) - 1u;   // steps that are run
   constexpr int ROWB = FG_ST_VS * 8;                 // bytes of one row of V
   const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3;
   const int vq = ne * ROWB;
@@ -50,14 +63,19 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
   { uint32_t vb32 = (uint32_t)__cvta_generic_to_shared(Vb); asm volatile("" : "+r"(vb32)); Vb = (const unsigned char*)__cvta_shared_to_generic(vb32); __builtin_assume(__isShared(Vb)); }
   double av[NRB], ab[NRB];
 #pragma unroll
-  for (int bi = 0; bi < NRB; ++bi) { av[bi] = part[bi]; ab[bi] = part[NRB + bi]; }
+  for (int bi = 0; bi < NRB; ++bi) { av[bi] = part.v[bi]; ab[bi] = part.v[NRB + bi]; }
   for (int g = 0; g < nseq; ++g) {       // consecutive groups of this class (same destination), each with its own free variables
     const uint4 gw = *(const uint4*)p; p += sizeof(FgGroupHdr);
     const int ntiles = (int)(gw.x & 0xffffu);
     const int v0 = (int)((gw.y >> 16) & 255u) * ROWB, v1 = (int)(gw.y >> 24) * ROWB, v2 = (int)(gw.z & 255u) * ROWB, v3 = (int)((gw.z >> 8) & 255u) * ROWB;
     // the lane's column of the A fragments of every k-step (monomial order: fg_tables.h, mma_monomials), built once per group
     double mono[NRB][STEPS];
-    {
+    if constexpr (K < 2) {       // one step {1, a0, aq0, 0}[c]
+      double2 A0 = make_double2(0.0, 0.0), Q0 = make_double2(0.0, 0.0);
+      if (K == 1) { A0 = *(const double2*)(Vb + v0); if (QX) Q0 = *(const double2*)(Vb + v0 + vq); }
+      mono[0][0] = (c == 0) ? 1.0 : (c == 1) ? A0.x : (c == 2) ? Q0.x : 0.0;
+      mono[1][0] = (c == 0) ? 1.0 : (c == 1) ? A0.y : (c == 2) ? Q0.y : 0.0;
+    } else {
       const double2 A0 = *(const double2*)(Vb + v0), A1 = *(const double2*)(Vb + v1);
       double2 A2 = make_double2(1.0, 1.0), A3 = make_double2(1.0, 1.0), Q0, Q1, Q2, Q3;
       if (K > 2) A2 = *(const double2*)(Vb + v2);
@@ -66,6 +84,26 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
 #pragma unroll
       for (int bi = 0; bi < NRB; ++bi) {
         const double a0 = bi ? A0.y : A0.x, a1 = bi ? A1.y : A1.x, a2 = bi ? A2.y : A2.x, a3 = bi ? A3.y : A3.x;
+        if (PAR4) {       // monomial order of k = 4: fg_tables.h (LO/HI pairs by parity; q steps = (j, parity) over the other three)
+          const bool c1 = (c & 1) != 0, c2 = (c & 2) != 0;
+          const double p01 = a0 * a1, p23 = a2 * a3;
+          const double lo0 = c1 ? p01 : 1.0, lo1 = c1 ? a1 : a0, hi0 = c2 ? p23 : 1.0, hi1 = c2 ? a3 : a2;
+          mono[bi][0] = lo0 * hi0; mono[bi][1] = lo1 * hi0; mono[bi][2] = lo0 * hi1; mono[bi][3] = lo1 * hi1;
+          if (QX) {
+            const double q0 = bi ? Q0.y : Q0.x, q1 = bi ? Q1.y : Q1.x, q2 = bi ? Q2.y : Q2.x, q3 = bi ? Q3.y : Q3.x;
+            const double p02 = a0 * a2, p03 = a0 * a3, p12 = a1 * a2, p13 = a1 * a3;
+            // even: {1, r0 r1, r0 r2, r1 r2}[c], odd: {r0 r1 r2, r2, r1, r0}[c] for (r0, r1, r2) = the variables other than j
+#define FG_EO(r0_, r1_, r2_, p01_, p02_, p12_, ev, od) \
+            const double ev = (c == 0) ? 1.0 : (c == 1) ? p01_ : (c == 2) ? p02_ : p12_; \
+            const double od = (c == 0) ? p01_ * r2_ : (c == 1) ? r2_ : (c == 2) ? r1_ : r0_;
+            FG_EO(a1, a2, a3, p12, p13, p23, e0, o0) FG_EO(a0, a2, a3, p02, p03, p23, e1, o1)
+            FG_EO(a0, a1, a3, p01, p03, p13, e2, o2) FG_EO(a0, a1, a2, p01, p02, p12, e3, o3)
+#undef FG_EO
+            mono[bi][4] = q0 * e0; mono[bi][5] = q0 * o0; mono[bi][6] = q1 * e1; mono[bi][7] = q1 * o1;
+            mono[bi][8] = q2 * e2; mono[bi][9] = q2 * o2; mono[bi][10] = q3 * e3; mono[bi][11] = q3 * o3;
+          }
+          continue;
+        }
         const double a01 = a0 * a1;
         const double mlo = (c & 2) ? ((c & 1) ? a01 : a1) : ((c & 1) ? a0 : 1.0);
         double hi[NM]; hi[0] = 1.0;
@@ -100,6 +138,7 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
       for (int bi = 0; bi < NRB; ++bi) { d[bi][0] = 0.0; d[bi][1] = 0.0; }
 #pragma unroll
       for (int st = 0; st < STEPS; ++st) {
+        if (!((SMASK >> st) & 1u)) continue;                         // (compile time) no record of this group has a coefficient in this step
 #if FG_KO & 2
         const double b = __hiloint2double(lane + st, 0);
 #else
@@ -144,13 +183,14 @@ __device__ __noinline__ void run_group_mma_rb(const unsigned char* __restrict__ 
     p += (size_t)ntiles * TILE;
   }
 #pragma unroll
-  for (int bi = 0; bi < NRB; ++bi) { part[bi] = av[bi]; part[NRB + bi] = ab[bi]; }
+  for (int bi = 0; bi < NRB; ++bi) { part.v[bi] = av[bi]; part.v[NRB + bi] = ab[bi]; }
+  return part;
 }
 
 // Running state of one program in the stream kernel.  acc/aab: accumulators of the current destination (owner threads:
 // thread t < FG_ST_SAMPLES owns sample t of the batch); part: per-lane tensor-core partial sums (all threads).
 struct StreamState {
-  double acc[2], aab[2], part[2 * FG_ST_NRB]; int cur, has_part, has_half, has_two;
+  double acc[2], aab[2]; MmaPart part; int cur, has_part, has_half, has_two;
 #ifdef FG_PHASE_PROF
   long long* prof; long long tlast;
 #endif
@@ -159,8 +199,22 @@ struct StreamState {
 // Hand the partial sums to the owner threads.  Tensor-core groups: quad-reduce, lane c == 0 of quad r posts the sums of sample
 // 32*sg + 8*b + r.  Scalar groups: the helper thread t + 256 (which ran the second half of the records of every scalar group
 // on the operands of sample t) posts its accumulators.  The owner adds both.  Block-uniform (every warp walks the same
-// stream), two block barriers (four if two-component records were met); called when the destination changes and at the
+// stream), two pair barriers (four if two-component records were met); called when the destination changes and at the
 // end of a program.  xbuf: [0, 512) tensor-core pairs, [512, 1024) helper pairs.
+#ifndef FG_DECOUPLE
+#define FG_DECOUPLE 1     // 1: warp pairs (w, w + 8) synchronise among themselves, chunk buffers are released by a counter (A/B: 0 = block barriers)
+#endif
+// Everything fold_parts exchanges stays inside a warp pair (w, w + 8): both serve sample group w % 8 (tensor-core partial
+// sums of its 32 samples; helper thread t + 256 mirrors owner t).  A named barrier per pair therefore replaces the
+// block barrier, and the eight pairs drift apart within the slack of the chunk ring: while one pair is in a group
+// prologue or a record epilogue another keeps the FP64 pipe busy.
+__device__ __forceinline__ void pair_sync() {
+#if FG_DECOUPLE
+  asm volatile("bar.sync %0, 64;" ::"r"(1 + (int)((threadIdx.x >> 5) & 7)) : "memory");
+#else
+  __syncthreads();
+#endif
+}
 __device__ __forceinline__ void fold_parts(StreamState& st, double* __restrict__ xbuf) {
   if (!st.has_part && !st.has_half) return;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, sg = w & 7, rb0 = FG_ST_NRB * (w >> 3);
@@ -168,25 +222,25 @@ __device__ __forceinline__ void fold_parts(StreamState& st, double* __restrict__
   if (st.has_part) {
 #pragma unroll
     for (int bi = 0; bi < FG_ST_NRB; ++bi) {
-      double v = st.part[bi], a = st.part[FG_ST_NRB + bi];
+      double v = st.part.v[bi], a = st.part.v[FG_ST_NRB + bi];
       v += __shfl_xor_sync(0xffffffffu, v, 1); a += __shfl_xor_sync(0xffffffffu, a, 1);
       v += __shfl_xor_sync(0xffffffffu, v, 2); a += __shfl_xor_sync(0xffffffffu, a, 2);
       if ((lane & 3) == 0) { const int smp = 32 * sg + 8 * rb0 + 2 * (lane >> 2) + bi; xbuf[2 * smp] = v; xbuf[2 * smp + 1] = a; }      // column map of run_group_mma_rb
-      st.part[bi] = 0.0; st.part[FG_ST_NRB + bi] = 0.0;
+      st.part.v[bi] = 0.0; st.part.v[FG_ST_NRB + bi] = 0.0;
     }
   }
   if (st.has_half && !owner) { xbuf[2 * FG_ST_SAMPLES + 2 * (tid - FG_ST_SAMPLES)] = st.acc[0]; xbuf[2 * FG_ST_SAMPLES + 2 * (tid - FG_ST_SAMPLES) + 1] = st.aab[0]; }
-  __syncthreads();
+  pair_sync();
   if (owner) {
     if (st.has_part) { st.acc[0] += xbuf[2 * tid]; st.aab[0] += xbuf[2 * tid + 1]; }
     if (st.has_half) { st.acc[0] += xbuf[2 * FG_ST_SAMPLES + 2 * tid]; st.aab[0] += xbuf[2 * FG_ST_SAMPLES + 2 * tid + 1]; }
   }
-  __syncthreads();
+  pair_sync();
   if (st.has_two) {        // second component of self-energy elements
     if (!owner) { xbuf[2 * (tid - FG_ST_SAMPLES)] = st.acc[1]; xbuf[2 * (tid - FG_ST_SAMPLES) + 1] = st.aab[1]; }
-    __syncthreads();
+    pair_sync();
     if (owner) { st.acc[1] += xbuf[2 * tid]; st.aab[1] += xbuf[2 * tid + 1]; }
-    __syncthreads();
+    pair_sync();
   }
   if (!owner) { st.acc[0] = st.acc[1] = 0.0; st.aab[0] = st.aab[1] = 0.0; }
   st.has_part = 0; st.has_half = 0; st.has_two = 0;
@@ -218,15 +272,26 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
       // consecutive tensor-core groups of the same class and destination are run by one call (run length and size come
       // from the planner)
       const unsigned char* p0 = p - sizeof(FgGroupHdr); const int nseq = gh.nseq;
-      switch (nf * 8 + k) {
-#define FG_MM(NF, K) case NF * 8 + K: if (qx) run_group_mma_rb<NF, K, true>(p0, nseq, Vw, ne, rb0, st.part); else run_group_mma_rb<NF, K, false>(p0, nseq, Vw, ne, rb0, st.part); break;
-        FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
-        FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
-#undef FG_MM
-        default: break;      // the planner makes tensor-core groups of these classes only
+      const int var = (flags & FG_REC_PAR_A) ? 1 : (flags & FG_REC_PAR_B) ? 2 : 0;
+#define FG_MM(NF, K) case NF * 8 + K: if (qx) st.part = run_group_mma_rb<NF, K, true>(p0, nseq, Vw, ne, rb0, st.part); else st.part = run_group_mma_rb<NF, K, false>(p0, nseq, Vw, ne, rb0, st.part); break;
+#define FG_MP(NF, V) case NF * 8 + V: if (qx) st.part = run_group_mma_rb<NF, 4, true, V>(p0, nseq, Vw, ne, rb0, st.part); else st.part = run_group_mma_rb<NF, 4, false, V>(p0, nseq, Vw, ne, rb0, st.part); break;
+      if (var) {       // k = 4 groups whose coefficients sit in one of the two parity step sets
+        switch (nf * 8 + var) {
+          FG_MP(0, 1) FG_MP(0, 2) FG_MP(1, 1) FG_MP(1, 2) FG_MP(2, 1) FG_MP(2, 2) FG_MP(3, 1) FG_MP(3, 2) FG_MP(4, 1) FG_MP(4, 2) FG_MP(5, 1) FG_MP(5, 2)
+          default: break;
+        }
+      } else {
+        switch (nf * 8 + k) {
+          FG_MM(0, 2) FG_MM(0, 3) FG_MM(0, 4) FG_MM(1, 2) FG_MM(1, 3) FG_MM(1, 4) FG_MM(2, 2) FG_MM(2, 3) FG_MM(2, 4)
+          FG_MM(3, 2) FG_MM(3, 3) FG_MM(3, 4) FG_MM(4, 2) FG_MM(4, 3) FG_MM(4, 4) FG_MM(5, 2) FG_MM(5, 3) FG_MM(5, 4)
+          FG_MM(0, 0) FG_MM(0, 1) FG_MM(1, 0) FG_MM(1, 1) FG_MM(2, 0) FG_MM(2, 1) FG_MM(3, 0) FG_MM(3, 1) FG_MM(4, 0) FG_MM(4, 1) FG_MM(5, 0) FG_MM(5, 1)
+          default: break;      // the planner makes tensor-core groups of these classes only
+        }
       }
-      FG_MARK(st, 9 + (k - 2) * 2 + (qx ? 1 : 0));      // 9..14: tensor-core groups by class (k = 2, 3, 4; without / with q-extension)
-      p = p0 + gh.seq_bytes; g += nseq - 1; continue;
+#undef FG_MM
+#undef FG_MP
+      FG_MARK(st, k < 2 ? 2 : 9 + (k - 2) * 2 + (qx ? 1 : 0));      // 2: k = 0, 1; 9..14: tensor-core groups by class (k = 2, 3, 4; without / with q-extension)
+      p = p0 + (size_t)gh.seq_units * 16; g += nseq - 1; continue;
     }
     const int bytes = nrec * (((flags & FG_REC_WIDE) ? (int)sizeof(FgRecW) : (int)sizeof(FgRecC)) + rec_ncoef(k, flags) * (int)sizeof(double));
     // scalar groups: the owner threads take records [0, half), the helper threads [half, nrec) on the same operands
@@ -236,9 +301,10 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
       bool done = false;
       if (!(flags & (FG_REC_WIDE | FG_REC_TWO))) {
         done = true;
+        AccPair ap; ap.acc = st.acc[0]; ap.aab = st.aab[0];
         switch (nf * 8 + k) {
-#define FG_CLS(NF, K) case NF * 8 + K: if (qx) run_group_static<double, 1, 1, NF, K, true>(p, r1, Vt, vs, ne, &st.acc[0], &st.aab[0], r0); \
-                                        else run_group_static<double, 1, 1, NF, K, false>(p, r1, Vt, vs, ne, &st.acc[0], &st.aab[0], r0); break;
+#define FG_CLS(NF, K) case NF * 8 + K: if (qx) ap = run_group_static_v<NF, K, true>(p, r1, Vt, vs, ne, ap, r0); \
+                                        else ap = run_group_static_v<NF, K, false>(p, r1, Vt, vs, ne, ap, r0); break;
           FG_CLS(0, 0) FG_CLS(0, 1) FG_CLS(0, 2) FG_CLS(0, 3) FG_CLS(0, 4)
           FG_CLS(1, 0) FG_CLS(1, 1) FG_CLS(1, 2) FG_CLS(1, 3) FG_CLS(1, 4)
           FG_CLS(2, 0) FG_CLS(2, 1) FG_CLS(2, 2) FG_CLS(2, 3) FG_CLS(2, 4)
@@ -248,6 +314,7 @@ __device__ __forceinline__ void run_chunk_s(const unsigned char* __restrict__ ch
 #undef FG_CLS
           default: done = false; break;
         }
+        st.acc[0] = ap.acc; st.aab[0] = ap.aab;
       }
       if (done) FG_MARK(st, 3);
       else {

@@ -68,9 +68,11 @@ struct FgTermDev {
 #define FG_REC_QEXT 2      // q-extension tables follow
 #define FG_REC_WIDE 4      // records use the wide header (nf > FG_NFC): generic slow path
 #define FG_REC_MMA 8       // tensor-core group: records that share their free variables, stored as 8-record tiles
+#define FG_REC_PAR_A 16    // tensor-core group, k = 4: coefficients only in the steps of set A (see below)
+#define FG_REC_PAR_B 32    // ... of set B
 #define FG_NFC 5           // product factors of a compact record (= Wick pairs, <= n)
 #ifndef FG_MMA_MINK
-#define FG_MMA_MINK 2      // tensor-core groups only for records with at least this many free variables
+#define FG_MMA_MINK 0      // tensor-core groups only for records with at least this many free variables
 #endif
 #ifndef FG_MMA_MINREC
 #define FG_MMA_MINREC 3    // a run of records with equal free variables becomes a tensor-core group from this length on
@@ -92,10 +94,25 @@ struct alignas(16) FgRecW {   // wide record header, 32 bytes
 static_assert(sizeof(FgRecC) == 16 && sizeof(FgRecW) == 32, "record header sizes");
 // Tensor-core group (FG_REC_MMA): for a fixed set of free variables the record values are a dense contraction
 //   Q[sample][record] = sum_J mono_J(a, a^q)[sample] * coef[J][record]
-// evaluated with DMMA m8n8k4 (8 samples x 4 monomials x 8 records).  Monomial J = 4*step + x:
+// evaluated with DMMA m8n8k4 (8 samples x 4 monomials x 8 records).  Monomial J = 4*step + x.
+// k = 0, 1 (one step): {1, a0, aq0, 0}[x] (whatever of it the class has): long runs of such records (products of beta's
+//   times a constant or a linear factor) go through the record epilogue of the tile path instead of the scalar interpreter.
+// k = 2, 3, 4:
 //   main  steps t < 2^(k-2):        mlo[x] * mhi[t],  mlo = {1, a0, a1, a0 a1}, mhi[t] = prod_{bit i of t} a_{2+i}
 //   low-q steps (q-extension):      {aq0, aq0 a1, aq1, aq1 a0}[x] * mhi[t]
 //   high-q steps, j = 2..k-1:       aq_j * mlo[x] * (product over the subset t' of the other high variables)
+// k = 4, groups flagged FG_REC_PAR_A / FG_REC_PAR_B.  The Dirac traces leave many tables with non-zero coefficients on
+// subsets of ONE parity only (main table and/or the q tables).  With a step order in which every step holds monomials of
+// one parity class,
+//   main  step s = plo + 2 phi:     LO[plo][x & 1] * HI[phi][x >> 1],  LO[0] = {1, a0 a1}, LO[1] = {a0, a1},
+//                                   HI[0] = {1, a2 a3}, HI[1] = {a2, a3}
+//   q     step 4 + 2 j + par:       aq_j * R[par][x] over the other three variables r0 < r1 < r2,
+//                                   R[0] = {1, r0 r1, r0 r2, r1 r2}, R[1] = {r0 r1 r2, r2, r1, r0}
+// a run of records that has no non-zero coefficient outside one of the two step sets met in practice,
+//   with q-extension:    A = main + odd q steps (0xaaf),  B = main + even q steps (0x55f)
+//   without:             A = steps 0, 3 (even subsets, 0x9),  B = steps 1, 2 (odd subsets, 0x6),
+// is stored in that order and flagged, and the kernel issues the DMMAs of that set only (a third to a half fewer).  The
+// tiles still hold every step, zeros included, so the interpreters of the upper rungs only need the order.
 // A tile = 8 x FgRecM (product factors, bound) + steps x 32 FgMmaCoef in B-fragment order (lane = 4*record + x).
 // The coefficients of a tile are stored as the HIGH 32-bit word of the double (sign, exponent, 20 mantissa bits): the
 // planner makes a tensor-core group only of records whose coefficients have a zero low word (integers below 2^21 times
@@ -115,6 +132,14 @@ static inline bool fg_mma_coef_pack(double c, FgMmaCoef* out) {   // host: false
   uint64_t u; __builtin_memcpy(&u, &c, 8); *out = (FgMmaCoef)(uint32_t)(u >> 32); return (u & 0xffffffffull) == 0;
 }
 #define FG_TILE_BYTES(steps) (8 * (int)sizeof(FgRecM) + (steps) * 32 * (int)sizeof(FgMmaCoef))
+#ifndef FG_MMA_PARITY
+#define FG_MMA_PARITY 1                                   // (A/B: 0 never sets FG_REC_PAR_A / FG_REC_PAR_B)
+#endif
+#define FG_MMA_PAR_MASK_A(qx) ((qx) ? 0xaafu : 0x9u)
+#define FG_MMA_PAR_MASK_B(qx) ((qx) ? 0x55fu : 0x6u)
+// subset (bits = variables) of monomial x of a k = 4 step: main steps (bits 0-3 = a0..a3), q steps (bits 0-2 = r0..r2)
+#define FG_MMA4_MAIN_SUBSET(step, x) ((((step) & 1) ? (((x) & 1) ? 2 : 1) : (((x) & 1) ? 3 : 0)) | ((((step) >> 1) ? (((x) >> 1) ? 2 : 1) : (((x) >> 1) ? 3 : 0)) << 2))
+#define FG_MMA4_Q_SUBSET(par, x) ((par) ? (7 ^ ((x) == 0 ? 0 : (x) == 1 ? 3 : (x) == 2 ? 5 : 6)) : ((x) == 0 ? 0 : (x) == 1 ? 3 : (x) == 2 ? 5 : 6))
 // Record header of a tile, 8 bytes: product factors, shared prefix depth, and cab16 = the top 16 bits of the double
 // sum |coef| rounded UP (sign, exponent, 4 mantissa bits: a bound, at most 6 % above the sum).
 struct alignas(8) FgRecM { uint8_t fidx[FG_NFC]; uint8_t keep; uint16_t cab16; };
@@ -126,9 +151,10 @@ static inline double fg_cab16_value(uint32_t c) { const uint64_t u = (uint64_t)c
 static inline uint16_t fg_cab16_pack(double c) {      // host: smallest representable value >= c (c >= 0)
   uint64_t u; __builtin_memcpy(&u, &c, 8); uint64_t top = u >> 48; if (u & 0xffffffffffffull) ++top; return (uint16_t)top;
 }
-// nseq / seq_bytes (tensor-core groups): number and total size of the consecutive groups of the same class and
-// destination that start here inside this chunk (one kernel call runs them all).
-struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint16_t nseq; uint32_t seq_bytes; };
+// Tensor-core groups: grp_units = size of the group's tiles, seq_units = total size (headers included) of the nseq
+// consecutive groups of the same class and destination that start here inside this chunk (one kernel call runs them
+// all); both in units of 16 bytes.
+struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_t vidx[FG_KMAX]; uint16_t nseq, seq_units, grp_units; };
 static_assert(sizeof(FgRecM) == 8 && sizeof(FgGroupHdr) == 16, "group header sizes");
 struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
 
