@@ -46,6 +46,11 @@ typedef struct { int32_t u, v; int32_t kind; } fg_edge;
 int fg_graph_create(const fg_edge* edges, int32_t n_edges, int32_t ext_photon_vertex, fg_graph** out);
 void fg_graph_destroy(fg_graph*);
 
+/* Gauge-invariant class (k, m, m') of a graph (Table I at 397-409): m and m' count the internal photons to
+ * the left and to the right of the external photon along the electron path ("or vice versa": kmm[1] >= kmm[2]), k those
+ * with their ends on opposite sides of it; k + m + m' = n.  kmm: three ints, written by the call.  Host only. */
+int fg_graph_class(const fg_graph*, int32_t* kmm);
+
 /* Plan options.  fg_plan_opts_default fills the Calc-2 constants of PAPER.md:370-377.
  *  C[4]      mixture weights C_1..C_4 of g = sum C_k g_k; must be >= 0 and sum to 1
  *  D         exponent scale of the third component
@@ -189,6 +194,11 @@ int fg_batch_fold(fg_batch*, int32_t graph, const fg_result* block, double secon
 int fg_batch_run(fg_batch*, uint64_t n_blocks, uint64_t block_samples, uint64_t seed, uint64_t sched_seed, void* stream);
 int fg_batch_result(const fg_batch*, int32_t graph, fg_result* out, double* abs_tol, double* seconds_per_sample);
 int fg_batch_total(const fg_batch*, double* value, double* sigma_down, uint64_t* n_total);
+/* Class sums (Table I): fg_batch_set_classes stores a class (k, m, m') for every graph of the batch (3 ints per
+ * graph, e.g. from fg_graph_class; borrowed for the call); fg_batch_class_total returns the value (sum of the means) and
+ * sigma_down by (19) of the graphs of one class and their number (0 graphs: value 0). */
+int fg_batch_set_classes(fg_batch*, const int32_t* kmm_per_graph);
+int fg_batch_class_total(const fg_batch*, const int32_t* kmm, double* value, double* sigma_down, int32_t* n_graphs);
 
 /* ---- parity / debug surface (device kernels; outputs are HOST arrays, any may be NULL) -------------------
  * fg_sample_dump: for samples first..first+n-1: all Philox words (n * M * 4, call-major), mixture component (n),

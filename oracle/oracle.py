@@ -88,6 +88,16 @@ def count_undirected(n):
     return lib().fgo_count_undirected(n)
 
 
+def gauge_class(x, photons):
+    """Class (k, m, m') of PAPER.md:393 (Table I): m, m' = internal photons to the left / right of the external photon
+    (the larger first), k = photons whose ends lie on opposite sides of it.  Plain definition."""
+    left = sum(1 for a, b in photons if max(a, b) < x)
+    right = sum(1 for a, b in photons if min(a, b) > x)
+    k = sum(1 for a, b in photons if min(a, b) < x < max(a, b))
+    assert left + right + k == len(photons)
+    return k, max(left, right), min(left, right)
+
+
 OPS = {0: "A", 1: "U", 2: "L", 3: "L-U"}
 
 

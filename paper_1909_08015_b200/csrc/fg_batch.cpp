@@ -37,6 +37,7 @@ struct GraphState {
   uint64_t next_sample = 0;   // first Philox sample id not yet handed out
   double t = 1.0;             // seconds per sample
   double abs_tol = 0.0;
+  int32_t kmm[3] = {-1, -1, -1};   // gauge-invariant class, set by fg_batch_set_classes
 };
 
 }  // namespace
@@ -178,6 +179,22 @@ int fg_batch_total(const fg_batch* b, double* value, double* sigma_down, uint64_
   if (value) *value = v;
   if (sigma_down) *sigma_down = std::sqrt(s2);     // (19)
   if (n_total) *n_total = n;
+  return FG_OK;
+}
+
+int fg_batch_set_classes(fg_batch* b, const int32_t* kmm_per_graph) {
+  if (!b || !kmm_per_graph) return bfail(FG_E_ARG, "NULL argument");
+  for (size_t j = 0; j < b->g.size(); ++j) for (int i = 0; i < 3; ++i) b->g[j].kmm[i] = kmm_per_graph[3 * j + i];
+  return FG_OK;
+}
+
+int fg_batch_class_total(const fg_batch* b, const int32_t* kmm, double* value, double* sigma_down, int32_t* n_graphs) {
+  if (!b || !kmm) return bfail(FG_E_ARG, "NULL argument");
+  double v = 0.0, s2 = 0.0; int32_t n = 0;
+  for (auto& s : b->g) if (s.kmm[0] == kmm[0] && s.kmm[1] == kmm[1] && s.kmm[2] == kmm[2]) { v += s.sum.mean; s2 += s.sum.variance > 0.0 ? s.sum.variance : 0.0; ++n; }
+  if (value) *value = v;
+  if (sigma_down) *sigma_down = std::sqrt(s2);     // (19) restricted to the class
+  if (n_graphs) *n_graphs = n;
   return FG_OK;
 }
 

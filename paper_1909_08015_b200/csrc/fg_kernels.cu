@@ -615,6 +615,14 @@ int fg_graph_create(const fg_edge* edges, int32_t n_edges, int32_t ext_photon_ve
 }
 void fg_graph_destroy(fg_graph* g) { delete g; }
 
+int fg_graph_class(const fg_graph* g, int32_t* kmm) {      // photons left of / right of / across the external photon
+  if (!g || !kmm) return fail(FG_E_ARG, "NULL argument");
+  int k = 0, left = 0, right = 0;
+  for (auto& ph : g->g.ph) { if (ph[1] < g->g.x) ++left; else if (ph[0] > g->g.x) ++right; else ++k; }
+  kmm[0] = k; kmm[1] = left > right ? left : right; kmm[2] = left > right ? right : left;
+  return FG_OK;
+}
+
 void fg_plan_opts_default(fg_plan_opts* o) {
   if (!o) return;
   std::memset(o, 0, sizeof(*o));

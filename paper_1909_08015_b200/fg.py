@@ -16,7 +16,7 @@ EXPORTS = ["fg_graph_create", "fg_graph_destroy", "fg_plan_opts_default", "fg_pl
            "fg_integrate_async", "fg_result_merge", "fg_sample_dump", "fg_eval_points", "fg_sample_eval_dump",
            "fg_dfma_peak", "fg_dmma_peak", "fg_strerror", "fg_last_error_message", "fg_version",
            "fg_batch_create", "fg_batch_destroy", "fg_batch_pilot", "fg_batch_set_times", "fg_batch_probabilities", "fg_batch_next",
-           "fg_batch_fold", "fg_batch_run", "fg_batch_result", "fg_batch_total",
+           "fg_batch_fold", "fg_batch_run", "fg_batch_result", "fg_batch_total", "fg_batch_set_classes", "fg_batch_class_total", "fg_graph_class",
            "fg_noalloc_setup", "fg_noalloc_limits", "fg_eval_points_dd_noalloc"]
 
 
@@ -90,6 +90,9 @@ def lib():
         L.fg_sample_eval_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp] + [vp] * 3
         L.fg_dfma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.fg_dmma_peak.argtypes = [C.c_int32, C.c_int32, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.fg_graph_class.argtypes = [vp, vp]
+        L.fg_batch_set_classes.argtypes = [vp, vp]
+        L.fg_batch_class_total.argtypes = [vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int32)]
         L.fg_batch_create.argtypes = [vp, C.c_int32, C.POINTER(vp)]
         L.fg_batch_destroy.argtypes = [vp]
         L.fg_batch_pilot.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, C.c_double, vp]
@@ -145,6 +148,12 @@ class Graph:
                 lib().fg_graph_destroy(self.h); self.h = None
         except Exception:
             pass
+
+    def gauge_class(self):
+        """fg_graph_class: (k, m, m') of PAPER.md:393."""
+        kmm = np.zeros(3, dtype=np.int32)
+        _check(lib().fg_graph_class(self.h, _p(kmm)))
+        return tuple(int(v) for v in kmm)
 
 
 class Plan:

@@ -62,3 +62,15 @@ class Batch:
         v = C.c_double(); s = C.c_double(); n = C.c_uint64()
         fg._check(fg.lib().fg_batch_total(self.h, C.byref(v), C.byref(s), C.byref(n)))
         return dict(value=v.value, sigma_down=s.value, n_samples=int(n.value))
+
+    def set_classes(self, classes):
+        """fg_batch_set_classes: one (k, m, m') per graph, e.g. [fg.Graph(...).gauge_class() ...]."""
+        a = np.ascontiguousarray(classes, dtype=np.int32).reshape(len(self.plans), 3)
+        fg._check(fg.lib().fg_batch_set_classes(self.h, fg._p(a)))
+
+    def class_total(self, kmm):
+        """fg_batch_class_total: value, sigma_down by (19) and number of graphs of one class."""
+        a = np.ascontiguousarray(kmm, dtype=np.int32).reshape(3)
+        v = C.c_double(); s = C.c_double(); n = C.c_int32()
+        fg._check(fg.lib().fg_batch_class_total(self.h, fg._p(a), C.byref(v), C.byref(s), C.byref(n)))
+        return dict(value=v.value, sigma_down=s.value, n_graphs=int(n.value))
