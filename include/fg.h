@@ -62,6 +62,10 @@ int fg_graph_class(const fg_graph*, int32_t* kmm);
  *            C_add, C_subI, C_subSE, C_subO (defaults 0.256, 0.839, 0.786, 0.2, 0, 0.2); carried for the paper's rule, not
  *            used by rule 0
  *  deg_table optional host array of 2^M doubles overriding Deg(s); NULL = deg_rule
+ *  rng       pseudorandom generator of the sample stream: 0 = Philox4x32-10 (Calc 2; counter = (sample id,
+ *            call), key = seed), 1 = MRG32k3a (Calc 1; L'Ecuyer 1999): seed -> starting values
+ *            1 + ((seed_lo | seed_hi) (i+1) + 12344) mod (m - 1), i.e. seed 0 is the reference implementation's 12345 x 6,
+ *            and sample s owns outputs 32 s, 32 s + 1, ... of that sequence (jump by powers of the recurrence matrices)
  *  structure_only  fg_host_plan only: stop after subgraphs, forests, terms and the Deg/Z tables (no Dirac tables)
  *  rel_tol, abs_tol  a sample whose estimated round-off error exceeds max(rel_tol*|I|, abs_tol*g) is
  *            re-evaluated in double-double (abs_tol plays the role of sigma/4 in (18))
@@ -76,7 +80,7 @@ typedef struct {
   double err_factor;
   double deg_consts[6];
   int32_t structure_only;
-  int32_t reserved;
+  int32_t rng;
 } fg_plan_opts;
 void fg_plan_opts_default(fg_plan_opts* o);
 

@@ -162,11 +162,49 @@ static double u01(uint32_t w0, uint32_t w1) {
   return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
 }
 
-// the k-th uniform of sample `sid` under `seed`: call index k/2, word pair k%2
-struct UniformStream {
-  uint64_t sid, seed; uint32_t call; uint32_t w[4]; int have;
-  UniformStream(uint64_t sid_, uint64_t seed_) : sid(sid_), seed(seed_), call(0), have(0) {}
+// Second generator: MRG32k3a (L'Ecuyer, Operations Research 47 (1999) 159; named in PAPER.md:365 as the generator of Calc 1):
+//   x1_n = (1403580 x1_{n-2} - 810728 x1_{n-3}) mod m1,  m1 = 2^32 - 209
+//   x2_n = (527612 x2_{n-1} - 1370589 x2_{n-3}) mod m2,  m2 = 2^32 - 22853
+//   u_n  = ((x1_n - x2_n) mod m1) / (m1 + 1), with 0 replaced by m1: u in (0, 1).
+// Reading (the paper uses cuRAND's sub-stream layout, which it does not describe): seed -> the six starting values
+// 1 + ((seed_lo or seed_hi) (i+1) + 12344) mod (m - 1) (seed 0 = the reference implementation's 12345 x 6); sample `sid`
+// owns outputs 32 sid, 32 sid + 1, ... of that sequence.  The jump is the plain matrix power A^(32 sid) by squaring.
+static const uint64_t MRG_M1 = 4294967087ull, MRG_M2 = 4294944443ull;
+struct Mrg32k3a {
+  uint64_t s1[3], s2[3];        // (x_{n-3}, x_{n-2}, x_{n-1}) of the two components
+  explicit Mrg32k3a(uint64_t seed) {
+    for (int i = 0; i < 3; ++i) { s1[i] = 1 + ((seed & 0xffffffffull) * (uint64_t)(i + 1) + 12344ull) % (MRG_M1 - 1); s2[i] = 1 + ((seed >> 32) * (uint64_t)(i + 1) + 12344ull) % (MRG_M2 - 1); }
+  }
   double next() {
+    const uint64_t p1 = (1403580ull * s1[1] + 810728ull * (MRG_M1 - s1[0])) % MRG_M1; s1[0] = s1[1]; s1[1] = s1[2]; s1[2] = p1;
+    const uint64_t p2 = (527612ull * s2[2] + 1370589ull * (MRG_M2 - s2[0])) % MRG_M2; s2[0] = s2[1]; s2[1] = s2[2]; s2[2] = p2;
+    return (double)(p1 > p2 ? p1 - p2 : p1 + MRG_M1 - p2) * 2.328306549295727688e-10;
+  }
+  static void matmul(const uint64_t a[3][3], const uint64_t b[3][3], uint64_t c[3][3], uint64_t m) {
+    uint64_t r[3][3];
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { unsigned __int128 t = 0; for (int k = 0; k < 3; ++k) t += (unsigned __int128)a[i][k] * b[k][j]; r[i][j] = (uint64_t)(t % m); }
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) c[i][j] = r[i][j];
+  }
+  static void advance(uint64_t s[3], const uint64_t A[3][3], uint64_t steps, uint64_t m) {      // s <- A^steps s
+    uint64_t P[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}}, B[3][3];
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) B[i][j] = A[i][j];
+    for (; steps; steps >>= 1) { if (steps & 1) matmul(B, P, P, m); matmul(B, B, B, m); }
+    uint64_t r[3];
+    for (int i = 0; i < 3; ++i) { unsigned __int128 t = 0; for (int k = 0; k < 3; ++k) t += (unsigned __int128)P[i][k] * s[k]; r[i] = (uint64_t)(t % m); }
+    for (int i = 0; i < 3; ++i) s[i] = r[i];
+  }
+  void jump(uint64_t steps) {
+    const uint64_t A1[3][3] = {{0, 1, 0}, {0, 0, 1}, {MRG_M1 - 810728ull, 1403580ull, 0}}, A2[3][3] = {{0, 1, 0}, {0, 0, 1}, {MRG_M2 - 1370589ull, 0, 527612ull}};
+    advance(s1, A1, steps, MRG_M1); advance(s2, A2, steps, MRG_M2);
+  }
+};
+
+// the k-th uniform of sample `sid` under `seed`: call index k/2, word pair k%2 (Philox); output 32 sid + k (MRG32k3a)
+struct UniformStream {
+  uint64_t sid, seed; uint32_t call; uint32_t w[4]; int have; int rng; Mrg32k3a mrg;
+  UniformStream(uint64_t sid_, uint64_t seed_, int rng_ = 0) : sid(sid_), seed(seed_), call(0), have(0), rng(rng_), mrg(seed_) { if (rng == 1) mrg.jump(32ull * sid); }
+  double next() {
+    if (rng == 1) return mrg.next();
     if (have == 0) {
       uint32_t ctr[4] = {(uint32_t)sid, (uint32_t)(sid >> 32), call, 0u};
       uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
@@ -540,7 +578,7 @@ static std::vector<Piece> pieces_for(int op, int sub_type, int comp, bool qpart,
 // The oracle object
 // ------------------------------------------------------------------------------------------
 struct Oracle {
-  Graph g; int merge = 0; int M = 0;
+  Graph g; int merge = 0; int M = 0; int rng = 0;      // rng: 0 Philox4x32-10, 1 MRG32k3a
   std::vector<std::vector<int>> var_lines;       // variable -> global line ids
   std::vector<Sub> subs;                         // subs[0] = G
   std::vector<std::vector<int>> forests;         // member lists (indices into subs), [0] = G
@@ -984,7 +1022,7 @@ struct SampleOut { int comp; uint8_t order[16]; double z[16]; double pdf_mant; i
 
 static void sample_point(const Oracle& o, uint64_t sid, uint64_t seed, SampleOut& out) {
   int M = o.M; size_t full = ((size_t)1 << M) - 1;
-  UniformStream us(sid, seed);
+  UniformStream us(sid, seed, o.rng);
   double uc = us.next();
   int comp = 3; { double c = 0; for (int k = 0; k < 4; ++k) { c = c + o.C[k]; if (uc < c) { comp = k; break; } } }
   out.comp = comp;
@@ -1076,6 +1114,14 @@ void* fgo_create(int n, int x, const int* photons, int merge, const double* C, d
   return o;
 }
 void fgo_destroy(void* h) { delete (Oracle*)h; }
+void fgo_set_rng(void* h, int rng) { ((Oracle*)h)->rng = rng; }
+// raw MRG32k3a outputs number first, first + 1, ... of the sequence of `seed`; by_jump: every output reached by its own
+// matrix power from the seed (else: one jump to `first`, then the recurrence)
+void fgo_mrg32k3a(uint64_t seed, uint64_t first, long n, int by_jump, double* out) {
+  if (by_jump) { for (long i = 0; i < n; ++i) { Mrg32k3a g(seed); g.jump(first + (uint64_t)i); out[i] = g.next(); } return; }
+  Mrg32k3a g(seed); g.jump(first);
+  for (long i = 0; i < n; ++i) out[i] = g.next();
+}
 
 // info: [M, n_subs, n_forests, n_terms, n_geoms, n_nums, total patterns]
 void fgo_info(void* h, long* out) {

@@ -32,6 +32,8 @@ def lib():
         L.fgo_create.restype = C.c_void_p
         L.fgo_create.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_int]
         L.fgo_destroy.argtypes = [C.c_void_p]
+        L.fgo_set_rng.argtypes = [C.c_void_p, C.c_int]
+        L.fgo_mrg32k3a.argtypes = [C.c_uint64, C.c_uint64, C.c_long, C.c_int, C.c_void_p]
         L.fgo_info.argtypes = [C.c_void_p, C.c_void_p]
         L.fgo_subs.argtypes = [C.c_void_p, C.c_void_p]
         L.fgo_terms.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
@@ -88,6 +90,13 @@ def count_undirected(n):
     return lib().fgo_count_undirected(n)
 
 
+def mrg32k3a(seed, first, n, by_jump=False):
+    """Raw MRG32k3a outputs first .. first+n-1 of the sequence of `seed` (seed 0 = L'Ecuyer's 12345 x 6)."""
+    out = np.zeros(n)
+    lib().fgo_mrg32k3a(int(seed), int(first), int(n), int(bool(by_jump)), _p(out))
+    return out
+
+
 def gauge_class(x, photons):
     """Class (k, m, m') of PAPER.md:393 (Table I): m, m' = internal photons to the left / right of the external photon
     (the larger first), k = photons whose ends lie on opposite sides of it.  Plain definition."""
@@ -114,6 +123,7 @@ class Oracle:
         self.h = lib().fgo_create(n, x, _p(ph), int(bool(merge)), _p(c4), float(D), _p(dt), int(bool(printed)), int(structure_only))
         if not self.h:
             raise ValueError("invalid graph")
+        self.rng = 0
         info = np.zeros(8, dtype=np.int64)
         lib().fgo_info(self.h, _p(info))
         self.M, self.n_subs, self.n_forests, self.n_terms, self.n_geoms, self.n_nums, self.n_patterns = map(int, info[:7])
@@ -169,6 +179,10 @@ class Oracle:
         z = np.ascontiguousarray(z, dtype=np.float64).reshape(-1, self.M); out = np.zeros(len(z))
         lib().fgo_eval_abs(self.h, _p(z), len(z), _p(out))
         return out
+
+    def set_rng(self, rng):
+        """0: Philox4x32-10 (Calc 2); 1: MRG32k3a (Calc 1)."""
+        self.rng = int(rng); lib().fgo_set_rng(self.h, int(rng))
 
     def sample(self, seed, first, n):
         M = self.M

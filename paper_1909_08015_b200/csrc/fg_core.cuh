@@ -32,10 +32,35 @@ FG_HD void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uin
 // 53-bit uniform in the open interval (0,1)
 FG_HD double uniform53(uint32_t w0, uint32_t w1) { return ((double)((((uint64_t)w0 << 32) | w1) >> 11) + 0.5) * 0x1p-53; }
 
+// Second stream: MRG32k3a (L'Ecuyer 1999): x1_n = (1403580 x1_{n-2} - 810728 x1_{n-3}) mod (2^32 - 209),
+// x2_n = (527612 x2_{n-1} - 1370589 x2_{n-3}) mod (2^32 - 22853), u = ((x1 - x2) mod m1) / (m1 + 1) in (0, 1).  Sample `sid`
+// owns outputs 32 sid, 32 sid + 1, ...: its state is reached from the seed's with the precomputed powers A^(32 2^j) of the
+// two recurrence matrices, one matrix-vector product mod m per set bit of sid (fg.h, option rng).
+#define FG_MRG_M1 4294967087ull
+#define FG_MRG_M2 4294944443ull
 struct UniformStream {
-  uint64_t sid, seed; uint32_t call, w[4]; int left;
-  FG_HD UniformStream(uint64_t sid_, uint64_t seed_) : sid(sid_), seed(seed_), call(0), left(0) {}
+  uint64_t sid, seed; uint32_t call, w[4]; int left; int rng; uint32_t s1[3], s2[3];
+  FG_HD UniformStream(uint64_t sid_, uint64_t seed_, int rng_ = 0, const uint32_t* __restrict__ jump = nullptr) : sid(sid_), seed(seed_), call(0), left(0), rng(rng_) {
+    if (rng == 1) {
+      for (int i = 0; i < 3; ++i) { s1[i] = (uint32_t)(1ull + ((seed & 0xffffffffull) * (uint64_t)(i + 1) + 12344ull) % (FG_MRG_M1 - 1ull)); s2[i] = (uint32_t)(1ull + ((seed >> 32) * (uint64_t)(i + 1) + 12344ull) % (FG_MRG_M2 - 1ull)); }
+      for (int j = 0; j < FG_MRG_JUMPS && (sid >> j) != 0; ++j) if ((sid >> j) & 1ull) {
+        const uint32_t* A = jump + 18 * j; uint32_t r1[3], r2[3];
+        for (int i = 0; i < 3; ++i) {      // three products below 2^64 / 3 each: reduce every product, then the sum
+          r1[i] = (uint32_t)(((uint64_t)A[3 * i] * s1[0] % FG_MRG_M1 + (uint64_t)A[3 * i + 1] * s1[1] % FG_MRG_M1 + (uint64_t)A[3 * i + 2] * s1[2] % FG_MRG_M1) % FG_MRG_M1);
+          r2[i] = (uint32_t)(((uint64_t)A[9 + 3 * i] * s2[0] % FG_MRG_M2 + (uint64_t)A[9 + 3 * i + 1] * s2[1] % FG_MRG_M2 + (uint64_t)A[9 + 3 * i + 2] * s2[2] % FG_MRG_M2) % FG_MRG_M2);
+        }
+        for (int i = 0; i < 3; ++i) { s1[i] = r1[i]; s2[i] = r2[i]; }
+      }
+    }
+  }
+  FG_HD double next_mrg() {
+    const uint64_t p1 = (1403580ull * s1[1] + 810728ull * (FG_MRG_M1 - s1[0])) % FG_MRG_M1;
+    const uint64_t p2 = (527612ull * s2[2] + 1370589ull * (FG_MRG_M2 - s2[0])) % FG_MRG_M2;
+    s1[0] = s1[1]; s1[1] = s1[2]; s1[2] = (uint32_t)p1; s2[0] = s2[1]; s2[1] = s2[2]; s2[2] = (uint32_t)p2;
+    return (double)(p1 > p2 ? p1 - p2 : p1 + FG_MRG_M1 - p2) * 2.328306549295727688e-10;
+  }
   FG_HD double next() {
+    if (rng == 1) return next_mrg();
     if (left == 0) { philox4x32_10((uint32_t)sid, (uint32_t)(sid >> 32), call++, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w); left = 2; }
     double u = (left == 2) ? uniform53(w[0], w[1]) : uniform53(w[2], w[3]);
     --left; return u;
@@ -52,7 +77,7 @@ struct Sample { double z[FG_MAXM]; uint8_t order[FG_MAXM]; double mant; int ex; 
 
 FG_HD void draw_sample(const FgPlanDev& P, const double* __restrict__ Z1, const double* __restrict__ Z3, uint64_t sid, uint64_t seed, Sample& r) {
   const int M = P.M; const uint32_t full = (1u << M) - 1u;
-  UniformStream us(sid, seed);
+  UniformStream us(sid, seed, P.rng, P.mrg_jump);
   double uc = us.next();
   int comp = 3; { double c = 0.0; for (int k = 0; k < 4; ++k) { c = f_add(c, P.C[k]); if (uc < c) { comp = k; break; } } }
   r.comp = comp;

@@ -515,6 +515,10 @@ __global__ void fg_sample_dump_kernel(const FgPlanDev P, uint64_t first, uint64_
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint64_t sid = first + i; const int M = P.M;
+  if (words && P.rng == 1) {      // MRG32k3a: the integers (x1 - x2) mod m1 (0 -> m1) of outputs 32 sid, 32 sid + 1, ... (u = integer / (m1 + 1))
+    UniformStream us(sid, seed, 1, P.mrg_jump);
+    for (int k = 0; k < 4 * M; ++k) words[i * M * 4 + k] = (uint32_t)(us.next_mrg() * 4294967088.0 + 0.5);
+  } else
   if (words) for (int c = 0; c < M; ++c) { uint32_t w[4]; philox4x32_10((uint32_t)sid, (uint32_t)(sid >> 32), (uint32_t)c, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w); for (int k = 0; k < 4; ++k) words[(i * M + c) * 4 + k] = w[k]; }
   Sample sp; draw_sample(P, P.Z1, P.Z3, sid, seed, sp);
   if (comp) comp[i] = sp.comp;
@@ -650,6 +654,7 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   if (device < 0 || device >= ndev) return fail(FG_E_ARG, "device out of range");
   fg_plan_opts o; if (opts) o = *opts; else fg_plan_opts_default(&o);
   if (o.deg_rule != 0) return fail(FG_E_OPTS, "deg_rule: only rule 0 is available (the paper's Deg algorithm is in its Refs. [42], [32], PAPER.md:250)");
+  if (o.rng != 0 && o.rng != 1) return fail(FG_E_OPTS, "rng: 0 = Philox4x32-10, 1 = MRG32k3a");
   PlanOpts po; for (int k = 0; k < 4; ++k) po.C[k] = o.C[k]; po.D = o.D; po.merge = o.merge_ext_lines ? 1 : 0;
   po.rel_tol = o.rel_tol; po.abs_tol = o.abs_tol; po.err_factor = o.err_factor;
   if (!(po.rel_tol >= 0) || !(po.abs_tol >= 0) || (po.rel_tol == 0 && po.abs_tol == 0)) return fail(FG_E_OPTS, "tolerances: need rel_tol >= 0, abs_tol >= 0, not both 0 (every sample would be rejected)");
@@ -674,6 +679,16 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   UP(H.d_geoms, geoms); UP(H.d_nums, nums); UP(H.d_nodes, nodes); UP(H.d_terms, terms); UP(H.d_geom_num_begin, geom_num_begin);
   UP(H.d_chunks, chunks); UP(H.d_chunk_used, chunk_used); UP(H.Z1, Z1); UP(H.Z3, Z3);
   UP(H.d_geom_voff, geom_voff);
+  D.rng = o.rng;
+  if (o.rng == 1) {      // MRG32k3a: A_c^(32 2^j) mod m_c of the two recurrence matrices, by repeated squaring from A_c^32
+    auto mm = [](const uint64_t* a, const uint64_t* b, uint64_t* c, uint64_t m) { uint64_t r[9]; for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { uint64_t t = 0; for (int k = 0; k < 3; ++k) t = (t + a[3 * i + k] * b[3 * k + j] % m) % m; r[3 * i + j] = t; } for (int i = 0; i < 9; ++i) c[i] = r[i]; };
+    const uint64_t m[2] = {FG_MRG_M1, FG_MRG_M2};
+    uint64_t B[2][9] = {{0, 1, 0, 0, 0, 1, FG_MRG_M1 - 810728ull, 1403580ull, 0}, {0, 1, 0, 0, 0, 1, FG_MRG_M2 - 1370589ull, 0, 527612ull}};
+    for (int c = 0; c < 2; ++c) for (int k = 0; k < 5; ++k) mm(B[c], B[c], B[c], m[c]);      // A^32
+    std::vector<uint32_t> jt((size_t)FG_MRG_JUMPS * 18);
+    for (int j = 0; j < FG_MRG_JUMPS; ++j) for (int c = 0; c < 2; ++c) { for (int i = 0; i < 9; ++i) jt[(size_t)18 * j + 9 * c + i] = (uint32_t)B[c][i]; mm(B[c], B[c], B[c], m[c]); }
+    UP(jt, mrg_jump);
+  }
 #undef UP
   D.vtot = H.vtot; D.vmax = H.vmax;
   const int vmax = H.vmax; p->vmax = vmax;

@@ -158,6 +158,7 @@ struct alignas(16) FgGroupHdr { uint16_t nrec; uint8_t nf, k, flags, dst; uint8_
 static_assert(sizeof(FgRecM) == 8 && sizeof(FgGroupHdr) == 16, "group header sizes");
 struct alignas(16) FgChunkHdr { int32_t ngroups; int32_t pad[3]; };
 
+#define FG_MRG_JUMPS 59      // sample ids below 2^59 (32 outputs per sample)
 // Everything the kernels need, passed by value.
 struct FgPlanDev {
   int32_t n, M, nlines, merge_var;    // merge_var: variable holding the two merged lines, or -1
@@ -173,6 +174,9 @@ struct FgPlanDev {
   int32_t vtot, vmax;                 // rows of all geometries together; of the largest one
   const unsigned char* chunks;        // nchunk * FG_CHUNK_BYTES
   const uint32_t* chunk_used;         // bytes in use of every chunk (multiple of 16): what the TMA copy moves
+  // random numbers
+  int32_t rng, rng_pad;               // 0 Philox4x32-10, 1 MRG32k3a
+  const uint32_t* mrg_jump;           // MRG32k3a: FG_MRG_JUMPS x 2 matrices A_c^(32 2^j) mod m_c, row-major (18 words per j)
   // density
   const double* Z1;                   // 2^M
   const double* Z3;                   // 2^M

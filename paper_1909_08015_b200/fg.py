@@ -33,7 +33,7 @@ class fg_edge(C.Structure):
 class fg_plan_opts(C.Structure):
     _fields_ = [("C", C.c_double * 4), ("D", C.c_double), ("merge_ext_lines", C.c_int32), ("deg_rule", C.c_int32),
                 ("deg_table", C.c_void_p), ("rel_tol", C.c_double), ("abs_tol", C.c_double), ("err_factor", C.c_double),
-                ("deg_consts", C.c_double * 6), ("structure_only", C.c_int32), ("reserved", C.c_int32)]
+                ("deg_consts", C.c_double * 6), ("structure_only", C.c_int32), ("rng", C.c_int32)]
 
 
 class fg_plan_stats(C.Structure):
@@ -160,8 +160,8 @@ class Plan:
     """fg_plan_create (+ fg_plan_info, fg_integrate, ... on the plan)."""
 
     def __init__(self, graph, merge_ext_lines=False, C4=None, D=None, deg_table=None, rel_tol=1e-12, abs_tol=0.0,
-                 err_factor=0.0, device=0, deg_rule=0, deg_consts=None):
-        o = fg_plan_opts(); lib().fg_plan_opts_default(C.byref(o))
+                 err_factor=0.0, device=0, deg_rule=0, deg_consts=None, rng=0):
+        o = fg_plan_opts(); lib().fg_plan_opts_default(C.byref(o)); o.rng = int(rng)
         if C4 is not None:
             for k in range(4):
                 o.C[k] = float(C4[k])
