@@ -122,9 +122,10 @@ def main_reference(args):
     print(json.dumps(line))
 
 
-# DRAM traffic of the dominant kernel from the ncu capture of this build (profiles/r02_stream_kernel_ncu.md):
-# dram__bytes_read.sum + dram__bytes_write.sum per launch divided by the samples of that launch, config-5 graph 0.
-STREAM_KERNEL_DRAM_BYTES_PER_SAMPLE = None
+# DRAM traffic of the dominant kernel from the ncu capture of build cbfb73c (written up in profiles/r02_stream_kernel_ncu.md;
+# a constant here: bench.py reads nothing under profiles/): dram__bytes_read.sum + dram__bytes_write.sum of one launch of
+# fg_stream_kernel divided by the 606208 samples of that launch, config-5 graph 0 (graph 17: 54.1 KB per sample).
+STREAM_KERNEL_DRAM_BYTES_PER_SAMPLE = 3754.0
 
 
 def main_fg(args):
@@ -233,7 +234,7 @@ def main_fg(args):
                        "kernel_ms": {"double_pass": ms_d, "extended_passes": ms_q, "share_double": ms_d / max(ms_d + ms_q, 1e-9)},
                        "exec_tflops_double_pass": execf / (ms_d * 1e-3) / 1e12},
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": traffic,
-                         "traffic_unit": "DRAM bytes per launch of one wave (ncu capture of this build, see profiles/)",
+                         "traffic_unit": "DRAM bytes per launch of fg_stream_kernel over one wave of graph 0 (ncu capture, profiles/r02_stream_kernel_ncu.md; algorithmic bytes: 0)",
                          "kernel": "fg_stream_kernel (with its fg_geom_kernel: the time is that of the double-precision pass, CUDA events around every slab in the timed region)",
                          "peak_source": "fg_dfma_peak measured in this run (MEASURED_PEAKS.json has no FP64 entry)", "dmma_peak": dmma_tf,
                          "frac_executed": execf / (ms_d * 1e-3) / 1e12 / peak_tf},
