@@ -565,7 +565,10 @@ static int fail(int code, const std::string& m) { return fg_internal_fail(code, 
 
 struct fg_graph { Graph g; };
 
-static const int NT_Q = 192, S_Q = 1;     // double-double pass: max threads per block (launch bound), samples per thread
+#ifndef FG_NT_Q
+#define FG_NT_Q 192
+#endif
+static const int NT_Q = FG_NT_Q, S_Q = 1;     // double-double pass: max threads per block (launch bound), samples per thread
 static const int NT_QD = 64;              // quad-double pass
 static const uint64_t SLAB = 1ull << 24;  // samples per slab (bounds the re-evaluation queue)
 static const size_t WAVE_BYTES = (size_t)3 << 30;   // budget of the operand tables one wave of the double pass keeps in HBM
@@ -699,7 +702,14 @@ int fg_plan_create(const fg_graph* g, const fg_plan_opts* opts, int32_t device, 
   // double-double pass: as many warps as the per-sample operand table V (vmax entries) leaves room for in shared memory
   const size_t ring_bytes = 2 * FG_CHUNK_BYTES + 128;
   auto fit = [&](int maxnt, size_t per_thread) { long nt = ((long)smem_max - (long)ring_bytes) / (long)per_thread - FG_VPAD; nt = std::min<long>(maxnt, nt / 32 * 32); return (int)nt; };
-  p->nt_q = fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd));
+  // The upper rungs keep run-time-indexed arrays and spills in local memory (7-14 KB of stack per thread); with the whole
+  // L1 carved out for shared memory every such access goes to L2 and a round crawls (profiles/r02_dd_kernel_ncu.md).  So a
+  // block takes only as many threads as leave ~64 KB of L1 (shared memory <= FG_UPPER_SMEM), but at least 64.
+#ifndef FG_UPPER_SMEM
+#define FG_UPPER_SMEM (148 * 1024)
+#endif
+  auto fit_l1 = [&](int nt, size_t per_thread) { long cap = ((long)FG_UPPER_SMEM - (long)ring_bytes) / (long)per_thread - FG_VPAD; cap = std::max<long>(64, cap / 32 * 32); return (int)std::min<long>(nt, cap); };
+  p->nt_q = fit_l1(fit(NT_Q, (size_t)vmax * S_Q * sizeof(dd)), (size_t)vmax * S_Q * sizeof(dd));
   if (p->nt_q < 32) { fg_plan_destroy(p); return fail(FG_E_LIMIT, "element tables do not fit in shared memory"); }
   p->smem_q = ring_bytes + (size_t)vmax * (p->nt_q * S_Q + FG_VPAD) * sizeof(dd);
   p->nt_qd = fit(NT_QD, (size_t)vmax * sizeof(qd));
