@@ -212,6 +212,23 @@ def test_ranges_shard_and_merge_exactly(fg):       # sharding by sa
     assert again.sum_y[0] == whole.sum_y[0] and again.sum_y2[0] == whole.sum_y2[0]
 
 
+def test_stream_kernel_repeats_bit_for_bit(fg):
+    """The warp pairs of fg_stream_kernel run up to one chunk apart (pair barriers, counter-released chunk ring: DESIGN.md 4);
+    a race between them would show as a run-to-run difference.  Twenty runs of the same ragged range of a 5-loop graph with
+    self-energy children (many programs, geometries and destination changes) must give the same bits; sum_y and sum_y2 are
+    double-double sums over every sample, the counters cover the re-evaluation queues."""
+    x, ph = inputs.config(5)["graphs"][1]
+    plan = fg.plan_for(x, ph, merge_ext_lines=True, rel_tol=0.0, abs_tol=1e-4)
+    ref = None
+    for k in range(20):
+        r = plan.integrate_range(12345, 200000 + 77, 6, raw=True)
+        sig = (r.sum_y[0], r.sum_y[1], r.sum_y2[0], r.sum_y2[1], r.n_flagged, r.n_flagged2, r.n_rejected, r.mean, r.variance)
+        if ref is None:
+            ref = sig
+        assert sig == ref, "run %d differs" % k
+    assert ref[7] == ref[7] and ref[8] > 0.0
+
+
 def test_more_than_one_slab(fg):                   # the integrator works in slabs of 2^24 samples
     plan, _ = pair(fg, *G1)
     n = (1 << 24) + 12345
