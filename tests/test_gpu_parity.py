@@ -324,6 +324,8 @@ def test_config4_ladder_prefix_one_million_samples(fg):
 # ---- config 5 (the configuration bench.py times): M = 14 after the merge of PAPER.md:222 -----------------------------
 CFG5 = inputs.config(5)["graphs"]
 CFG5_SET = [0, 15, 17, 30]      # 2 terms; 40 terms; self-energy children, 1.8e5 records (two-component and wide records); 36 terms
+if os.environ.get("FG_TEST_CONFIG5_SET"):      # other graphs of the batch, e.g. "1,2,6" or "all" (about two minutes of oracle time each; results kept in profiles/)
+    CFG5_SET = list(range(32)) if os.environ["FG_TEST_CONFIG5_SET"] == "all" else [int(t) for t in os.environ["FG_TEST_CONFIG5_SET"].split(",")]
 
 
 @pytest.mark.parametrize("gi", CFG5_SET)
