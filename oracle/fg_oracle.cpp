@@ -490,10 +490,12 @@ static void dirac_matching_table(const std::vector<Tok>& toks, int nslots, int n
     }
   }
   // every weight is a multiple of 1/48 and every trace an integer: the exact value is k/48.
-  // Round the double sum to that rational (one rounding, independent of the order of the pieces).
+  // Round the double sum to that rational (one rounding, independent of the order of the pieces).  The sum carries the
+  // rounding noise of its cancelling pieces (3.7e-6 in these units on config-5 graph 18, whose four nested photons make the
+  // largest traces met so far); the guard only has to tell k/48 from another small denominator (k/96: 0.5 away).
   for (size_t Tm = 0; Tm < nT; ++Tm) {
     double k = std::nearbyint(out[Tm] * 48.0);
-    if (std::fabs(out[Tm] * 48.0 - k) > 1e-6) { std::fprintf(stderr, "fg_oracle: coefficient not a multiple of 1/48\n"); std::abort(); }
+    if (std::fabs(out[Tm] * 48.0 - k) > 1e-3) { std::fprintf(stderr, "fg_oracle: coefficient not a multiple of 1/48\n"); std::abort(); }
     out[Tm] = k / 48.0;
   }
 }
